@@ -1,0 +1,163 @@
+/*
+ * wstack.h -- C ABI of the B200-native w-stacking hot path (arxiv 2301.06061).
+ *
+ * The chain follows the paper's statement of the problem (PAPER.md:66-68 Eq. 2, :76-88 steps 1-5):
+ *
+ *   ws_grid_visibilities   a1 + a2: bin the visibilities by (w-plane, uv-tile) and convolve them onto
+ *                          the stack of w-planes (Eq. 3 at :80)
+ *   ws_fft_planes          a3: one 2-D inverse FFT per w-plane -- cuFFT
+ *   ws_wcorrect_accumulate a4: phase screen exp(2 pi i w_k (sqrt(1-l^2-m^2)-1)) times plane k, summed
+ *                          over planes (PAPER.md:68 Eq. 2, :86)
+ *   ws_dirty_image         a5: real part of the accumulated image
+ *
+ * Conventions (DESIGN.md sections 2-3 give the readings R1-R16 of the paper behind them):
+ *   - All data pointers are DEVICE pointers unless the argument is marked "host".  The caller owns every
+ *     buffer and the stream; the library owns only the opaque plan.  Pointers must be 16-byte aligned.
+ *   - Every call enqueues work on `stream` and returns; buffers must stay alive until the stream drains.
+ *     Only ws_plan_create/destroy, ws_get_bins, ws_async_status and ws_image_from_host synchronise.
+ *   - Every call returns WS_OK (0) or a negative WS_ERR_* code; nothing throws, exits or prints.
+ *     Arguments are validated before any launch.
+ *   - Mesh ("grid") layout: complex64 [n_wplanes][n_pix][n_pix], u fastest, FFT-NATIVE storage order:
+ *     logical cell (j, i)  <->  (v, u) = ((j - N/2) du, (i - N/2) du), du = 1/(N cell_rad), is stored at
+ *     row (j + N/2) mod N, column (i + N/2) mod N, so that the FFT needs no shift pass.  After
+ *     ws_fft_planes logical pixel (q, p) of plane k sits at the same wrapped position.
+ *   - Image layout: complex64 [n_pix][n_pix], CENTRED: pixel (q, p) <-> (m, l) = ((q-N/2), (p-N/2)) cell_rad.
+ *   - One plan per host thread.
+ */
+#ifndef WSTACK_H
+#define WSTACK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WS_VERSION 100
+
+/* error codes */
+#define WS_OK 0
+#define WS_ERR_INVALID_ARG (-1)
+#define WS_ERR_UNSUPPORTED (-2)
+#define WS_ERR_WORKSPACE (-3)   /* workspace too small / record capacity exceeded */
+#define WS_ERR_CUDA (-4)
+#define WS_ERR_CUFFT (-5)
+
+/* ws_grid_visibilities mode */
+#define WS_GRID_ACCUMULATE 0 /* add onto the existing mesh (call ws_grid_zero first); tiles without visibilities untouched */
+#define WS_GRID_OVERWRITE 1  /* the mesh is taken as zero on entry and EVERY cell is written: no ws_grid_zero needed */
+
+/* kernel_type */
+#define WS_KERNEL_GAUSSIAN 0 /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)) */
+
+typedef struct ws_plan ws_plan; /* opaque */
+
+typedef struct ws_params {
+    int32_t n_pix;        /* N: mesh and image side; multiple of 2*tile                                   */
+    int32_t n_wplanes;    /* N_w >= 1                                                                      */
+    int32_t support;      /* S: odd, 1..15; full S x S footprint ("kernel size of 7 cells")    */
+    int32_t kernel_type;  /* WS_KERNEL_GAUSSIAN                                                            */
+    double kernel_param;  /* Gaussian sigma in cells (> 0); 1.0 is the default reading R1                  */
+    double cell_rad;      /* image pixel size in radians (> 0)                                             */
+    double w_min, w_max;  /* w range covered by the planes, wavelengths; w_max > w_min.  Plane k covers    */
+                          /* [w_min + k dw, w_min + (k+1) dw), dw = (w_max-w_min)/N_w, value = midpoint     */
+    int32_t tile;         /* uv-tile side T of the bin key; 0 = auto (32); only 32 is supported            */
+    int32_t device;       /* CUDA device ordinal                                                           */
+    uint32_t flags;       /* reserved, 0                                                                   */
+} ws_params;
+
+/* ---- plan ------------------------------------------------------------------------------------------- */
+/* Validates `p`, selects the device, creates the cuFFT plan (work area NOT allocated: it comes from the
+ * caller's workspace).  *out is NULL on failure. */
+int ws_plan_create(const ws_params* p, ws_plan** out);
+int ws_plan_destroy(ws_plan* plan);
+
+/* ---- sizes: all device memory is allocated by the caller ---------------------------------------------- */
+size_t ws_grid_bytes(const ws_plan* plan);   /* 8 N^2 N_w */
+size_t ws_image_bytes(const ws_plan* plan);  /* 8 N^2     */
+size_t ws_dirty_bytes(const ws_plan* plan);  /* 4 N^2     */
+/* Workspace that is always enough for ws_grid_visibilities with up to max_vis_per_call visibilities
+ * (worst-case halo duplication) and for ws_fft_planes.  A smaller workspace may be passed: the record
+ * capacity is then what fits, and exceeding it is reported by ws_async_status as WS_ERR_WORKSPACE. */
+size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis_per_call);
+/* The least workspace ws_grid_visibilities accepts for max_vis_per_call visibilities when at most
+ * `dup_factor` records per visibility are stored (1.0 .. 4.0; typical data needs (1 + (S-1)/T)^2). */
+size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis_per_call, double dup_factor);
+size_t ws_fft_workspace_bytes(const ws_plan* plan);
+int ws_plan_tile(const ws_plan* plan);       /* T */
+int64_t ws_plan_n_bins(const ws_plan* plan); /* N_w (N/T)^2 */
+
+/* ---- a0: clear the mesh (needed before WS_GRID_ACCUMULATE calls only) ---------------------------------- */
+int ws_grid_zero(ws_plan* plan, void* grid, void* stream);
+
+/* ---- a1 + a2: binning and gridding, Eq. 3 ----------------------------------------------- */
+/* uvw     [n_rows][3] float32: (u, v, w) per (baseline, time) row.
+ * vis     [n_rows][n_chan] complex64 (re, im).      weights [n_rows][n_chan] float32.
+ * freq_hz HOST pointer, [n_chan] doubles, or NULL.  Not NULL: uvw are metres, channel c is scaled by
+ *         freq_hz[c]/c, c = 299792458 m/s.  NULL: uvw are wavelengths shared by the n_chan visibilities
+ *         of the row (the paper's narrow-band mode).
+ * Position rule (bit-exact contract, O2-O4): pu = fma(u, su_c, N/2), i0 = floor(pu + 1/2),
+ * plane k = clamp(floor(fma(w, sw_c, ow))), dropped unless the S x S footprint lies on the mesh;
+ * key = (k nt + j0/T) nt + i0/T, nt = N/T.  Contribution: weight * vis * g(a - fu) g(b - fv) at logical
+ * cell (k, j0 + b, i0 + a), |a|,|b| <= (S-1)/2, fp32.  n_rows * n_chan <= 2^30, n_chan <= 128.
+ * Non-finite uvw is a caller error (undefined).  mode: WS_GRID_ACCUMULATE or WS_GRID_OVERWRITE. */
+int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                         const double* freq_hz, int64_t n_rows, int32_t n_chan, void* grid, int32_t mode,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
+/* The two halves of ws_grid_visibilities as separate calls (same arguments, same workspace): a1 leaves the bins
+ * and the per-tile record lists in `workspace`; a2 consumes them.  ws_grid_visibilities == a1 then a2. */
+int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
+                        size_t workspace_bytes, void* stream);
+int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a3: per-plane un-normalised inverse 2-D FFT, in place -------------------------- */
+/* P_k[q][p] = sum_ji G_k[j][i] exp(+2 pi i ((i-N/2)(p-N/2) + (j-N/2)(q-N/2)) / N) in logical indices. */
+int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a4: w-correction and reduction over planes, Eq. 2 ------------------------------ */
+/* image[q][p] (+)= sum_k exp(2 pi i w_k t) P_k[q][p], t = sqrt(1-l^2-m^2) - 1, w_k = w_min + (k+1/2) dw;
+ * pixels with l^2 + m^2 >= 1 receive 0.  accumulate: 0 overwrite, 1 add to image.
+ * dirty may be NULL; otherwise Re(image) after this call is also written there (float32 [N][N]). */
+int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32_t accumulate, float* dirty,
+                           void* stream);
+
+/* ---- a5: dirty[q][p] = Re image[q][p]; norm_flags must be 0 ---------------------------- */
+int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream);
+
+/* ---- the whole path from HOST buffers (end-to-end entry) ----------------------------------------------- */
+/* uvw_h, vis_h, weights_h, dirty_h are HOST pointers (pinned memory gives asynchronous copies); dev_inputs
+ * is a device scratch of at least 12 n_rows + 12 n_rows n_chan + 64 bytes; grid, image, dirty_d, workspace
+ * are device buffers as above.  Copies the inputs in, runs a1..a5 with WS_GRID_OVERWRITE, copies the dirty
+ * image out and synchronises the stream. */
+int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, const float* weights_h,
+                       const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
+                       size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- parity export of the bins of the LAST ws_grid_visibilities call ----------------------------------- */
+/* Device pointers into that call's workspace, valid until the next call on the plan: keys[n_vis] in input
+ * order (0xFFFFFFFF = dropped), sorted_keys[n_kept] ascending, perm[n_kept] flat visibility indices
+ * (row * n_chan + c) grouped by ascending key -- the order INSIDE a bin is unspecified (atomic slot
+ * assignment) -- and bin_start[n_bins + 1].  Synchronises `stream`.  Any output pointer may be NULL. */
+int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_keys, const uint32_t** perm,
+                const uint32_t** bin_start, int64_t* n_vis, int64_t* n_bins, int64_t* n_dropped,
+                int64_t* n_records, void* stream);
+
+/* Synchronises `stream` and returns the deferred status of the work enqueued so far (record capacity
+ * exceeded -> WS_ERR_WORKSPACE, CUDA fault -> WS_ERR_CUDA). */
+int ws_async_status(ws_plan* plan, void* stream);
+
+/* Number of kernels this library has launched through `plan` since it was created. */
+int64_t ws_launch_count(const ws_plan* plan);
+
+const char* ws_strerror(int code);
+const char* ws_last_error(const ws_plan* plan);
+int ws_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WSTACK_H */

@@ -1,0 +1,8 @@
+"""B200-native w-stacking hot path (arxiv 2301.06061): thin Python binding over the C ABI of include/wstack.h.
+
+PyTorch is used for device memory and streams only; every step runs in libwstack.so (hand-written CUDA for
+sm_100a, cuFFT for the per-plane FFT).  There is no CPU fallback: importing `wstack` fails if the library
+cannot be built or loaded.
+"""
+from .wstack import (WS_GRID_ACCUMULATE, WS_GRID_OVERWRITE, Plan, WStackError, lib, library_path,  # noqa: F401
+                     EXPORTED_SYMBOLS)

@@ -1,0 +1,406 @@
+// Host side of libwstack: the C ABI of include/wstack.h.  Argument validation, the workspace carve-up, the
+// fp64 per-channel constants of the position rule (O1), the cuFFT plan for a3
+// and the sequencing of the kernels in ws_bin.cu / ws_grid.cu / ws_wcorrect.cu.  No device arithmetic here.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ws_internal.h"
+
+namespace {
+
+constexpr double C_LIGHT = 299792458.0;
+constexpr double PI = 3.14159265358979323846264338327950288;
+constexpr int64_t MAX_VIS = (int64_t)1 << 30;
+
+int fail(ws_plan* plan, int code, const char* msg) {
+    if (plan) plan->last_error = msg;
+    return code;
+}
+
+int cuda_fail(ws_plan* plan, cudaError_t e, const char* where) {
+    if (plan) plan->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    return WS_ERR_CUDA;
+}
+
+// Workspace layout for n_vis visibilities and a record capacity.  Head (counters .. block sums) is cleared per call.
+WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) {
+    WsLayout L;
+    const size_t nb = plan->geom.n_bins;
+    const size_t A = 256;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = ws_align_up(off + bytes, A); return o; };
+    L.off_counts_home = take((nb + 1) * 4);
+    L.off_counts_all = take((nb + 1) * 4);
+    L.off_cursor_home = take(nb * 4);
+    L.off_cursor_all = take(nb * 4);
+    L.off_block_sums = take(2 * ((nb + 1) / 4096 + 2) * 4);
+    L.off_keys = take((size_t)n_vis * 4);
+    L.off_perm = take((size_t)n_vis * 4);
+    L.off_sorted_keys = take((size_t)n_vis * 4);
+    L.rec_capacity = rec_capacity;
+    L.item_capacity = (uint32_t)(rec_capacity / WS_CHUNK + 1);
+    L.off_items = take((size_t)L.item_capacity * sizeof(uint4));
+    L.off_records = take((size_t)rec_capacity * sizeof(float4));
+    L.total = off;
+    return L;
+}
+
+// Largest record capacity whose layout fits into `bytes` (0 if even the fixed part does not fit).
+bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out) {
+    WsLayout L0 = make_layout(plan, n_vis, 0);
+    if (L0.total > bytes) return false;
+    const uint64_t want = (uint64_t)n_vis * 4;                      // worst case: every footprint in 4 tiles
+    const size_t spare = bytes - L0.total;
+    // per record: 16 B + 16/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
+    uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 16.0 / WS_CHUNK)) : 0;
+    if (cap > want) cap = want;
+    WsLayout L = make_layout(plan, n_vis, cap);
+    while (L.total > bytes && cap > 0) {
+        cap = cap > 64 ? cap - 64 : 0;
+        L = make_layout(plan, n_vis, cap);
+    }
+    if (L.total > bytes) return false;
+    *out = L;
+    return true;
+}
+
+int make_fft_plan(ws_plan* plan) {
+    const long long n[2] = {plan->prm.n_pix, plan->prm.n_pix};
+    const size_t plane_bytes = (size_t)plan->prm.n_pix * plan->prm.n_pix * 8;
+    // all planes in one batched transform unless its work area is out of proportion; else plane by plane
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const int batch = attempt == 0 ? plan->prm.n_wplanes : 1;
+        cufftHandle h;
+        if (cufftCreate(&h) != CUFFT_SUCCESS) return WS_ERR_CUFFT;
+        size_t work = 0;
+        if (cufftSetAutoAllocation(h, 0) != CUFFT_SUCCESS ||
+            cufftMakePlanMany64(h, 2, const_cast<long long*>(n), nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, batch, &work) !=
+                CUFFT_SUCCESS) {
+            cufftDestroy(h);
+            if (attempt == 0) continue;
+            return WS_ERR_CUFFT;
+        }
+        if (attempt == 0 && batch > 1 && work > 2 * plane_bytes + (64u << 20)) {
+            cufftDestroy(h);
+            continue;
+        }
+        plan->fft = h;
+        plan->fft_ok = true;
+        plan->fft_work_bytes = work;
+        plan->fft_batch = batch;
+        return WS_OK;
+    }
+    return WS_ERR_CUFFT;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ws_version(void) { return WS_VERSION; }
+
+const char* ws_strerror(int code) {
+    switch (code) {
+        case WS_OK: return "ok";
+        case WS_ERR_INVALID_ARG: return "invalid argument";
+        case WS_ERR_UNSUPPORTED: return "unsupported configuration";
+        case WS_ERR_WORKSPACE: return "workspace too small";
+        case WS_ERR_CUDA: return "CUDA error";
+        case WS_ERR_CUFFT: return "cuFFT error";
+    }
+    return "unknown error";
+}
+
+const char* ws_last_error(const ws_plan* plan) { return plan ? plan->last_error.c_str() : ""; }
+
+int ws_plan_create(const ws_params* p, ws_plan** out) {
+    if (!out) return WS_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!p) return WS_ERR_INVALID_ARG;
+    if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
+    if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
+    if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
+    if (p->flags != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
+    if (p->support > 2 * WS_HALO_MAX + 1) return WS_ERR_UNSUPPORTED;
+    if (p->kernel_type != WS_KERNEL_GAUSSIAN) return WS_ERR_UNSUPPORTED;
+    if (p->tile != 0 && p->tile != WS_TILE) return WS_ERR_UNSUPPORTED;
+    if (p->n_pix % (2 * WS_TILE) != 0 || p->n_pix > 32768) return WS_ERR_INVALID_ARG;
+    const uint64_t nt = (uint64_t)p->n_pix / WS_TILE;
+    if (nt * nt * (uint64_t)p->n_wplanes >= 0xFFFFFFFFull / 2) return WS_ERR_UNSUPPORTED;
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || p->device >= n_dev) return WS_ERR_CUDA;
+    if (cudaSetDevice(p->device) != cudaSuccess) return WS_ERR_CUDA;
+    ws_plan* plan = new (std::nothrow) ws_plan();
+    if (!plan) return WS_ERR_CUDA;
+    plan->prm = *p;
+    plan->prm.tile = WS_TILE;
+    WsGeom& g = plan->geom;
+    g.n_pix = p->n_pix;
+    g.n_wplanes = p->n_wplanes;
+    g.support = p->support;
+    g.halo = (p->support - 1) / 2;
+    g.nt = (int32_t)nt;
+    g.n_bins = (uint32_t)(nt * nt * (uint64_t)p->n_wplanes);
+    const double sigma = p->kernel_param;
+    g.tap_c = (float)(-1.4426950408889634 / (2.0 * sigma * sigma));
+    g.norm2 = (float)(1.0 / (2.0 * PI * sigma * sigma));
+    plan->fft_ok = false;
+    plan->launches = 0;
+    plan->last_valid = false;
+    plan->sorted_keys_valid = false;
+    plan->sticky_status = WS_OK;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) {
+        delete plan;
+        return WS_ERR_CUDA;
+    }
+    plan->sm_count = prop.multiProcessorCount;
+    plan->d_status = nullptr;
+    plan->last_ws = nullptr;
+    if (cudaMalloc((void**)&plan->d_status, sizeof(WsStatus)) != cudaSuccess ||
+        cudaMemset(plan->d_status, 0, sizeof(WsStatus)) != cudaSuccess) {
+        delete plan;
+        return WS_ERR_CUDA;
+    }
+    const int rc = make_fft_plan(plan);
+    if (rc != WS_OK) {
+        cudaFree(plan->d_status);
+        delete plan;
+        return rc;
+    }
+    *out = plan;
+    return WS_OK;
+}
+
+int ws_plan_destroy(ws_plan* plan) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (plan->fft_ok) cufftDestroy(plan->fft);
+    if (plan->d_status) cudaFree(plan->d_status);
+    delete plan;
+    return WS_OK;
+}
+
+size_t ws_grid_bytes(const ws_plan* plan) {
+    return plan ? (size_t)8 * plan->prm.n_pix * plan->prm.n_pix * plan->prm.n_wplanes : 0;
+}
+size_t ws_image_bytes(const ws_plan* plan) { return plan ? (size_t)8 * plan->prm.n_pix * plan->prm.n_pix : 0; }
+size_t ws_dirty_bytes(const ws_plan* plan) { return plan ? (size_t)4 * plan->prm.n_pix * plan->prm.n_pix : 0; }
+size_t ws_fft_workspace_bytes(const ws_plan* plan) { return plan ? plan->fft_work_bytes : 0; }
+int ws_plan_tile(const ws_plan* plan) { return plan ? WS_TILE : 0; }
+int64_t ws_plan_n_bins(const ws_plan* plan) { return plan ? (int64_t)plan->geom.n_bins : 0; }
+
+size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_factor) {
+    if (!plan || max_vis < 0 || max_vis > MAX_VIS) return 0;
+    if (!(dup_factor >= 1.0)) dup_factor = 1.0;
+    if (dup_factor > 4.0) dup_factor = 4.0;
+    const uint64_t cap = (uint64_t)std::ceil((double)max_vis * dup_factor) + 64;
+    const size_t a = make_layout(plan, max_vis, cap).total;
+    return a > plan->fft_work_bytes ? a : plan->fft_work_bytes;
+}
+
+size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis) { return ws_workspace_bytes_for(plan, max_vis, 4.0); }
+
+int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
+    if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_zero: null argument");
+    const int rc = ws_launch_zero(plan, grid, ws_grid_bytes(plan), (cudaStream_t)stream);
+    return rc < 0 ? fail(plan, rc, "ws_grid_zero: memset failed") : WS_OK;
+}
+
+int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (n_rows < 0 || n_chan <= 0) return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad n_rows / n_chan");
+    if (n_chan > WS_MAX_CHAN) return fail(plan, WS_ERR_UNSUPPORTED, "ws_bin_visibilities: n_chan > 128");
+    if (n_rows > MAX_VIS || n_rows * n_chan > MAX_VIS)
+        return fail(plan, WS_ERR_UNSUPPORTED, "ws_bin_visibilities: more than 2^30 visibilities in one call");
+    if (!workspace || (n_rows > 0 && (!uvw || !vis || !weights)))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: null pointer");
+    if (((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)workspace) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: pointers must be 16-byte aligned");
+    const int64_t n_vis = n_rows * n_chan;
+    WsLayout L;
+    if (!fit_layout(plan, n_vis, workspace_bytes, &L) || (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
+        return fail(plan, WS_ERR_WORKSPACE, "ws_bin_visibilities: workspace too small (see ws_workspace_bytes_for)");
+
+    // O1: per-channel constants, fp64, in exactly this operation order (the bit-exact bin contract)
+    const ws_params& P = plan->prm;
+    WsChanConsts cc;
+    std::memset(&cc, 0, sizeof(cc));
+    const double dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
+    for (int c = 0; c < n_chan; ++c) {
+        if (freq_hz) {
+            if (!(freq_hz[c] > 0.0) || !std::isfinite(freq_hz[c]))
+                return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad frequency");
+            cc.su[c] = (freq_hz[c] / C_LIGHT) * ((double)P.n_pix * P.cell_rad);
+            cc.sw[c] = (freq_hz[c] / C_LIGHT) / dw;
+        } else {
+            cc.su[c] = (double)P.n_pix * P.cell_rad;
+            cc.sw[c] = 1.0 / dw;
+        }
+    }
+    cc.ow = -P.w_min / dw;
+    cc.half = (double)(P.n_pix / 2);
+
+    plan->last_valid = false;
+    plan->sorted_keys_valid = false;
+    const int rc = ws_launch_bin(plan, L, (char*)workspace, cc, uvw, (const float2*)vis, weights, n_rows, n_chan,
+                                 (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_bin_visibilities: launch failed");
+    plan->launches += rc;
+    plan->last_ws = workspace;
+    plan->last_layout = L;
+    plan->last_n_vis = n_vis;
+    plan->last_valid = true;
+    return WS_OK;
+}
+
+int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!grid || !workspace) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: null pointer");
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: bad mode");
+    if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: grid must be 16-byte aligned");
+    if (!plan->last_valid || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: workspace does not hold the bins of ws_bin_visibilities");
+    const int rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                         const double* freq_hz, int64_t n_rows, int32_t n_chan, void* grid, int32_t mode,
+                         void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: bad mode");
+    const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
+    if (rc != WS_OK) return rc;
+    return ws_grid_binned(plan, grid, mode, workspace, workspace_bytes, stream);
+}
+
+int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_planes: null argument");
+    if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
+        return fail(plan, WS_ERR_WORKSPACE, "ws_fft_planes: workspace smaller than ws_fft_workspace_bytes");
+    if (cufftSetStream(plan->fft, (cudaStream_t)stream) != CUFFT_SUCCESS)
+        return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftSetStream");
+    if (plan->fft_work_bytes > 0 && cufftSetWorkArea(plan->fft, workspace) != CUFFT_SUCCESS)
+        return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftSetWorkArea");
+    // the records of the last grid call share the workspace with the FFT work area
+    plan->last_valid = plan->last_valid && plan->fft_work_bytes == 0;
+    const size_t plane = (size_t)plan->prm.n_pix * plan->prm.n_pix;
+    for (int k = 0; k < plan->prm.n_wplanes; k += plan->fft_batch) {
+        cufftComplex* p = (cufftComplex*)grid + (size_t)k * plane;
+        if (cufftExecC2C(plan->fft, p, p, CUFFT_INVERSE) != CUFFT_SUCCESS)
+            return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftExecC2C");
+    }
+    return WS_OK;
+}
+
+int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32_t accumulate, float* dirty,
+                           void* stream) {
+    if (!plan || !planes || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: null argument");
+    if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: bad flag");
+    if (((uintptr_t)planes | (uintptr_t)image | (uintptr_t)dirty) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: pointers must be 16-byte aligned");
+    const int rc = ws_launch_wcorrect(plan, (const float2*)planes, (float2*)image, accumulate, dirty, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_wcorrect_accumulate: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream) {
+    if (!plan || !image || !dirty) return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: null argument");
+    if (norm_flags != 0) return fail(plan, WS_ERR_UNSUPPORTED, "ws_dirty_image: norm_flags must be 0");
+    if (((uintptr_t)image | (uintptr_t)dirty) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: pointers must be 16-byte aligned");
+    const int rc = ws_launch_dirty(plan, (const float2*)image, dirty, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_dirty_image: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, const float* weights_h,
+                       const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
+                       size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!uvw_h || !vis_h || !weights_h || !dev_inputs || !grid || !image || !dirty_d || !dirty_h || !workspace)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: null argument");
+    if (n_rows <= 0 || n_chan <= 0 || n_rows * n_chan > MAX_VIS)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: bad sizes");
+    const size_t n_vis = (size_t)n_rows * n_chan;
+    const size_t b_uvw = ws_align_up((size_t)n_rows * 12, 16), b_vis = n_vis * 8, b_wt = n_vis * 4;
+    if (dev_inputs_bytes < b_uvw + b_vis + b_wt) return fail(plan, WS_ERR_WORKSPACE, "ws_image_from_host: dev_inputs too small");
+    cudaStream_t st = (cudaStream_t)stream;
+    char* d = (char*)dev_inputs;
+    float* uvw_d = (float*)d;
+    void* vis_d = d + b_uvw;
+    float* wt_d = (float*)(d + b_uvw + b_vis);
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(uvw_d, uvw_h, (size_t)n_rows * 12, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(vis_d, vis_h, b_vis, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(wt_d, weights_h, b_wt, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(plan, e, "ws_image_from_host: H2D copy");
+    int rc = ws_grid_visibilities(plan, uvw_d, vis_d, wt_d, freq_hz, n_rows, n_chan, grid, WS_GRID_OVERWRITE, workspace,
+                                  workspace_bytes, stream);
+    if (rc != WS_OK) return rc;
+    if ((rc = ws_fft_planes(plan, grid, workspace, workspace_bytes, stream)) != WS_OK) return rc;
+    if ((rc = ws_wcorrect_accumulate(plan, grid, image, 0, dirty_d, stream)) != WS_OK) return rc;
+    if ((e = cudaMemcpyAsync(dirty_h, dirty_d, ws_dirty_bytes(plan), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(plan, e, "ws_image_from_host: D2H copy");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(plan, e, "ws_image_from_host: synchronize");
+    return WS_OK;
+}
+
+int ws_async_status(ws_plan* plan, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_async_status: synchronize");
+    WsStatus s;
+    e = cudaMemcpy(&s, plan->d_status, sizeof(s), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_async_status: status read");
+    if (s.overflow)
+        return fail(plan, WS_ERR_WORKSPACE, "record capacity of the workspace exceeded: gridding was skipped");
+    return WS_OK;
+}
+
+int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_keys, const uint32_t** perm,
+                const uint32_t** bin_start, int64_t* n_vis, int64_t* n_bins, int64_t* n_dropped,
+                int64_t* n_records, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!plan->last_valid) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_bins: no bins (no grid call, or workspace reused by the FFT)");
+    cudaStream_t st = (cudaStream_t)stream;
+    char* ws = (char*)plan->last_ws;
+    const WsLayout& L = plan->last_layout;
+    if (sorted_keys && !plan->sorted_keys_valid) {
+        const int rc = ws_launch_sorted_keys(plan, L, ws, st);
+        if (rc < 0) return fail(plan, rc, "ws_get_bins: launch failed");
+        plan->launches += rc;
+        plan->sorted_keys_valid = true;
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_bins: synchronize");
+    WsStatus s;
+    e = cudaMemcpy(&s, plan->d_status, sizeof(s), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_bins: status read");
+    if (keys) *keys = (const uint32_t*)(ws + L.off_keys);
+    if (sorted_keys) *sorted_keys = (const uint32_t*)(ws + L.off_sorted_keys);
+    if (perm) *perm = (const uint32_t*)(ws + L.off_perm);
+    if (bin_start) *bin_start = (const uint32_t*)(ws + L.off_counts_home);
+    if (n_vis) *n_vis = plan->last_n_vis;
+    if (n_bins) *n_bins = (int64_t)plan->geom.n_bins;
+    if (n_dropped) *n_dropped = plan->last_n_vis - (int64_t)s.n_kept;
+    if (n_records) *n_records = (int64_t)s.n_records;
+    if (s.overflow) return fail(plan, WS_ERR_WORKSPACE, "record capacity of the workspace exceeded: gridding was skipped");
+    return WS_OK;
+}
+
+int64_t ws_launch_count(const ws_plan* plan) { return plan ? plan->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,85 @@
+// Internal declarations shared by the translation units of libwstack (CUDA product path only).
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+
+#include "../../include/wstack.h"
+
+#define WS_TILE 32            // T: uv-tile side of the bin key, one warp owns one tile-plane
+#define WS_MAX_CHAN 128       // per-channel constants travel as a kernel parameter
+#define WS_CHUNK 1024         // records a warp accumulates in shared memory before it flushes
+#define WS_HALO_MAX 7         // (S-1)/2 for S <= 15
+#define WS_WC_GROUP 8          // planes per Horner block in the w-correction (exact restart between blocks)
+
+// Per-channel position constants (O1): fp64, computed on the host exactly as the header states.
+struct WsChanConsts {
+    double su[WS_MAX_CHAN];   // cells per stored-uvw unit
+    double sw[WS_MAX_CHAN];   // planes per stored-uvw unit
+    double ow;                // plane offset = -w_min / dw
+    double half;              // N/2
+};
+
+// Geometry the binning and gridding kernels need.
+struct WsGeom {
+    int32_t n_pix, n_wplanes, support, halo;   // N, N_w, S, h
+    int32_t nt;                                 // N / T
+    uint32_t n_bins;                            // N_w nt^2
+    float tap_c;                                // -log2(e) / (2 sigma^2): g(x) = norm1 * 2^(tap_c x^2)
+    float norm2;                                // 1 / (2 pi sigma^2): product of the two 1-D normalisations
+};
+
+// Workspace carve-up for one ws_grid_visibilities call (all offsets 256-byte aligned).
+struct WsLayout {
+    size_t off_counts_home, off_counts_all;     // [n_bins + 1] u32 each: histogram -> exclusive scan (bin_start / rec_start)
+    size_t off_cursor_home, off_cursor_all;     // [n_bins] u32: running slot cursors of the scatter
+    size_t off_block_sums;                      // scan scratch
+    size_t off_keys, off_perm, off_sorted_keys; // [n_vis] u32 each
+    size_t off_items;                           // heavy-chunk work items (uint4)
+    size_t off_records;                         // float4 records
+    size_t total;                               // bytes used for capacity `rec_capacity`
+    uint64_t rec_capacity;                      // records that fit
+    uint32_t item_capacity;
+};
+
+struct WsStatus {                               // device-side, 64 bytes
+    uint32_t n_kept;                            // kept visibilities (home histogram total)
+    uint32_t n_records;                         // records incl. halo copies
+    uint32_t n_items;                           // heavy chunks queued
+    uint32_t overflow;                          // 1: record or item capacity exceeded, gridding skipped
+    uint32_t pad[12];
+};
+
+struct ws_plan {
+    ws_params prm;
+    WsGeom geom;
+    int sm_count;
+    cufftHandle fft;
+    bool fft_ok;
+    size_t fft_work_bytes;
+    int fft_batch;                              // planes per cufftExec call
+    int64_t launches;
+    std::string last_error;
+    // state of the last grid call (for ws_get_bins)
+    void* last_ws;
+    WsLayout last_layout;
+    int64_t last_n_vis;
+    bool last_valid;
+    bool sorted_keys_valid;
+    int sticky_status;
+    WsStatus* d_status;                         // plan-owned 64-byte device block: totals and the overflow flag
+};
+
+static inline size_t ws_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- launchers (each returns the number of kernels it launched, or a negative WS_ERR_*) ----------------
+int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
+                  const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
+int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);
+int ws_launch_sorted_keys(ws_plan* plan, const WsLayout& L, char* ws, cudaStream_t st);
+int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
+                       cudaStream_t st);
+int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, cudaStream_t st);
+int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);

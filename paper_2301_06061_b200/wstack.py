@@ -1,0 +1,247 @@
+"""ctypes binding of libwstack.so -- argument marshalling only (same names as include/wstack.h)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+WS_GRID_ACCUMULATE = 0
+WS_GRID_OVERWRITE = 1
+
+EXPORTED_SYMBOLS = [
+    "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_grid_bytes",
+    "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
+    "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
+    "ws_wcorrect_accumulate", "ws_dirty_image", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_launch_count",
+]
+
+
+class WStackError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libwstack error {code}: {msg}")
+        self.code = code
+
+
+class _Params(C.Structure):
+    _fields_ = [("n_pix", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.c_int32), ("kernel_type", C.c_int32),
+                ("kernel_param", C.c_double), ("cell_rad", C.c_double), ("w_min", C.c_double), ("w_max", C.c_double),
+                ("tile", C.c_int32), ("device", C.c_int32), ("flags", C.c_uint32)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Loads (building if needed) libwstack.so.  Raises if that is impossible: there is no fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, i32, i64, u32, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_size_t
+    sig = {
+        "ws_version": (C.c_int, []),
+        "ws_strerror": (C.c_char_p, [C.c_int]),
+        "ws_last_error": (C.c_char_p, [vp]),
+        "ws_plan_create": (C.c_int, [C.POINTER(_Params), C.POINTER(vp)]),
+        "ws_plan_destroy": (C.c_int, [vp]),
+        "ws_grid_bytes": (sz, [vp]), "ws_image_bytes": (sz, [vp]), "ws_dirty_bytes": (sz, [vp]),
+        "ws_workspace_bytes": (sz, [vp, i64]),
+        "ws_workspace_bytes_for": (sz, [vp, i64, C.c_double]),
+        "ws_fft_workspace_bytes": (sz, [vp]),
+        "ws_plan_tile": (C.c_int, [vp]), "ws_plan_n_bins": (i64, [vp]),
+        "ws_grid_zero": (C.c_int, [vp, vp, vp]),
+        "ws_grid_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, i32, vp, sz, vp]),
+        "ws_bin_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp]),
+        "ws_grid_binned": (C.c_int, [vp, vp, i32, vp, sz, vp]),
+        "ws_fft_planes": (C.c_int, [vp, vp, vp, sz, vp]),
+        "ws_wcorrect_accumulate": (C.c_int, [vp, vp, vp, i32, vp, vp]),
+        "ws_dirty_image": (C.c_int, [vp, vp, vp, u32, vp]),
+        "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
+        "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
+                                  C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
+        "ws_async_status": (C.c_int, [vp, vp]),
+        "ws_launch_count": (i64, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _stream(stream) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> int:
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise ValueError(f"{name}: expected a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def _freq(freq_hz: Optional[Sequence[float]], n_chan: int):
+    if freq_hz is None:
+        return None, None
+    arr = (C.c_double * n_chan)(*[float(f) for f in freq_hz])
+    return arr, C.cast(arr, C.POINTER(C.c_double))
+
+
+class Plan:
+    """An imaging plan (ws_plan).  All buffers are torch CUDA tensors owned by the caller."""
+
+    def __init__(self, n_pix: int, n_wplanes: int, support: int, cell_rad: float, w_min: float, w_max: float,
+                 sigma: float = 1.0, tile: int = 0, device: int = 0):
+        self._h = C.c_void_p()
+        prm = _Params(n_pix, n_wplanes, support, 0, sigma, cell_rad, w_min, w_max, tile, device, 0)
+        rc = lib().ws_plan_create(C.byref(prm), C.byref(self._h))
+        if rc != 0:
+            self._h = C.c_void_p()
+            raise WStackError(rc, lib().ws_strerror(rc).decode())
+        self.n_pix, self.n_wplanes, self.support, self.device = n_pix, n_wplanes, support, device
+
+    # -- plumbing ---------------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise WStackError(rc, lib().ws_last_error(self._h).decode() or lib().ws_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().ws_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- sizes ------------------------------------------------------------------------------------------
+    @property
+    def tile(self) -> int:
+        return lib().ws_plan_tile(self._h)
+
+    @property
+    def n_bins(self) -> int:
+        return lib().ws_plan_n_bins(self._h)
+
+    def grid_bytes(self) -> int:
+        return lib().ws_grid_bytes(self._h)
+
+    def image_bytes(self) -> int:
+        return lib().ws_image_bytes(self._h)
+
+    def workspace_bytes(self, max_vis: int, dup_factor: Optional[float] = None) -> int:
+        if dup_factor is None:
+            return lib().ws_workspace_bytes(self._h, max_vis)
+        return lib().ws_workspace_bytes_for(self._h, max_vis, dup_factor)
+
+    def fft_workspace_bytes(self) -> int:
+        return lib().ws_fft_workspace_bytes(self._h)
+
+    def launch_count(self) -> int:
+        return lib().ws_launch_count(self._h)
+
+    # -- allocation helpers (torch owns the memory) ------------------------------------------------------
+    def alloc_grid(self) -> torch.Tensor:
+        return torch.empty((self.n_wplanes, self.n_pix, self.n_pix), dtype=torch.complex64, device=f"cuda:{self.device}")
+
+    def alloc_image(self) -> torch.Tensor:
+        return torch.empty((self.n_pix, self.n_pix), dtype=torch.complex64, device=f"cuda:{self.device}")
+
+    def alloc_dirty(self) -> torch.Tensor:
+        return torch.empty((self.n_pix, self.n_pix), dtype=torch.float32, device=f"cuda:{self.device}")
+
+    def alloc_workspace(self, max_vis: int, dup_factor: Optional[float] = None) -> torch.Tensor:
+        n = self.workspace_bytes(max_vis, dup_factor)
+        return torch.empty((n + 255) // 256 * 256, dtype=torch.uint8, device=f"cuda:{self.device}")
+
+    # -- the chain --------------------------------------------------------------------------------------
+    def grid_zero(self, grid: torch.Tensor, stream=None):
+        self._check(lib().ws_grid_zero(self._h, _dev(grid, torch.complex64, "grid"), _stream(stream)))
+
+    def grid_visibilities(self, uvw, vis, weights, freq_hz, grid, workspace, mode: int = WS_GRID_OVERWRITE, stream=None):
+        n_rows = int(uvw.shape[0])
+        n_chan = int(vis.shape[1]) if vis.dim() == 2 else 1
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_grid_visibilities(
+            self._h, _dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"),
+            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan, _dev(grid, torch.complex64, "grid"), mode,
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+        self._ws = workspace
+
+    def bin_visibilities(self, uvw, vis, weights, freq_hz, workspace, stream=None):
+        n_rows = int(uvw.shape[0])
+        n_chan = int(vis.shape[1]) if vis.dim() == 2 else 1
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_bin_visibilities(
+            self._h, _dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"),
+            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan,
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+        self._ws = workspace
+
+    def grid_binned(self, grid, workspace, mode: int = WS_GRID_OVERWRITE, stream=None):
+        self._check(lib().ws_grid_binned(self._h, _dev(grid, torch.complex64, "grid"), mode,
+                                         _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def fft_planes(self, grid, workspace, stream=None):
+        self._check(lib().ws_fft_planes(self._h, _dev(grid, torch.complex64, "grid"),
+                                        _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def wcorrect_accumulate(self, planes, image, accumulate: bool = False, dirty=None, stream=None):
+        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
+        self._check(lib().ws_wcorrect_accumulate(self._h, _dev(planes, torch.complex64, "planes"),
+                                                 _dev(image, torch.complex64, "image"), int(accumulate), d,
+                                                 _stream(stream)))
+
+    def dirty_image(self, image, dirty, stream=None):
+        self._check(lib().ws_dirty_image(self._h, _dev(image, torch.complex64, "image"),
+                                         _dev(dirty, torch.float32, "dirty"), 0, _stream(stream)))
+
+    def image_from_host(self, uvw_h, vis_h, weights_h, freq_hz, dev_inputs, grid, image, dirty_d, dirty_h, workspace,
+                        stream=None):
+        """The whole path from HOST tensors (pinned for asynchronous copies) to a host dirty image."""
+        for t, dt, nm in ((uvw_h, torch.float32, "uvw_h"), (vis_h, torch.complex64, "vis_h"),
+                          (weights_h, torch.float32, "weights_h"), (dirty_h, torch.float32, "dirty_h")):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != dt:
+                raise ValueError(f"{nm}: expected a contiguous host tensor of {dt}")
+        n_rows, n_chan = int(uvw_h.shape[0]), int(vis_h.shape[1])
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_image_from_host(
+            self._h, uvw_h.data_ptr(), vis_h.data_ptr(), weights_h.data_ptr(), fp, n_rows, n_chan,
+            _dev(dev_inputs, torch.uint8, "dev_inputs"), dev_inputs.numel(), _dev(grid, torch.complex64, "grid"),
+            _dev(image, torch.complex64, "image"), _dev(dirty_d, torch.float32, "dirty_d"), dirty_h.data_ptr(),
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def async_status(self, stream=None):
+        self._check(lib().ws_async_status(self._h, _stream(stream)))
+
+    def get_bins(self, stream=None) -> dict:
+        """Bins of the last grid call as numpy arrays (copied to the host): keys, sorted_keys, perm, bin_start,
+        n_vis, n_bins, n_dropped, n_records."""
+        p = [C.c_void_p() for _ in range(4)]
+        n = [C.c_int64() for _ in range(4)]
+        self._check(lib().ws_get_bins(self._h, *[C.byref(x) for x in p], *[C.byref(x) for x in n], _stream(stream)))
+        n_vis, n_bins, n_dropped, n_records = (int(x.value) for x in n)
+        ws = self._ws
+        base = ws.data_ptr()
+
+        def view(ptr, count):
+            off = ptr.value - base
+            return ws[off: off + 4 * count].view(torch.int32).cpu().numpy().view(np.uint32)
+
+        n_kept = n_vis - n_dropped
+        return dict(keys=view(p[0], n_vis), sorted_keys=view(p[1], n_kept), perm=view(p[2], n_kept),
+                    bin_start=view(p[3], n_bins + 1), n_vis=n_vis, n_bins=n_bins, n_dropped=n_dropped,
+                    n_records=n_records)

@@ -1,0 +1,169 @@
+"""GPU parity: the CUDA path through the C ABI against the fp64 oracle, element by element (-m gpu)."""
+import numpy as np
+import pytest
+import torch
+
+from synth import get_config, make_dataset, make_random_dataset
+
+from . import gpu_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+def _np(d):
+    return d.uvw.numpy(), d.vis.numpy(), d.weights.numpy(), d.freqs_hz
+
+
+def _full_check(oracle, d, **kw):
+    out = U.run_chain(d, **kw)
+    prm = U.oracle_params(oracle, d, out["plan"].tile)
+    U.check_bins(oracle, prm, d, out["bins"])
+    D, G = oracle.dirty_image(prm, *_np(d), return_grid=True)
+    eg = U.assert_close(out["grid"], G, "grid")
+    ei = U.assert_close(out["image"], D, "image")
+    assert np.array_equal(out["dirty"], out["image"].real)
+    return out, eg, ei
+
+
+def test_library_loaded_is_the_cuda_one():
+    import paper_2301_06061_b200 as ws
+    assert ws.lib().ws_version() == 100
+    assert torch.cuda.is_available()
+
+
+def test_tiny_config(oracle):
+    d = make_dataset(get_config("tiny"))
+    out, eg, ei = _full_check(oracle, d)
+    print("tiny grid/image errors", eg, ei)
+    assert out["plan"].launch_count() >= 9
+
+
+@pytest.mark.parametrize("support", [1, 3, 5, 7, 9, 11, 13, 15])
+def test_random_all_supports_with_drops_and_channels(oracle, support):
+    # fill > 1: some visibilities fall off the mesh (drop rule); 3 channels in metres + frequencies
+    d = make_random_dataset(100 + support, 4000, 3, 256, 5, support, wavelengths=False, fill=1.03, w_span=70.0,
+                            cell_rad=2e-3)
+    out, _, _ = _full_check(oracle, d)
+    assert out["bins"]["n_dropped"] > 0
+
+
+def test_plane_count_not_multiple_of_group_and_wide_field(oracle):
+    # N_w = 11 (ragged last Horner block); cell so large that corner pixels have l^2 + m^2 >= 1 (R14)
+    d = make_random_dataset(7, 3000, 1, 128, 11, 7, fill=0.9, w_span=20.0, cell_rad=0.012)
+    out, _, _ = _full_check(oracle, d)
+    assert out["image"][0, 0] == 0 and out["image"][64, 64] != 0
+
+
+def test_heavy_bin_is_chunked(oracle):
+    # 6000 visibilities inside one 32 x 32 tile of one plane: > WS_CHUNK, so the reduce-add kernel runs
+    d = make_random_dataset(8, 6000, 1, 256, 2, 7, fill=0.05, w_span=1.0, cell_rad=1e-3)
+    d.uvw[:, 2] = 0.3
+    d.w_min, d.w_max = -1.0, 1.0
+    out, _, _ = _full_check(oracle, d)
+    counts = np.diff(out["bins"]["bin_start"].astype(np.int64))
+    assert counts.max() > 1024
+
+
+def test_empty_input_writes_zeros(oracle):
+    d = make_random_dataset(9, 0, 1, 128, 3, 7)
+    out = U.run_chain(d)
+    assert not np.any(out["grid"]) and not np.any(out["image"])
+    assert out["bins"]["n_vis"] == 0 and out["bins"]["n_dropped"] == 0
+
+
+def test_all_dropped(oracle):
+    d = make_random_dataset(10, 500, 1, 128, 3, 7, fill=0.9)
+    d.uvw[:, 0] = 0.8 / d.cell_rad        # everything outside the mesh (its edge is at 0.5 / cell_rad)
+    out = U.run_chain(d)
+    assert out["bins"]["n_dropped"] == 500 and not np.any(out["grid"])
+
+
+def test_accumulate_mode_equals_one_shot(oracle):
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(11, 9000, 2, 256, 4, 7, wavelengths=False, fill=0.98, w_span=40.0, cell_rad=1.5e-3)
+    plan = U.make_plan(d)
+    dev = d.to("cuda")
+    grid = plan.alloc_grid()
+    wsp = plan.alloc_workspace(d.n_vis)
+    plan.grid_zero(grid)
+    for lo, hi in ((0, 2000), (2000, 2000), (2000, 9000)):      # includes an empty chunk
+        plan.grid_visibilities(dev.uvw[lo:hi].contiguous(), dev.vis[lo:hi].contiguous(),
+                               dev.weights[lo:hi].contiguous(), d.freqs_hz, grid, wsp, mode=ws.WS_GRID_ACCUMULATE)
+    plan.async_status()
+    prm = U.oracle_params(oracle, d, plan.tile)
+    G = oracle.grid(prm, *_np(d))
+    U.assert_close(U.logical(grid), G, "accumulated grid")
+
+
+def test_wcorrect_accumulate_flag_and_fused_dirty(oracle):
+    d = make_random_dataset(12, 10, 1, 128, 9, 7, w_span=300.0, cell_rad=4e-3)
+    plan = U.make_plan(d)
+    rng = np.random.default_rng(5)
+    P = (rng.standard_normal((9, 128, 128)) + 1j * rng.standard_normal((9, 128, 128))).astype(np.complex64)
+    prm = U.oracle_params(oracle, d, plan.tile)
+    ref = oracle.wcorrect(prm, P.astype(np.complex128))
+    stored = torch.fft.ifftshift(torch.from_numpy(P).cuda(), dim=(-2, -1)).contiguous()
+    image, dirty = plan.alloc_image(), plan.alloc_dirty()
+    plan.wcorrect_accumulate(stored, image, accumulate=False, dirty=dirty)
+    U.assert_close(image.cpu().numpy(), ref, "w-correction")
+    assert np.array_equal(dirty.cpu().numpy(), image.cpu().numpy().real)
+    plan.wcorrect_accumulate(stored, image, accumulate=True)
+    U.assert_close(image.cpu().numpy(), 2 * ref, "w-correction, accumulate")
+
+
+def test_fft_planes_matches_oracle_transform(oracle):
+    d = make_random_dataset(13, 10, 1, 256, 3, 7)
+    plan = U.make_plan(d)
+    rng = np.random.default_rng(6)
+    G = (rng.standard_normal((3, 256, 256)) + 1j * rng.standard_normal((3, 256, 256))).astype(np.complex64)
+    stored = torch.fft.ifftshift(torch.from_numpy(G).cuda(), dim=(-2, -1)).contiguous()
+    wsp = plan.alloc_workspace(16)
+    plan.fft_planes(stored, wsp)
+    got = U.logical(stored)
+    for k in range(3):
+        U.assert_close(got[k], oracle.fft2(G[k].astype(np.complex128)), f"fft plane {k}")
+
+
+def test_small_workspace_reports_overflow(oracle):
+    import paper_2301_06061_b200 as ws
+    # every visibility near a tile corner: 4 records each; a workspace sized for 1.0 records per visibility overflows
+    d = make_random_dataset(14, 2000, 1, 128, 1, 7, fill=0.9)
+    d.uvw[:, :2] = torch.round(d.uvw[:, :2] * (128 * d.cell_rad) / 32) * 32 / (128 * d.cell_rad)
+    plan = U.make_plan(d)
+    dev = d.to("cuda")
+    grid = plan.alloc_grid()
+    wsp = plan.alloc_workspace(d.n_vis, dup_factor=1.0)
+    plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp)
+    with pytest.raises(ws.WStackError) as e:
+        plan.async_status()
+    assert e.value.code == -3
+    out = U.run_chain(d)            # the default (worst-case) workspace works
+    prm = U.oracle_params(oracle, d, plan.tile)
+    U.assert_close(out["grid"], oracle.grid(prm, *_np(d)), "corner grid")
+    assert out["bins"]["n_records"] > 3 * (d.n_vis - out["bins"]["n_dropped"])
+
+
+def test_argument_validation():
+    import paper_2301_06061_b200 as ws
+    for bad in (dict(n_pix=250), dict(support=8), dict(support=17), dict(w_max=-5.0), dict(cell_rad=0.0), dict(tile=64)):
+        kw = dict(n_pix=256, n_wplanes=4, support=7, cell_rad=1e-3, w_min=-1.0, w_max=1.0)
+        kw.update(bad)
+        with pytest.raises(ws.WStackError):
+            ws.Plan(**kw)
+    plan = ws.Plan(256, 4, 7, 1e-3, -1.0, 1.0)
+    grid = plan.alloc_grid()
+    tiny_ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    uvw = torch.zeros((10, 3), device="cuda")
+    vis = torch.zeros((10, 1), dtype=torch.complex64, device="cuda")
+    wt = torch.ones((10, 1), device="cuda")
+    with pytest.raises(ws.WStackError) as e:
+        plan.grid_visibilities(uvw, vis, wt, None, grid, tiny_ws)
+    assert e.value.code == -3
+    with pytest.raises(ws.WStackError):
+        plan.grid_visibilities(uvw, vis, wt, None, grid, plan.alloc_workspace(10), mode=7)
+
+
+def test_small_config(oracle):
+    d = make_dataset(get_config("small"))
+    out, eg, ei = _full_check(oracle, d)
+    print("small grid/image errors", eg, ei)
