@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""Benchmark of the w-stacking hot path (BASELINE.json metric: Mvis/s and image wall time on one B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over the synthetic workload, inputs resident in HBM:
+a1 bin -> a2 grid (WS_GRID_OVERWRITE: every mesh cell written, no memset) -> a3 cuFFT per plane -> a4 fused
+w-correction + accumulation (also writes a5, the real dirty image).  Prints ONE JSON line (rank 0).
+N > 1 runs N independent replicas (the path is built for one GPU, "replicas only").
+`--impl reference` times the fp64 CPU oracle on a bounded sample of the same workload (see cpu_baseline()).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from synth import get_config, make_dataset  # noqa: E402
+
+METRIC = "Mvis/s through the whole w-stacking path (bin+grid+FFT+w-correct) on 1 B200"
+UNIT = "Mvis/s"
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_params(orc, d, tile=32):
+    return orc.OracleParams(n_pix=d.n_pix, n_wplanes=d.n_wplanes, support=d.support, cell_rad=d.cell_rad,
+                            w_min=d.w_min, w_max=d.w_max, sigma=d.sigma_cells, tile=tile)
+
+
+def cpu_baseline(d, n_sample_planes=2):
+    """The fp64 oracle as it stands, plane-streamed like oracle.dirty_image, timed on the host cores on a bounded
+    sample: `n_sample_planes` of the N_w planes (each plane pass = place + grid all visibilities onto that plane,
+    transform it, w-correct it); the whole-workload time is the sample time x N_w / n_sample_planes."""
+    from oracle import wstack_oracle as orc
+    prm = oracle_params(orc, d)
+    uvw, vis, wt = d.uvw.cpu().numpy(), d.vis.cpu().numpy(), d.weights.cpu().numpy()
+    n_s = min(n_sample_planes, d.n_wplanes)
+    planes = sorted(set(int(round((i + 0.5) * d.n_wplanes / n_s - 0.5)) for i in range(n_s)))
+    D = np.zeros((d.n_pix, d.n_pix), np.complex128)
+    t0 = time.perf_counter()
+    for k in planes:
+        G = orc.grid(prm, uvw, vis, wt, d.freqs_hz, k, k + 1)
+        orc.wcorrect(prm, orc.transform(G[0])[None], k, D)
+    dt = time.perf_counter() - t0
+    full = dt * d.n_wplanes / len(planes)
+    return {"value": d.n_vis / full / 1e6, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"planes {planes} of {d.n_wplanes} (all {d.n_vis} visibilities placed per plane pass, fp64 grid + "
+                      f"radix-2 FFT + w-correction of those planes): {dt:.1f} s, whole workload extrapolated x"
+                      f"{d.n_wplanes / len(planes):.0f} = {full:.0f} s",
+            "sample_seconds": dt}
+
+
+def run_reference(args, d, cfg_name):
+    n_planes = 2 if args.steps + args.warmup <= 6 else 1
+    for _ in range(args.warmup):
+        cpu_baseline(d, n_planes)
+    vals = [cpu_baseline(d, n_planes) for _ in range(args.steps)]
+    v = float(np.mean([x["value"] for x in vals]))
+    cb = dict(vals[-1]); cb["value"] = v
+    ms = d.n_vis / (v * 1e6) * 1e3
+    return {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(d, cfg_name),
+            "cpu_baseline": cb, "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def workload_config(d, cfg_name):
+    return {"workload": f"{cfg_name}: {d.n_vis} visibilities ({d.n_rows} rows x {d.n_chan} channels), "
+                        f"{d.n_pix}x{d.n_pix} complex64 mesh, {d.n_wplanes} w-planes, Gaussian support {d.support}",
+            "n_vis": d.n_vis, "n_pix": d.n_pix, "n_wplanes": d.n_wplanes, "support": d.support,
+            "l2": "inputs (%.2f GB) and mesh (%.1f GB) larger than the 126 MB L2; no flush needed" %
+                  ((12 * d.n_rows + 12 * d.n_vis) / 1e9, 8.0 * d.n_pix ** 2 * d.n_wplanes / 1e9)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="large")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = get_config(args.config)
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        dev = f"cuda:{local_rank}" if torch.cuda.is_available() else "cpu"
+        d = make_dataset(cfg, device=dev).to("cpu")
+        print(json.dumps(run_reference(args, d, cfg.name)), flush=True)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    import paper_2301_06061_b200 as ws
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+
+    d = make_dataset(cfg, device=f"cuda:{local_rank}")
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank)
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis)
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+        if ev: ev[1].record()
+        plan.grid_binned(grid, wsp, mode=ws.WS_GRID_OVERWRITE)
+        if ev: ev[2].record()
+        plan.fft_planes(grid, wsp)
+        if ev: ev[3].record()
+        plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
+        if ev: ev[4].record()
+
+    for _ in range(args.warmup):
+        step()
+    plan.async_status()
+    bins_info = None
+    plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+    b = plan.get_bins(fields=("bin_start",))
+    bins_info = {"n_dropped": b["n_dropped"], "n_records": b["n_records"],
+                 "max_bin": int(np.diff(b["bin_start"].astype(np.int64)).max()),
+                 "empty_bins_frac": float((np.diff(b["bin_start"].astype(np.int64)) == 0).mean())}
+    n_records = b["n_records"]
+    del b
+
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    clocks = ClockSampler(local_rank)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    clocks.start()
+    l0 = plan.launch_count()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for i in range(args.steps):
+        step(evs[i])
+    t_end.record()
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    launches = plan.launch_count() - l0
+    clk = clocks.stop()
+    total_ms = t_start.elapsed_time(t_end)
+    if dist:
+        t = torch.tensor([total_ms], device=f"cuda:{local_rank}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    plan.async_status()
+    ms_step = total_ms / args.steps
+    st = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])     # bin, grid, fft, wcorrect
+    med = np.median(st, axis=0)
+    value = world * d.n_vis / (ms_step * 1e-3) / 1e6
+
+    # ---- roofline of the dominant own kernel (algorithmic bytes) ---------------------
+    peak, peak_src = peaks()
+    mesh_b = 8.0 * d.n_pix ** 2 * d.n_wplanes
+    alg = {"k_grid_tiles": mesh_b + 16.0 * n_records,                        # every cell written once + records read
+           "k_wcorrect": mesh_b + 8.0 * d.n_pix ** 2 + 4.0 * d.n_pix ** 2}   # planes read once + image + dirty written
+    times = {"k_grid_tiles": med[1], "k_wcorrect": med[3]}
+    dom = max(times, key=times.get)
+    ach = alg[dom] / (times[dom] * 1e-3) / 1e9
+    roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
+            "launch_ms": float(times[dom])}
+    b_path = 12.0 * d.n_rows + 12.0 * d.n_vis + 2 * mesh_b + 8.0 * d.n_pix ** 2
+    t_path = med[0] + med[1] + med[3]
+    roof_path = {"what": "a1+a2+a4 (path without the library FFT), SURVEY 8(d) B_alg(path)", "bytes": b_path,
+                 "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
+                 "frac_of_measured_peak": b_path / (t_path * 1e-3) / 1e9 / peak,
+                 "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+           "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
+           "stages_ms_median": {"bin": float(med[0]), "grid": float(med[1]), "fft_cufft": float(med[2]),
+                                "wcorrect": float(med[3])},
+           "mvis_per_s_gridding": d.n_vis / ((med[0] + med[1]) * 1e-3) / 1e6,
+           "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
+           "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "roofline_path": roof_path}
+
+    # ---- end to end through the C ABI with HOST buffers --------------------------------------------------
+    if not args.no_e2e:
+        uvw_h, vis_h, wt_h = (t.cpu().pin_memory() for t in (d.uvw, d.vis, d.weights))
+        dirty_h = torch.empty((d.n_pix, d.n_pix), dtype=torch.float32).pin_memory()
+        dev_in = torch.empty(12 * d.n_rows + 12 * d.n_vis + 256, dtype=torch.uint8, device=f"cuda:{local_rank}")
+        k_e2e = max(2, min(args.steps, 5))
+        plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+        torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) / k_e2e * 1e3
+        if dist:
+            t = torch.tensor([e2e_ms], device=f"cuda:{local_rank}")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        out["e2e"] = {"value": world * d.n_vis / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": e2e_ms,
+                      "h2d_bytes_per_step": 12 * d.n_rows + 12 * d.n_vis, "d2h_bytes_per_step": 4 * d.n_pix ** 2,
+                      "steps": k_e2e, "checksum": float(dirty_h[d.n_pix // 2, d.n_pix // 2])}
+        del dev_in
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        del grid, image, dirty, wsp
+        torch.cuda.empty_cache()
+        out["cpu_baseline"] = cpu_baseline(d.to("cpu"))
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -40,7 +40,7 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) 
     L.off_perm = take((size_t)n_vis * 4);
     L.off_sorted_keys = take((size_t)n_vis * 4);
     L.rec_capacity = rec_capacity;
-    L.item_capacity = (uint32_t)(rec_capacity / WS_CHUNK + 1);
+    L.item_capacity = (uint32_t)(2 * rec_capacity / WS_CHUNK + 2);   // sum of ceil(cnt/CHUNK) over bins with cnt > CHUNK
     L.off_items = take((size_t)L.item_capacity * sizeof(uint4));
     L.off_records = take((size_t)rec_capacity * sizeof(float4));
     L.total = off;
@@ -53,8 +53,8 @@ bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out)
     if (L0.total > bytes) return false;
     const uint64_t want = (uint64_t)n_vis * 4;                      // worst case: every footprint in 4 tiles
     const size_t spare = bytes - L0.total;
-    // per record: 16 B + 16/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
-    uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 16.0 / WS_CHUNK)) : 0;
+    // per record: 16 B + 32/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
+    uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 32.0 / WS_CHUNK)) : 0;
     if (cap > want) cap = want;
     WsLayout L = make_layout(plan, n_vis, cap);
     while (L.total > bytes && cap > 0) {
@@ -197,7 +197,7 @@ size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_f
     if (!(dup_factor >= 1.0)) dup_factor = 1.0;
     if (dup_factor > 4.0) dup_factor = 4.0;
     const uint64_t cap = (uint64_t)std::ceil((double)max_vis * dup_factor) + 64;
-    const size_t a = make_layout(plan, max_vis, cap).total;
+    const size_t a = make_layout(plan, max_vis, cap).total + 4096;   // slack for fit_layout's alignment margin
     return a > plan->fft_work_bytes ? a : plan->fft_work_bytes;
 }
 

@@ -44,32 +44,72 @@ __device__ __forceinline__ uint32_t bin_of(const WsGeom& g, int k, int ty, int t
     return ((uint32_t)k * (uint32_t)g.nt + (uint32_t)ty) * (uint32_t)g.nt + (uint32_t)tx;
 }
 
+// Warp-aggregated counting (the dense core of the uv plane, sends a large share of all
+// visibilities to a few bins; one atomic per visibility serialises on those addresses).  The lanes of a warp
+// that share the home bin are found with ONE match.any; the lanes among them that also share a neighbour tile
+// (same side) follow from ballots.  Each group elects its lowest lane, which adds the group's size.
+struct Groups {
+    unsigned home, nx, ny, nc;     // peer masks: home bin, x-neighbour, y-neighbour, corner neighbour (0 if none)
+};
+__device__ __forceinline__ Groups warp_groups(uint32_t home, int dx, int dy) {
+    Groups q;
+    q.home = __match_any_sync(0xffffffffu, home);
+    const unsigned xm = __ballot_sync(0xffffffffu, dx < 0), xp = __ballot_sync(0xffffffffu, dx > 0);
+    const unsigned ym = __ballot_sync(0xffffffffu, dy < 0), yp = __ballot_sync(0xffffffffu, dy > 0);
+    const unsigned sx = dx < 0 ? xm : (dx > 0 ? xp : 0u), sy = dy < 0 ? ym : (dy > 0 ? yp : 0u);
+    q.nx = q.home & sx;
+    q.ny = q.home & sy;
+    q.nc = q.home & sx & sy;
+    return q;
+}
+__device__ __forceinline__ bool leads(unsigned group, int lane) { return group && lane == __ffs(group) - 1; }
+__device__ __forceinline__ uint32_t rank_in(unsigned group, int lane) { return (uint32_t)__popc(group & ((1u << lane) - 1u)); }
+
+__device__ __forceinline__ void row_chan(uint32_t m, uint32_t n_chan, int chan_shift, uint32_t& row, uint32_t& c) {
+    if (chan_shift >= 0) {
+        row = m >> chan_shift;
+        c = m & (n_chan - 1u);
+    } else {
+        row = m / n_chan;
+        c = m - row * n_chan;
+    }
+}
+
 // ---- pass A: keys + histograms -------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
-            const float* __restrict__ uvw, uint32_t n_vis, uint32_t n_chan,
+            const float* __restrict__ uvw, uint32_t n_vis, uint32_t n_chan, int chan_shift,
             uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_all) {
     const uint32_t m = blockIdx.x * 256u + threadIdx.x;
-    if (m >= n_vis) return;
-    const uint32_t row = m / n_chan, c = m - row * n_chan;
-    const float* p = uvw + 3ull * row;
+    const int lane = threadIdx.x & 31;
     Placed pl;
-    if (!place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl)) {
-        keys[m] = 0xFFFFFFFFu;
-        return;
+    bool kept = false;
+    if (m < n_vis) {
+        uint32_t row, c;
+        row_chan(m, n_chan, chan_shift, row, c);
+        const float* p = uvw + 3ull * row;
+        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl);
     }
-    const int tx = pl.i0 >> T_LOG2, ty = pl.j0 >> T_LOG2;
-    const int lx = pl.i0 & (T - 1), ly = pl.j0 & (T - 1);
-    const uint32_t home = bin_of(g, pl.k, ty, tx);
-    keys[m] = home;
-    atomicAdd(counts_home + home, 1u);
-    // tiles the footprint overlaps: own, and the neighbour on each side it sticks out of
-    const int dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
-    const int dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-    atomicAdd(counts_all + home, 1u);
-    if (dx) atomicAdd(counts_all + bin_of(g, pl.k, ty, tx + dx), 1u);
-    if (dy) atomicAdd(counts_all + bin_of(g, pl.k, ty + dy, tx), 1u);
-    if (dx && dy) atomicAdd(counts_all + bin_of(g, pl.k, ty + dy, tx + dx), 1u);
+    uint32_t home = 0xFFFFFFFFu;
+    int tx = 0, ty = 0, dx = 0, dy = 0, k = 0;
+    if (kept) {
+        tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
+        const int lx = pl.i0 & (T - 1), ly = pl.j0 & (T - 1);
+        home = bin_of(g, k, ty, tx);
+        // tiles the footprint overlaps: own, and the neighbour on each side it sticks out of
+        dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
+        dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
+    }
+    if (m < n_vis) keys[m] = home;
+    const Groups q = warp_groups(home, dx, dy);
+    if (kept && leads(q.home, lane)) {
+        const uint32_t n = (uint32_t)__popc(q.home);
+        atomicAdd(counts_home + home, n);
+        atomicAdd(counts_all + home, n);
+    }
+    if (leads(q.nx, lane)) atomicAdd(counts_all + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
+    if (leads(q.ny, lane)) atomicAdd(counts_all + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
+    if (leads(q.nc, lane)) atomicAdd(counts_all + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
 }
 
 // ---- exclusive prefix scan over n entries of two arrays (blockIdx.y selects), in place ------------------
@@ -175,62 +215,73 @@ k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t* __r
 __global__ void __launch_bounds__(256)
 k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
           const float* __restrict__ uvw, const float2* __restrict__ vis, const float* __restrict__ wt,
-          uint32_t n_vis, uint32_t n_chan, uint32_t* __restrict__ cursor_home, uint32_t* __restrict__ cursor_all,
-          uint32_t* __restrict__ perm, float4* __restrict__ records, const WsStatus* __restrict__ status) {
+          uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home,
+          uint32_t* __restrict__ cursor_all, uint32_t* __restrict__ perm, float4* __restrict__ records,
+          const WsStatus* __restrict__ status) {
     if (status->overflow) return;
     const uint32_t m = blockIdx.x * 256u + threadIdx.x;
-    if (m >= n_vis) return;
-    const uint32_t row = m / n_chan, c = m - row * n_chan;
-    const float* p = uvw + 3ull * row;
+    const int lane = threadIdx.x & 31;
     Placed pl;
-    if (!place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl)) return;
-    const int tx = pl.i0 >> T_LOG2, ty = pl.j0 >> T_LOG2;
-    const int lx = pl.i0 & (T - 1), ly = pl.j0 & (T - 1);
-    const uint32_t home = bin_of(g, pl.k, ty, tx);
-    perm[atomicAdd(cursor_home + home, 1u)] = m;
+    bool kept = false;
+    if (m < n_vis) {
+        uint32_t row, c;
+        row_chan(m, n_chan, chan_shift, row, c);
+        const float* p = uvw + 3ull * row;
+        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl);
+    }
+    uint32_t home = 0xFFFFFFFFu;
+    int tx = 0, ty = 0, lx = 0, ly = 0, dx = 0, dy = 0, k = 0;
+    float2 v = make_float2(0.f, 0.f);
+    float w = 0.f;
+    if (kept) {
+        v = __ldcs(vis + m);
+        w = __ldcs(wt + m);
+        tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
+        lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
+        home = bin_of(g, k, ty, tx);
+        dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
+        dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
+    }
+    // slots: every group leader issues its atomics back to back, the results are broadcast afterwards
+    const Groups q = warp_groups(home, dx, dy);
+    uint32_t bh = 0, ba = 0, bx = 0, by = 0, bc = 0;
+    if (kept && leads(q.home, lane)) {
+        const uint32_t n = (uint32_t)__popc(q.home);
+        bh = atomicAdd(cursor_home + home, n);
+        ba = atomicAdd(cursor_all + home, n);
+    }
+    if (leads(q.nx, lane)) bx = atomicAdd(cursor_all + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
+    if (leads(q.ny, lane)) by = atomicAdd(cursor_all + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
+    if (leads(q.nc, lane)) bc = atomicAdd(cursor_all + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
 
-    const float2 v = __ldg(vis + m);
-    const float wn = __ldg(wt + m) * g.norm2;
-    uint32_t qx = __double2uint_rn(__dadd_rn(pl.fu, 0.5) * 16777216.0);
-    uint32_t qy = __double2uint_rn(__dadd_rn(pl.fv, 0.5) * 16777216.0);
-    qx = qx > 0xFFFFFFu ? 0xFFFFFFu : qx;
-    qy = qy > 0xFFFFFFu ? 0xFFFFFFu : qy;
-    const float vr = v.x * wn, vi = v.y * wn;
-    const int dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
-    const int dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-        const int ddx = (t & 1) ? dx : 0, ddy = (t & 2) ? dy : 0;
-        if (((t & 1) && !dx) || ((t & 2) && !dy)) continue;
-        const uint32_t b = bin_of(g, pl.k, ty + ddy, tx + ddx);
-        const uint32_t slot = atomicAdd(cursor_all + b, 1u);
-        // centre cell relative to the receiving tile's origin: lx - ddx*T (negative wraps into the signed byte)
+    uint32_t qx = 0, qy = 0;
+    float vr = 0.f, vi = 0.f;
+    if (kept) {
+        const float wn = w * g.norm2;
+        qx = __double2uint_rn(__dadd_rn(pl.fu, 0.5) * 16777216.0);
+        qy = __double2uint_rn(__dadd_rn(pl.fv, 0.5) * 16777216.0);
+        qx = qx > 0xFFFFFFu ? 0xFFFFFFu : qx;
+        qy = qy > 0xFFFFFFu ? 0xFFFFFFu : qy;
+        vr = v.x * wn; vi = v.y * wn;
+    }
+    const int lh = __ffs(q.home) - 1;
+    bh = __shfl_sync(0xffffffffu, bh, lh) + rank_in(q.home, lane);
+    ba = __shfl_sync(0xffffffffu, ba, lh) + rank_in(q.home, lane);
+    bx = __shfl_sync(0xffffffffu, bx, q.nx ? __ffs(q.nx) - 1 : lane) + rank_in(q.nx, lane);
+    by = __shfl_sync(0xffffffffu, by, q.ny ? __ffs(q.ny) - 1 : lane) + rank_in(q.ny, lane);
+    bc = __shfl_sync(0xffffffffu, bc, q.nc ? __ffs(q.nc) - 1 : lane) + rank_in(q.nc, lane);
+    if (!kept) return;
+    // centre cell relative to the receiving tile's origin: lx - ddx*T (negative wraps into the signed byte)
+    auto emit = [&](uint32_t slot, int ddx, int ddy) {
         const uint32_t X = ((uint32_t)(lx - ddx * T) << 24) | qx;
         const uint32_t Y = ((uint32_t)(ly - ddy * T) << 24) | qy;
         records[slot] = make_float4(__uint_as_float(X), __uint_as_float(Y), vr, vi);
-    }
-}
-
-// ---- heavy bins: every chunk after the first becomes a work item of the reduce-add kernel ---------------
-__global__ void __launch_bounds__(256)
-k_build_items(const uint32_t* __restrict__ rec_start, uint32_t n_bins, uint4* __restrict__ items,
-              uint32_t item_capacity, WsStatus* __restrict__ status) {
-    const uint32_t b = blockIdx.x * 256u + threadIdx.x;
-    if (b >= n_bins || status->overflow) return;
-    const uint32_t s = rec_start[b], e = rec_start[b + 1];
-    const uint32_t cnt = e - s;
-    if (cnt <= WS_CHUNK) return;
-    const uint32_t extra = (cnt - 1) / WS_CHUNK;
-    const uint32_t base = atomicAdd(&status->n_items, extra);
-    if (base + extra > item_capacity) {
-        status->overflow = 1u;
-        return;
-    }
-    for (uint32_t i = 0; i < extra; ++i) {
-        const uint32_t lo = s + (i + 1) * WS_CHUNK;
-        const uint32_t hi = lo + WS_CHUNK < e ? lo + WS_CHUNK : e;
-        items[base + i] = make_uint4(b, lo, hi, 0u);
-    }
+    };
+    perm[bh] = m;
+    emit(ba, 0, 0);
+    if (q.nx) emit(bx, dx, 0);
+    if (q.ny) emit(by, 0, dy);
+    if (q.nc) emit(bc, dx, dy);
 }
 
 // ---- parity export: sorted_keys[] expanded from bin_start (run lengths) ---------------------------------
@@ -256,9 +307,11 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     WsStatus* status = plan->d_status;
     uint32_t* keys = (uint32_t*)(ws + L.off_keys);
     uint32_t* perm = (uint32_t*)(ws + L.off_perm);
-    uint4* items = (uint4*)(ws + L.off_items);
     float4* records = (float4*)(ws + L.off_records);
     int launches = 0;
+    int chan_shift = -1;   // log2(n_chan) when it is a power of two: row = m >> shift instead of a division
+    for (int b = 0; b < 8; ++b)
+        if (n_chan == (1 << b)) chan_shift = b;
 
     // the counters are contiguous at the head of the workspace: one clear, plus the plan's status block
     if (cudaMemsetAsync(ws, 0, L.off_keys, st) != cudaSuccess) return WS_ERR_CUDA;
@@ -267,7 +320,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     const uint32_t n_scan = g.n_bins + 1;
     const uint32_t n_blocks = (n_scan + SCAN_BLOCK - 1) / SCAN_BLOCK;
     if (n_vis) {
-        k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, keys, counts_home,
+        k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, chan_shift, keys, counts_home,
                                                          counts_all);
         ++launches;
     }
@@ -277,12 +330,10 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
                                                              block_sums, n_blocks, status, L.rec_capacity);
     launches += 3;
     if (n_vis) {
-        k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, cursor_home,
+        k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift, cursor_home,
                                                        cursor_all, perm, records, status);
         ++launches;
     }
-    k_build_items<<<(g.n_bins + 255) / 256, 256, 0, st>>>(counts_all, g.n_bins, items, L.item_capacity, status);
-    ++launches;
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return launches;
 }

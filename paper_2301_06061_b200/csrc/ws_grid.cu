@@ -8,16 +8,19 @@
 //     plain LDS / FFMA / STS (the lanes of a warp cover distinct taps of one visibility, so there are no
 //     collisions and no atomics), and writes it ONCE with coalesced stores -- in WS_GRID_OVERWRITE mode the
 //     tile (zeros included) is simply stored, so the mesh needs no memset and no read-modify-write;
-//   * taps are evaluated in registers: lane (a, b) computes g(a - fu) and g(b - fv) itself (ex2.approx);
-//   * bins with more than WS_CHUNK records are cut into chunks; chunk 0 is handled as above, the others are
-//     work items of k_grid_items, which adds its tile with vector red.global.add.f32x2.
+//   * taps are evaluated in registers, 32 visibilities at a time (lane r evaluates the 2 S taps of record r
+//     with ex2.approx and parks them in shared memory), then lane (a, b) of the warp applies tap (a, b) of
+//     one record after the other;
+//   * a bin with more than WS_CHUNK records ("heavy": the dense core of the uv plane) is cut
+//     into chunks that become work items of their own; k_prepare_heavy queues them and clears their tiles,
+//     and the chunks are added with vector red.global.add.f32x2.  Tiles and items are interleaved in ONE
+//     persistent kernel so that the store stream of the (mostly empty) tiles overlaps the arithmetic of the
+//     dense ones.
 #include "ws_internal.h"
 
 namespace {
 
 constexpr int T = WS_TILE;
-constexpr int GRID_WARPS = 8;                 // warps per CTA
-constexpr int GRID_THREADS = GRID_WARPS * 32;
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -32,7 +35,11 @@ struct TileCfg {
     static constexpr int R = 32 / S;                // footprint rows a warp covers per round
     static constexpr int NR = (S + R - 1) / R;      // rounds per visibility
     static constexpr int TILE_CELLS = T * P;
-    static constexpr size_t WARP_BYTES = (size_t)TILE_CELLS * sizeof(float2) + 32 * sizeof(float4);
+    // per warp: tile | meta[32] float4 | gu[32][S] | gv[32][S]
+    static constexpr size_t WARP_BYTES =
+        ((size_t)TILE_CELLS * sizeof(float2) + 32 * sizeof(float4) + 2 * 32 * S * sizeof(float) + 15) / 16 * 16;
+    static constexpr int WARPS = (113 * 1024) / WARP_BYTES >= 8 ? 8 : (int)((113 * 1024) / WARP_BYTES);
+    static constexpr int THREADS = WARPS * 32;
 };
 
 // storage origin (FFT-native order, wstack.h) of tile `bin`: returns the pointer to its first cell
@@ -47,52 +54,81 @@ __device__ __forceinline__ float2* tile_origin(const WsGeom& g, float2* grid, ui
     return grid + ((size_t)k * N + sy) * N + sx;
 }
 
+// 32 rows x 256 B of zeros: 16 lanes x 16 B per row, two rows per store instruction
+__device__ __forceinline__ void store_zero_tile(float2* out, size_t N, int lane) {
+    float4* o4 = (float4*)(out + (size_t)(lane >> 4) * N) + (lane & 15);
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int y = 0; y < T; y += 2) __stcs(o4 + (size_t)y * (N / 2), z);
+}
+
+template <int S>
+struct WarpSmem {
+    float2* tile;
+    float4* meta;
+    float* gu;
+    float* gv;
+    __device__ __forceinline__ WarpSmem(unsigned char* base) {
+        using C = TileCfg<S>;
+        tile = (float2*)base;
+        meta = (float4*)(tile + C::TILE_CELLS);
+        gu = (float*)(meta + 32);
+        gv = gu + 32 * S;
+    }
+};
+
 // Accumulates records [lo, hi) into the warp's shared tile.
 template <int S>
 __device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
-                                           float2* tile, float4* stage, int lane) {
+                                           const WarpSmem<S>& sm, int lane) {
     using C = TileCfg<S>;
     const int a = lane % S, br = lane / S;
     const bool active = br < C::R;
-    const float da = (float)(a - C::H);
     const float tap_c = g.tap_c;
+    const int lane_idx = br * C::P + a;            // tap (a, br) relative to the footprint's first cell
     float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lo + lane < hi) nxt = __ldcs(records + lo + lane);
     for (uint32_t base = lo; base < hi; base += 32) {
         const int n = (int)min(32u, hi - base);
-        stage[lane] = nxt;
+        {   // vector phase: lane r prepares record r of the batch
+            const uint32_t X = __float_as_uint(nxt.x), Y = __float_as_uint(nxt.y);
+            const int cxp = ((int)X >> 24) - C::H, cyp = ((int)Y >> 24) - C::H;   // footprint's first cell, tile frame
+            const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
+            const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                const float dx = (float)(i - C::H) - fx, dy = (float)(i - C::H) - fy;
+                sm.gu[lane * S + i] = ex2_approx(tap_c * dx * dx);
+                sm.gv[lane * S + i] = ex2_approx(tap_c * dy * dy);
+            }
+            sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cxp & 0xFFFF) | (cyp << 16)),
+                                        __int_as_float(cyp * C::P + cxp));
+        }
         if (base + 32 + lane < hi) nxt = __ldcs(records + base + 32 + lane);   // prefetch the next batch
         __syncwarp();
         for (int r = 0; r < n; ++r) {
-            const float4 q = stage[r];                       // broadcast
-            const uint32_t X = __float_as_uint(q.x), Y = __float_as_uint(q.y);
-            const int cx = (int)X >> 24, cy = (int)Y >> 24;  // centre cell relative to the tile origin
-            const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
-            const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
-            const int x = cx - C::H + a;
-            const float dx = da - fx;
-            const float gu = ex2_approx(tap_c * dx * dx);
-            const bool okx = active && (unsigned)x < (unsigned)T;
+            const float4 m = sm.meta[r];                       // broadcast
+            const float u = sm.gu[r * S + a];
+            const int xy = __float_as_int(m.z);
+            const int cxp = (int)(short)(xy & 0xFFFF), cyp = xy >> 16;
+            const bool okx = active && (unsigned)(cxp + a) < (unsigned)T;
+            const int idx0 = __float_as_int(m.w) + lane_idx;
             float2 cell[C::NR];
             float t[C::NR];
             bool ok[C::NR];
-            int idx[C::NR];
 #pragma unroll
             for (int rr = 0; rr < C::NR; ++rr) {
                 const int b = br + rr * C::R;
-                const int y = cy - C::H + b;
-                const float dy = (float)(b - C::H) - fy;
-                t[rr] = gu * ex2_approx(tap_c * dy * dy);
-                ok[rr] = okx && b < S && (unsigned)y < (unsigned)T;
-                idx[rr] = y * C::P + x;
-                if (ok[rr]) cell[rr] = tile[idx[rr]];
+                ok[rr] = okx && b < S && (unsigned)(cyp + b) < (unsigned)T;
+                t[rr] = u * sm.gv[r * S + (b < S ? b : 0)];
+                if (ok[rr]) cell[rr] = sm.tile[idx0 + rr * C::R * C::P];
             }
 #pragma unroll
             for (int rr = 0; rr < C::NR; ++rr) {
                 if (ok[rr]) {
-                    cell[rr].x = fmaf(q.z, t[rr], cell[rr].x);
-                    cell[rr].y = fmaf(q.w, t[rr], cell[rr].y);
-                    tile[idx[rr]] = cell[rr];
+                    cell[rr].x = fmaf(m.x, t[rr], cell[rr].x);
+                    cell[rr].y = fmaf(m.y, t[rr], cell[rr].y);
+                    sm.tile[idx0 + rr * C::R * C::P] = cell[rr];
                 }
             }
             __syncwarp();
@@ -107,42 +143,103 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
     __syncwarp();
 }
 
-// One warp per tile-plane, tiles strided over all warps of the (persistent) grid.
+// Queues the chunks of the heavy bins as work items and (OVERWRITE mode) clears their tiles.
+__global__ void __launch_bounds__(256)
+k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, uint4* __restrict__ items,
+                uint32_t item_capacity, WsStatus* __restrict__ status, float2* __restrict__ grid, int mode) {
+    if (status->overflow) return;
+    const uint32_t b = blockIdx.x * 256u + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    uint32_t s = 0, cnt = 0;
+    if (b < g.n_bins) {
+        s = rec_start[b];
+        cnt = rec_start[b + 1] - s;
+    }
+    const bool heavy = cnt > WS_CHUNK;
+    const uint32_t chunks = heavy ? (cnt + WS_CHUNK - 1) / WS_CHUNK : 0u;
+    const unsigned hm = __ballot_sync(0xffffffffu, heavy);
+    if (!hm) return;
+    uint32_t inc = chunks;                       // inclusive warp scan of the chunk counts
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+    uint32_t base = 0;
+    if (lane == 0) base = atomicAdd(&status->n_items, total);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (base + total > item_capacity) {
+        if (lane == 0) status->overflow = 1u;
+        return;
+    }
+    if (heavy) {
+        uint32_t o = base + inc - chunks;
+        for (uint32_t lo = s; lo < s + cnt; lo += WS_CHUNK) items[o++] = make_uint4(b, lo, min(lo + WS_CHUNK, s + cnt), 0u);
+    }
+    if (mode == WS_GRID_OVERWRITE) {
+        for (unsigned m = hm; m; m &= m - 1) {
+            const uint32_t hb = (b - lane) + (__ffs(m) - 1);
+            store_zero_tile(tile_origin(g, grid, hb), (size_t)g.n_pix, lane);
+        }
+    }
+}
+
+// Persistent kernel: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
 template <int S>
-__global__ void __launch_bounds__(GRID_THREADS, 2)
-k_grid_tiles(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
-             const float4* __restrict__ records, float2* __restrict__ grid, int mode,
-             const WsStatus* __restrict__ status) {
+__global__ void __launch_bounds__(TileCfg<S>::THREADS, 2)
+k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint4* __restrict__ items,
+       const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float4* stage = (float4*)(smem_raw + (size_t)wid * C::WARP_BYTES);
-    float2* tile = (float2*)(stage + 32);
+    const WarpSmem<S> sm(smem_raw + (size_t)wid * C::WARP_BYTES);
     if (status->overflow) return;
-    const uint32_t n_warps = gridDim.x * GRID_WARPS;
+    const uint32_t n_items = status->n_items;
+    const uint32_t n_warps = gridDim.x * C::WARPS;
+    const uint32_t gw = blockIdx.x * C::WARPS + wid;
     const size_t N = (size_t)g.n_pix;
-    for (uint32_t bin = blockIdx.x * GRID_WARPS + wid; bin < g.n_bins; bin += n_warps) {
+    const uint32_t my_tiles = gw < g.n_bins ? (g.n_bins - gw + n_warps - 1) / n_warps : 0u;
+    const uint32_t my_items = gw < n_items ? (n_items - gw + n_warps - 1) / n_warps : 0u;
+    const uint32_t gap = my_items ? max(1u, my_tiles / my_items) : 0xFFFFFFFFu;
+    uint32_t it = gw, since = 0;
+
+    auto do_item = [&]() {
+        const uint4 w = items[it];
+        it += n_warps;
+        float2* out = tile_origin(g, grid, w.x);
+        zero_tile<S>(sm.tile, lane);
+        accumulate<S>(g, records, w.y, w.z, sm, lane);
+#pragma unroll 4
+        for (int y = 0; y < T; ++y) {
+            const float2 v = sm.tile[y * C::P + lane];
+            if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
+        }
+        __syncwarp();
+    };
+
+    for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
+        if (it < n_items && since >= gap) {
+            do_item();
+            since = 0;
+        }
+        ++since;
         const uint32_t s = rec_start[bin], e = rec_start[bin + 1];
+        if (e - s > WS_CHUNK) continue;                     // heavy: its chunks are items
         float2* out = tile_origin(g, grid, bin);
         if (s == e) {
-            if (mode == WS_GRID_OVERWRITE) {
-                // 32 rows x 256 B of zeros: 16 lanes x 16 B per row, two rows per store instruction
-                float4* o4 = (float4*)(out + (size_t)(lane >> 4) * N) + (lane & 15);
-                const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                for (int y = 0; y < T; y += 2) __stcs(o4 + (size_t)y * (N / 2), z);
-            }
+            if (mode == WS_GRID_OVERWRITE) store_zero_tile(out, N, lane);
             continue;
         }
-        zero_tile<S>(tile, lane);
-        accumulate<S>(g, records, s, min(e, s + (uint32_t)WS_CHUNK), tile, stage, lane);
+        zero_tile<S>(sm.tile, lane);
+        accumulate<S>(g, records, s, e, sm, lane);
         if (mode == WS_GRID_OVERWRITE) {
 #pragma unroll 4
-            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tile[y * C::P + lane]);
+            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, sm.tile[y * C::P + lane]);
         } else {
 #pragma unroll 4
             for (int y = 0; y < T; ++y) {
-                float2 v = tile[y * C::P + lane];
+                float2 v = sm.tile[y * C::P + lane];
                 float2* p = out + (size_t)y * N + lane;
                 const float2 old = *p;
                 v.x += old.x;
@@ -152,54 +249,27 @@ k_grid_tiles(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_
         }
         __syncwarp();
     }
-}
-
-// Heavy bins: chunks 1.. of a bin, added onto the tile chunk 0 already stored (stream order).
-template <int S>
-__global__ void __launch_bounds__(GRID_THREADS, 2)
-k_grid_items(const __grid_constant__ WsGeom g, const uint4* __restrict__ items, const float4* __restrict__ records,
-             float2* __restrict__ grid, const WsStatus* __restrict__ status) {
-    using C = TileCfg<S>;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    float4* stage = (float4*)(smem_raw + (size_t)wid * C::WARP_BYTES);
-    float2* tile = (float2*)(stage + 32);
-    if (status->overflow) return;
-    const uint32_t n_items = status->n_items;
-    const uint32_t n_warps = gridDim.x * GRID_WARPS;
-    const size_t N = (size_t)g.n_pix;
-    for (uint32_t it = blockIdx.x * GRID_WARPS + wid; it < n_items; it += n_warps) {
-        const uint4 w = items[it];
-        float2* out = tile_origin(g, grid, w.x);
-        zero_tile<S>(tile, lane);
-        accumulate<S>(g, records, w.y, w.z, tile, stage, lane);
-#pragma unroll 4
-        for (int y = 0; y < T; ++y) {
-            const float2 v = tile[y * C::P + lane];
-            if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
-        }
-        __syncwarp();
-    }
+    while (it < n_items) do_item();
 }
 
 template <int S>
 int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
     using C = TileCfg<S>;
-    const size_t smem = C::WARP_BYTES * GRID_WARPS;
+    const size_t smem = C::WARP_BYTES * C::WARPS;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_grid_tiles<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-            cudaFuncSetAttribute(k_grid_items<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_grid<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return WS_ERR_CUDA;
         attr_set = true;
     }
     const uint32_t* rec_start = (const uint32_t*)(ws + L.off_counts_all);
     const float4* records = (const float4*)(ws + L.off_records);
-    const WsStatus* status = plan->d_status;
-    const uint4* items = (const uint4*)(ws + L.off_items);
-    const int ctas = plan->sm_count * 2;
-    k_grid_tiles<S><<<ctas, GRID_THREADS, smem, st>>>(plan->geom, rec_start, records, grid, mode, status);
-    k_grid_items<S><<<ctas, GRID_THREADS, smem, st>>>(plan->geom, items, records, grid, status);
+    WsStatus* status = plan->d_status;
+    uint4* items = (uint4*)(ws + L.off_items);
+    const WsGeom& g = plan->geom;
+    if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode);
+    k_grid<S><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }

@@ -227,12 +227,14 @@ class Plan:
     def async_status(self, stream=None):
         self._check(lib().ws_async_status(self._h, _stream(stream)))
 
-    def get_bins(self, stream=None) -> dict:
-        """Bins of the last grid call as numpy arrays (copied to the host): keys, sorted_keys, perm, bin_start,
-        n_vis, n_bins, n_dropped, n_records."""
+    def get_bins(self, stream=None, fields=("keys", "sorted_keys", "perm", "bin_start")) -> dict:
+        """Bins of the last grid call as numpy arrays (copied to the host; only `fields`): keys, sorted_keys, perm,
+        bin_start; plus n_vis, n_bins, n_dropped, n_records."""
+        names = ("keys", "sorted_keys", "perm", "bin_start")
         p = [C.c_void_p() for _ in range(4)]
         n = [C.c_int64() for _ in range(4)]
-        self._check(lib().ws_get_bins(self._h, *[C.byref(x) for x in p], *[C.byref(x) for x in n], _stream(stream)))
+        ptr_args = [C.byref(x) if nm in fields else None for nm, x in zip(names, p)]
+        self._check(lib().ws_get_bins(self._h, *ptr_args, *[C.byref(x) for x in n], _stream(stream)))
         n_vis, n_bins, n_dropped, n_records = (int(x.value) for x in n)
         ws = self._ws
         base = ws.data_ptr()
@@ -242,6 +244,9 @@ class Plan:
             return ws[off: off + 4 * count].view(torch.int32).cpu().numpy().view(np.uint32)
 
         n_kept = n_vis - n_dropped
-        return dict(keys=view(p[0], n_vis), sorted_keys=view(p[1], n_kept), perm=view(p[2], n_kept),
-                    bin_start=view(p[3], n_bins + 1), n_vis=n_vis, n_bins=n_bins, n_dropped=n_dropped,
-                    n_records=n_records)
+        counts = dict(keys=n_vis, sorted_keys=n_kept, perm=n_kept, bin_start=n_bins + 1)
+        out = dict(n_vis=n_vis, n_bins=n_bins, n_dropped=n_dropped, n_records=n_records)
+        for nm, x in zip(names, p):
+            if nm in fields:
+                out[nm] = view(x, counts[nm])
+        return out
