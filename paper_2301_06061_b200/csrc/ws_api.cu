@@ -24,7 +24,7 @@ int cuda_fail(ws_plan* plan, cudaError_t e, const char* where) {
     return WS_ERR_CUDA;
 }
 
-// Workspace layout for n_vis visibilities and a record capacity.  Head (counters .. block sums) is cleared per call.
+// Workspace layout for n_vis visibilities and a record capacity.  The two histograms at the head are cleared per call.
 WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) {
     WsLayout L;
     const size_t nb = plan->geom.n_bins;
@@ -32,9 +32,10 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) 
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = ws_align_up(off + bytes, A); return o; };
     L.off_counts_home = take((nb + 1) * 4);
-    L.off_counts_all = take((nb + 1) * 4);
+    L.off_counts_halo = take((nb + 1) * 4);
+    L.off_rec_start = take((nb + 1) * 4);
     L.off_cursor_home = take(nb * 4);
-    L.off_cursor_all = take(nb * 4);
+    L.off_cursor_halo = take(nb * 4);
     L.off_block_sums = take(2 * ((nb + 1) / 4096 + 2) * 4);
     L.off_keys = take((size_t)n_vis * 4);
     L.off_perm = take((size_t)n_vis * 4);

@@ -18,9 +18,8 @@ struct Placed {
     double fu, fv;
 };
 
-__device__ __forceinline__ bool place(const WsChanConsts& cc, const WsGeom& g, float u, float v, float w, int c,
-                                      Placed& o) {
-    const double su = cc.su[c], sw = cc.sw[c];
+__device__ __forceinline__ bool place(const WsChanConsts& cc, const WsGeom& g, float u, float v, float w, double su,
+                                      double sw, Placed& o) {
     const double pu = __fma_rn((double)u, su, cc.half);
     const double pv = __fma_rn((double)v, su, cc.half);
     const double pw = __fma_rn((double)w, sw, cc.ow);
@@ -65,6 +64,16 @@ __device__ __forceinline__ Groups warp_groups(uint32_t home, int dx, int dy) {
 __device__ __forceinline__ bool leads(unsigned group, int lane) { return group && lane == __ffs(group) - 1; }
 __device__ __forceinline__ uint32_t rank_in(unsigned group, int lane) { return (uint32_t)__popc(group & ((1u << lane) - 1u)); }
 
+// The per-channel constants are staged in shared memory: indexing the kernel parameter with a per-lane channel
+// would be a divergent constant-bank load, replayed once per distinct channel in the warp.
+__device__ __forceinline__ void stage_consts(const WsChanConsts& cc, uint32_t n_chan, double* s_su, double* s_sw) {
+    for (uint32_t i = threadIdx.x; i < n_chan; i += blockDim.x) {
+        s_su[i] = cc.su[i];
+        s_sw[i] = cc.sw[i];
+    }
+    __syncthreads();
+}
+
 __device__ __forceinline__ void row_chan(uint32_t m, uint32_t n_chan, int chan_shift, uint32_t& row, uint32_t& c) {
     if (chan_shift >= 0) {
         row = m >> chan_shift;
@@ -79,7 +88,9 @@ __device__ __forceinline__ void row_chan(uint32_t m, uint32_t n_chan, int chan_s
 __global__ void __launch_bounds__(256)
 k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
             const float* __restrict__ uvw, uint32_t n_vis, uint32_t n_chan, int chan_shift,
-            uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_all) {
+            uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_halo) {
+    __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
+    stage_consts(cc, n_chan, s_su, s_sw);
     const uint32_t m = blockIdx.x * 256u + threadIdx.x;
     const int lane = threadIdx.x & 31;
     Placed pl;
@@ -88,7 +99,7 @@ k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsG
         uint32_t row, c;
         row_chan(m, n_chan, chan_shift, row, c);
         const float* p = uvw + 3ull * row;
-        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl);
+        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), s_su[c], s_sw[c], pl);
     }
     uint32_t home = 0xFFFFFFFFu;
     int tx = 0, ty = 0, dx = 0, dy = 0, k = 0;
@@ -101,15 +112,13 @@ k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsG
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
     }
     if (m < n_vis) keys[m] = home;
+    // two histograms: visibilities per home bin (-> bin_start) and halo copies received per bin; the record
+    // list of a bin is its home records followed by its halo records (rec_start = their sum, k_finish_offsets)
     const Groups q = warp_groups(home, dx, dy);
-    if (kept && leads(q.home, lane)) {
-        const uint32_t n = (uint32_t)__popc(q.home);
-        atomicAdd(counts_home + home, n);
-        atomicAdd(counts_all + home, n);
-    }
-    if (leads(q.nx, lane)) atomicAdd(counts_all + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
-    if (leads(q.ny, lane)) atomicAdd(counts_all + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
-    if (leads(q.nc, lane)) atomicAdd(counts_all + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
+    if (kept && leads(q.home, lane)) atomicAdd(counts_home + home, (uint32_t)__popc(q.home));
+    if (leads(q.nx, lane)) atomicAdd(counts_halo + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
+    if (leads(q.ny, lane)) atomicAdd(counts_halo + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
+    if (leads(q.nc, lane)) atomicAdd(counts_halo + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
 }
 
 // ---- exclusive prefix scan over n entries of two arrays (blockIdx.y selects), in place ------------------
@@ -173,13 +182,11 @@ k_scan_block_sums(uint32_t* __restrict__ block_sums, uint32_t n_blocks) {
     }
 }
 
-// Writes the exclusive scan in place, seeds the scatter cursors, and records the totals.
+// Writes the exclusive scans in place (bin_start, halo_start).
 __global__ void __launch_bounds__(SCAN_THREADS)
-k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t* __restrict__ cur0,
-             uint32_t* __restrict__ cur1, uint32_t n, const uint32_t* __restrict__ block_sums, uint32_t n_blocks,
-             WsStatus* __restrict__ status, uint64_t rec_capacity) {
+k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t n, const uint32_t* __restrict__ block_sums,
+             uint32_t n_blocks) {
     uint32_t* a = blockIdx.y ? a1 : a0;
-    uint32_t* cur = blockIdx.y ? cur1 : cur0;
     const uint32_t base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
     uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -192,19 +199,28 @@ k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t* __r
     uint32_t run = block_sums[blockIdx.y * n_blocks + blockIdx.x] + inc - s;
 #pragma unroll
     for (int i = 0; i < SCAN_ITEMS; ++i) {
-        const uint32_t idx = base + i;
-        if (idx < n) {
-            a[idx] = run;
-            if (idx < n - 1) cur[idx] = run;
-            else {   // entry n-1 = n_bins: the grand total
-                if (blockIdx.y == 0) status->n_kept = run;
-                else {
-                    status->n_records = run;
-                    if ((uint64_t)run > rec_capacity) status->overflow = 1u;
-                }
-            }
-        }
+        if (base + i < n) a[base + i] = run;
         run += v[i];
+    }
+}
+
+// rec_start = bin_start + halo_start; cursors: home slots start at bin_start[b] (perm), halo records of bin b
+// start after its home records, at rec_start[b] + count_home[b]; totals and the capacity check.
+__global__ void __launch_bounds__(256)
+k_finish_offsets(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
+                 uint32_t* __restrict__ rec_start, uint32_t* __restrict__ cursor_home, uint32_t* __restrict__ cursor_halo,
+                 uint32_t n_bins, WsStatus* __restrict__ status, uint64_t rec_capacity) {
+    const uint32_t b = blockIdx.x * 256u + threadIdx.x;
+    if (b > n_bins) return;
+    const uint32_t bs = bin_start[b], hs = halo_start[b];
+    rec_start[b] = bs + hs;
+    if (b < n_bins) {
+        cursor_home[b] = bs;
+        cursor_halo[b] = bin_start[b + 1] + hs;
+    } else {
+        status->n_kept = bs;
+        status->n_records = bs + hs;
+        if ((uint64_t)bs + (uint64_t)hs > rec_capacity) status->overflow = 1u;
     }
 }
 
@@ -216,9 +232,11 @@ __global__ void __launch_bounds__(256)
 k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
           const float* __restrict__ uvw, const float2* __restrict__ vis, const float* __restrict__ wt,
           uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home,
-          uint32_t* __restrict__ cursor_all, uint32_t* __restrict__ perm, float4* __restrict__ records,
-          const WsStatus* __restrict__ status) {
+          uint32_t* __restrict__ cursor_halo, const uint32_t* __restrict__ halo_start, uint32_t* __restrict__ perm,
+          float4* __restrict__ records, const WsStatus* __restrict__ status) {
     if (status->overflow) return;
+    __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
+    stage_consts(cc, n_chan, s_su, s_sw);
     const uint32_t m = blockIdx.x * 256u + threadIdx.x;
     const int lane = threadIdx.x & 31;
     Placed pl;
@@ -227,9 +245,9 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         uint32_t row, c;
         row_chan(m, n_chan, chan_shift, row, c);
         const float* p = uvw + 3ull * row;
-        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), (int)c, pl);
+        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), s_su[c], s_sw[c], pl);
     }
-    uint32_t home = 0xFFFFFFFFu;
+    uint32_t home = 0xFFFFFFFFu, hs = 0;
     int tx = 0, ty = 0, lx = 0, ly = 0, dx = 0, dy = 0, k = 0;
     float2 v = make_float2(0.f, 0.f);
     float w = 0.f;
@@ -239,20 +257,18 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
         lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
         home = bin_of(g, k, ty, tx);
+        hs = __ldg(halo_start + home);
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
     }
-    // slots: every group leader issues its atomics back to back, the results are broadcast afterwards
+    // slots: every group leader issues its atomics back to back, the results are broadcast afterwards.  The home
+    // copy needs no second atomic: its record slot is its perm slot shifted by the bin's halo_start.
     const Groups q = warp_groups(home, dx, dy);
-    uint32_t bh = 0, ba = 0, bx = 0, by = 0, bc = 0;
-    if (kept && leads(q.home, lane)) {
-        const uint32_t n = (uint32_t)__popc(q.home);
-        bh = atomicAdd(cursor_home + home, n);
-        ba = atomicAdd(cursor_all + home, n);
-    }
-    if (leads(q.nx, lane)) bx = atomicAdd(cursor_all + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
-    if (leads(q.ny, lane)) by = atomicAdd(cursor_all + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
-    if (leads(q.nc, lane)) bc = atomicAdd(cursor_all + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
+    uint32_t bh = 0, bx = 0, by = 0, bc = 0;
+    if (kept && leads(q.home, lane)) bh = atomicAdd(cursor_home + home, (uint32_t)__popc(q.home));
+    if (leads(q.nx, lane)) bx = atomicAdd(cursor_halo + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
+    if (leads(q.ny, lane)) by = atomicAdd(cursor_halo + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
+    if (leads(q.nc, lane)) bc = atomicAdd(cursor_halo + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
 
     uint32_t qx = 0, qy = 0;
     float vr = 0.f, vi = 0.f;
@@ -264,9 +280,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         qy = qy > 0xFFFFFFu ? 0xFFFFFFu : qy;
         vr = v.x * wn; vi = v.y * wn;
     }
-    const int lh = __ffs(q.home) - 1;
-    bh = __shfl_sync(0xffffffffu, bh, lh) + rank_in(q.home, lane);
-    ba = __shfl_sync(0xffffffffu, ba, lh) + rank_in(q.home, lane);
+    bh = __shfl_sync(0xffffffffu, bh, __ffs(q.home) - 1) + rank_in(q.home, lane);
     bx = __shfl_sync(0xffffffffu, bx, q.nx ? __ffs(q.nx) - 1 : lane) + rank_in(q.nx, lane);
     by = __shfl_sync(0xffffffffu, by, q.ny ? __ffs(q.ny) - 1 : lane) + rank_in(q.ny, lane);
     bc = __shfl_sync(0xffffffffu, bc, q.nc ? __ffs(q.nc) - 1 : lane) + rank_in(q.nc, lane);
@@ -278,7 +292,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         records[slot] = make_float4(__uint_as_float(X), __uint_as_float(Y), vr, vi);
     };
     perm[bh] = m;
-    emit(ba, 0, 0);
+    emit(bh + hs, 0, 0);
     if (q.nx) emit(bx, dx, 0);
     if (q.ny) emit(by, 0, dy);
     if (q.nc) emit(bc, dx, dy);
@@ -299,10 +313,11 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {
     const WsGeom& g = plan->geom;
     const uint32_t n_vis = (uint32_t)(n_rows * n_chan);
-    uint32_t* counts_home = (uint32_t*)(ws + L.off_counts_home);
-    uint32_t* counts_all = (uint32_t*)(ws + L.off_counts_all);
+    uint32_t* counts_home = (uint32_t*)(ws + L.off_counts_home);   // -> bin_start
+    uint32_t* counts_halo = (uint32_t*)(ws + L.off_counts_halo);   // -> halo_start
+    uint32_t* rec_start = (uint32_t*)(ws + L.off_rec_start);
     uint32_t* cursor_home = (uint32_t*)(ws + L.off_cursor_home);
-    uint32_t* cursor_all = (uint32_t*)(ws + L.off_cursor_all);
+    uint32_t* cursor_halo = (uint32_t*)(ws + L.off_cursor_halo);
     uint32_t* block_sums = (uint32_t*)(ws + L.off_block_sums);
     WsStatus* status = plan->d_status;
     uint32_t* keys = (uint32_t*)(ws + L.off_keys);
@@ -313,25 +328,26 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     for (int b = 0; b < 8; ++b)
         if (n_chan == (1 << b)) chan_shift = b;
 
-    // the counters are contiguous at the head of the workspace: one clear, plus the plan's status block
-    if (cudaMemsetAsync(ws, 0, L.off_keys, st) != cudaSuccess) return WS_ERR_CUDA;
+    // the two histograms are contiguous at the head of the workspace: one clear, plus the plan's status block
+    if (cudaMemsetAsync(ws, 0, L.off_rec_start, st) != cudaSuccess) return WS_ERR_CUDA;
     if (cudaMemsetAsync(status, 0, sizeof(WsStatus), st) != cudaSuccess) return WS_ERR_CUDA;
 
     const uint32_t n_scan = g.n_bins + 1;
     const uint32_t n_blocks = (n_scan + SCAN_BLOCK - 1) / SCAN_BLOCK;
     if (n_vis) {
-        k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, chan_shift, keys, counts_home,
-                                                         counts_all);
+        k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, chan_shift, keys,
+                                                         counts_home, counts_halo);
         ++launches;
     }
-    k_scan_reduce<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_all, n_scan, block_sums, n_blocks);
+    k_scan_reduce<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
     k_scan_block_sums<<<dim3(1, 2), SCAN_THREADS, 0, st>>>(block_sums, n_blocks);
-    k_scan_apply<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_all, cursor_home, cursor_all, n_scan,
-                                                             block_sums, n_blocks, status, L.rec_capacity);
-    launches += 3;
+    k_scan_apply<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
+    k_finish_offsets<<<(n_scan + 255) / 256, 256, 0, st>>>(counts_home, counts_halo, rec_start, cursor_home, cursor_halo,
+                                                          g.n_bins, status, L.rec_capacity);
+    launches += 4;
     if (n_vis) {
-        k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift, cursor_home,
-                                                       cursor_all, perm, records, status);
+        k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift,
+                                                       cursor_home, cursor_halo, counts_halo, perm, records, status);
         ++launches;
     }
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;

@@ -262,7 +262,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
             return WS_ERR_CUDA;
         attr_set = true;
     }
-    const uint32_t* rec_start = (const uint32_t*)(ws + L.off_counts_all);
+    const uint32_t* rec_start = (const uint32_t*)(ws + L.off_rec_start);
     const float4* records = (const float4*)(ws + L.off_records);
     WsStatus* status = plan->d_status;
     uint4* items = (uint4*)(ws + L.off_items);

@@ -33,8 +33,9 @@ struct WsGeom {
 
 // Workspace carve-up for one ws_grid_visibilities call (all offsets 256-byte aligned).
 struct WsLayout {
-    size_t off_counts_home, off_counts_all;     // [n_bins + 1] u32 each: histogram -> exclusive scan (bin_start / rec_start)
-    size_t off_cursor_home, off_cursor_all;     // [n_bins] u32: running slot cursors of the scatter
+    size_t off_counts_home, off_counts_halo;    // [n_bins + 1] u32 each: histograms -> exclusive scans (bin_start / halo_start)
+    size_t off_rec_start;                       // [n_bins + 1] u32: bin_start + halo_start = first record of each bin
+    size_t off_cursor_home, off_cursor_halo;    // [n_bins] u32: running slot cursors of the scatter
     size_t off_block_sums;                      // scan scratch
     size_t off_keys, off_perm, off_sorted_keys; // [n_vis] u32 each
     size_t off_items;                           // heavy-chunk work items (uint4)
