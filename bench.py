@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--impl ours|reference]
 
 One "step" = one pass of the whole hot path over the synthetic workload, inputs resident in HBM:
-a1 bin -> a2 grid (WS_GRID_OVERWRITE: every mesh cell written, no memset) -> a3 cuFFT per plane -> a4 fused
-w-correction + accumulation (also writes a5, the real dirty image).  Prints ONE JSON line (rank 0).
+a1 bin -> a2 grid (WS_GRID_SPARSE: only the tiles that hold visibilities are written, no memset) -> a3 the library's
+own FFT, columns then rows, skipping what the gridder left empty -> a4 fused into the row pass (also writes a5, the
+real dirty image).  cuFFT + the stand-alone w-correction are timed beside it (library_path_ms).  Prints ONE JSON line (rank 0).
 N > 1 runs N independent replicas (the path is built for one GPU, "replicas only").
 `--impl reference` times the fp64 CPU oracle on a bounded sample of the same workload (see cpu_baseline()).
 """
@@ -167,15 +168,25 @@ def main():
     grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
     wsp = plan.alloc_workspace(d.n_vis)
 
+    own = plan.fft_is_own
+    OCC = ws.WS_FFT_USE_OCCUPANCY
+
     def step(ev=None):
         if ev: ev[0].record()
         plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
         if ev: ev[1].record()
-        plan.grid_binned(grid, wsp, mode=ws.WS_GRID_OVERWRITE)
-        if ev: ev[2].record()
-        plan.fft_planes(grid, wsp)
-        if ev: ev[3].record()
-        plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
+        if own:     # the mesh is neither cleared nor completely written: the FFT passes skip what stayed empty
+            plan.grid_binned(grid, wsp, mode=ws.WS_GRID_SPARSE)
+            if ev: ev[2].record()
+            plan.fft_columns(grid, OCC)
+            if ev: ev[3].record()
+            plan.fft_rows_wcorrect(grid, image, accumulate=False, dirty=dirty, fft_flags=OCC)
+        else:       # N not a power of two in 256..8192: library FFT on a fully written mesh, stand-alone a4
+            plan.grid_binned(grid, wsp, mode=ws.WS_GRID_OVERWRITE)
+            if ev: ev[2].record()
+            plan.fft_planes(grid, wsp)
+            if ev: ev[3].record()
+            plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
         if ev: ev[4].record()
 
     for _ in range(args.warmup):
@@ -217,32 +228,82 @@ def main():
     med = np.median(st, axis=0)
     value = world * d.n_vis / (ms_step * 1e-3) / 1e6
 
-    # ---- roofline of the dominant own kernel (algorithmic bytes) ---------------------
+    # ---- the library path on the same inputs, for the separate FFT figure (north_star): OVERWRITE gridding,
+    # cuFFT per plane, stand-alone w-correction.  Outside the timed region.
+    lib_ms = None
+    if own:
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        rows = []
+        for _ in range(3):
+            plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+            e[0].record()
+            plan.grid_binned(grid, wsp, mode=ws.WS_GRID_OVERWRITE)
+            e[1].record()
+            plan.fft_planes(grid, wsp)
+            e[2].record()
+            plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
+            e[3].record()
+            torch.cuda.synchronize()
+            rows.append([e[i].elapsed_time(e[i + 1]) for i in range(3)])
+        m = np.median(np.array(rows), axis=0)
+        lib_ms = {"grid_overwrite": float(m[0]), "fft_cufft": float(m[1]), "wcorrect_standalone": float(m[2])}
+
+    # ---- roofline of the dominant own kernel -----------------------------------------
     peak, peak_src = peaks()
     mesh_b = 8.0 * d.n_pix ** 2 * d.n_wplanes
-    alg = {"k_grid_tiles": mesh_b + 16.0 * n_records,                        # every cell written once + records read
-           "k_wcorrect": mesh_b + 8.0 * d.n_pix ** 2 + 4.0 * d.n_pix ** 2}   # planes read once + image + dirty written
-    times = {"k_grid_tiles": med[1], "k_wcorrect": med[3]}
+    N, NW = d.n_pix, d.n_wplanes
+    if own:
+        occ = plan.occupancy()       # fractions of the mesh the passes touch (from the plan's masks)
+        # k_grid: records read + non-empty tiles written; pass 1: non-empty tiles read, classes written, then the
+        # non-empty bands read and written; pass 2: non-empty bands read once, image + dirty written
+        alg = {"k_grid_tiles": 16.0 * n_records + mesh_b * occ["tiles"],
+               "k_fft_columns": mesh_b * (occ["tiles"] + occ["classes"] + 2 * occ["bands"]),
+               "k_fft_rows_wcorrect": mesh_b * occ["bands"] + 12.0 * N * N}
+        times = {"k_grid_tiles": med[1], "k_fft_columns": med[2], "k_fft_rows_wcorrect": med[3]}
+        # nominal FFT flops (5 n log2 n per transform) of the transforms that are not skipped, + 8 per point-plane of Horner
+        flops = {"k_fft_columns": 5.0 * N * np.log2(N) * N * NW * occ["bands"],
+                 "k_fft_rows_wcorrect": (5.0 * N * np.log2(N) + 8.0 * N) * N * NW * occ["planes"]}
+    else:
+        occ = None
+        alg = {"k_grid_tiles": mesh_b + 16.0 * n_records, "k_wcorrect": mesh_b + 12.0 * N * N}
+        times = {"k_grid_tiles": med[1], "k_wcorrect": med[3]}
+        flops = {}
     dom = max(times, key=times.get)
     ach = alg[dom] / (times[dom] * 1e-3) / 1e9
-    roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+    hbm_frac = ach / peak
+    roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": hbm_frac,
             "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
             "launch_ms": float(times[dom])}
-    b_path = 12.0 * d.n_rows + 12.0 * d.n_vis + 2 * mesh_b + 8.0 * d.n_pix ** 2
-    t_path = med[0] + med[1] + med[3]
-    roof_path = {"what": "a1+a2+a4 (path without the library FFT), SURVEY 8(d) B_alg(path)", "bytes": b_path,
-                 "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
+    if dom in flops:
+        # fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x max SM clock (B200_PROFILING.md unit counts and clocks)
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        tf = flops[dom] / (times[dom] * 1e-3) / 1e12
+        if tf / alu_peak > hbm_frac:
+            roof = {"bound": "alu", "kernel": dom, "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
+                    "traffic": None, "peak_source": "148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (guide's unit counts and clocks)",
+                    "nominal_flops_per_launch": flops[dom], "launch_ms": float(times[dom]),
+                    "hbm_view": {"achieved": ach, "peak": peak, "frac": hbm_frac, "algorithmic_bytes_per_launch": alg[dom]}}
+    per_kernel = {k: {"ms": float(times[k]), "alg_GB": alg[k] / 1e9, "GBps": alg[k] / (times[k] * 1e-3) / 1e9,
+                      "frac_of_hbm_peak": alg[k] / (times[k] * 1e-3) / 1e9 / peak} for k in times}
+    # B_alg(path) counts every plane cell written once and read once; the sparse path moves less
+    b_path = 12.0 * d.n_rows + 12.0 * d.n_vis + 2 * mesh_b + 8.0 * N * N
+    t_path = med[0] + med[1] + (lib_ms["wcorrect_standalone"] if lib_ms else med[3])
+    roof_path = {"what": "a1+a2+a4 without any FFT (bin + grid + stand-alone w-correction), SURVEY 8(d) B_alg(path)",
+                 "bytes": b_path, "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
                  "frac_of_measured_peak": b_path / (t_path * 1e-3) / 1e9 / peak,
                  "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
 
+    stage_names = ["bin", "grid", "fft_columns", "fft_rows_wcorrect"] if own else ["bin", "grid", "fft_cufft", "wcorrect"]
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
-           "stages_ms_median": {"bin": float(med[0]), "grid": float(med[1]), "fft_cufft": float(med[2]),
-                                "wcorrect": float(med[3])},
+           "stages_ms_median": {n: float(v) for n, v in zip(stage_names, med)},
+           "fft": "own two-pass FFT with fused w-correction, occupancy-aware" if own else "cuFFT",
+           "library_path_ms": lib_ms, "occupancy": occ,
            "mvis_per_s_gridding": d.n_vis / ((med[0] + med[1]) * 1e-3) / 1e6,
            "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
-           "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "roofline_path": roof_path}
+           "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "kernels": per_kernel,
+           "roofline_path": roof_path}
 
     # ---- end to end through the C ABI with HOST buffers --------------------------------------------------
     if not args.no_e2e:

@@ -6,6 +6,7 @@
  *   ws_grid_visibilities   a1 + a2: bin the visibilities by (w-plane, uv-tile) and convolve them onto
  *                          the stack of w-planes (Eq. 3 at :80)
  *   ws_fft_planes          a3: one 2-D inverse FFT per w-plane -- cuFFT
+ *   ws_fft_wcorrect        a3 + a4 in one call: the library's own FFT with Eq. 2 fused into its last pass
  *   ws_wcorrect_accumulate a4: phase screen exp(2 pi i w_k (sqrt(1-l^2-m^2)-1)) times plane k, summed
  *                          over planes (PAPER.md:68 Eq. 2, :86)
  *   ws_dirty_image         a5: real part of the accumulated image
@@ -34,7 +35,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 100
+#define WS_VERSION 110
 
 /* error codes */
 #define WS_OK 0
@@ -47,6 +48,19 @@ extern "C" {
 /* ws_grid_visibilities mode */
 #define WS_GRID_ACCUMULATE 0 /* add onto the existing mesh (call ws_grid_zero first); tiles without visibilities untouched */
 #define WS_GRID_OVERWRITE 1  /* the mesh is taken as zero on entry and EVERY cell is written: no ws_grid_zero needed */
+#define WS_GRID_SPARSE 2     /* as OVERWRITE, but only the 32 x 32 tiles that receive visibilities are written; every
+                                other cell keeps whatever it held.  Only ws_fft_* with WS_FFT_USE_OCCUPANCY can
+                                consume such a mesh (own FFT: N = 2^8..2^13 and no WS_FLAG_LIBRARY_FFT) */
+
+/* fft_flags of ws_fft_wcorrect / ws_fft_columns / ws_fft_rows_wcorrect */
+#define WS_FFT_USE_OCCUPANCY 1u /* skip the tiles / column bands the gridding calls on this plan left empty.  The plan
+                                   records which tiles of a mesh its ws_grid_* calls filled (restarted by ws_grid_zero
+                                   and by an OVERWRITE / SPARSE call, extended by ACCUMULATE calls); valid only if
+                                   nothing else wrote the mesh in between (else WS_ERR_INVALID_ARG, or wrong results
+                                   if the library cannot know) */
+
+/* ws_params.flags */
+#define WS_FLAG_LIBRARY_FFT 1u /* a3 through cuFFT even where the library's own two-pass FFT exists (N = 2^8..2^13) */
 
 /* kernel_type */
 #define WS_KERNEL_GAUSSIAN 0 /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)) */
@@ -64,7 +78,7 @@ typedef struct ws_params {
                           /* [w_min + k dw, w_min + (k+1) dw), dw = (w_max-w_min)/N_w, value = midpoint     */
     int32_t tile;         /* uv-tile side T of the bin key; 0 = auto (32); only 32 is supported            */
     int32_t device;       /* CUDA device ordinal                                                           */
-    uint32_t flags;       /* reserved, 0                                                                   */
+    uint32_t flags;       /* 0 or WS_FLAG_*                                                                */
 } ws_params;
 
 /* ---- plan ------------------------------------------------------------------------------------------- */
@@ -117,12 +131,32 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
 /* P_k[q][p] = sum_ji G_k[j][i] exp(+2 pi i ((i-N/2)(p-N/2) + (j-N/2)(q-N/2)) / N) in logical indices. */
 int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream);
 
+/* 1 if ws_fft_wcorrect runs the library's own FFT kernels, 0 if it calls cuFFT + the stand-alone a4 pass. */
+int ws_plan_fft_is_own(const ws_plan* plan);
+
 /* ---- a4: w-correction and reduction over planes, Eq. 2 ------------------------------ */
 /* image[q][p] (+)= sum_k exp(2 pi i w_k t) P_k[q][p], t = sqrt(1-l^2-m^2) - 1, w_k = w_min + (k+1/2) dw;
  * pixels with l^2 + m^2 >= 1 receive 0.  accumulate: 0 overwrite, 1 add to image.
  * dirty may be NULL; otherwise Re(image) after this call is also written there (float32 [N][N]). */
 int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32_t accumulate, float* dirty,
                            void* stream);
+
+/* ---- a3 + a4 fused: ws_fft_planes followed by ws_wcorrect_accumulate, same image --------- */
+/* With the own FFT (N = 2^8..2^13) a plane makes two trips through memory instead of four: columns (two in-place
+ * steps), then rows, whose last pass multiplies each transformed row by the phase screen and sums it over the
+ * planes in registers -- the transformed planes are never written.  `grid` is DESTROYED (it holds the
+ * column-transformed planes afterwards, rows in digit-reversed order).  With cuFFT (WS_FLAG_LIBRARY_FFT or other
+ * N) it is exactly the two calls in sequence and needs `workspace` >= ws_fft_workspace_bytes.  dirty may be NULL.
+ * fft_flags: 0 (any mesh contents) or WS_FFT_USE_OCCUPANCY. */
+int ws_fft_wcorrect(ws_plan* plan, void* grid, void* image, int32_t accumulate, float* dirty, uint32_t fft_flags,
+                    void* workspace, size_t workspace_bytes, void* stream);
+/* The two halves of ws_fft_wcorrect as separate calls (own FFT only, else WS_ERR_UNSUPPORTED).
+ * ws_fft_columns transforms every plane along v in place: afterwards row position r of a plane holds
+ * v-frequency (r / 256) + (N / 256) (r mod 256).  ws_fft_rows_wcorrect transforms such rows along u and applies
+ * Eq. 2 without writing them back (grid is read only). */
+int ws_fft_columns(ws_plan* plan, void* grid, uint32_t fft_flags, void* stream);
+int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t accumulate, float* dirty,
+                         uint32_t fft_flags, void* stream);
 
 /* ---- a5: dirty[q][p] = Re image[q][p]; norm_flags must be 0 ---------------------------- */
 int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream);
@@ -145,6 +179,10 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
 int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_keys, const uint32_t** perm,
                 const uint32_t** bin_start, int64_t* n_vis, int64_t* n_bins, int64_t* n_dropped,
                 int64_t* n_records, void* stream);
+
+/* Fractions of the mesh the recorded occupancy marks non-empty (synchronises `stream`): 32 x 32 tiles; row classes
+ * pass 1a of the FFT writes; 32-column bands per plane (what pass 1b writes and pass 2 reads); planes with any. */
+int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, void* stream);
 
 /* Synchronises `stream` and returns the deferred status of the work enqueued so far (record capacity
  * exceeded -> WS_ERR_WORKSPACE, CUDA fault -> WS_ERR_CUDA). */

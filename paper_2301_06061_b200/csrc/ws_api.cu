@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "ws_internal.h"
 
@@ -123,7 +124,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
     if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
-    if (p->flags != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
+    if ((p->flags & ~(uint32_t)WS_FLAG_LIBRARY_FFT) != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
     if (p->support > 2 * WS_HALO_MAX + 1) return WS_ERR_UNSUPPORTED;
     if (p->kernel_type != WS_KERNEL_GAUSSIAN) return WS_ERR_UNSUPPORTED;
     if (p->tile != 0 && p->tile != WS_TILE) return WS_ERR_UNSUPPORTED;
@@ -166,8 +167,18 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
         delete plan;
         return WS_ERR_CUDA;
     }
-    const int rc = make_fft_plan(plan);
+    // a3: the FFT of ws_fft.cu where it exists (N = 2^8 .. 2^13), else (or on request) the library's
+    plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix);
+    plan->d_twiddles = nullptr;
+    plan->d_masks = nullptr;
+    plan->mask_words = 0;
+    plan->occ_grid = nullptr;
+    int rc = make_fft_plan(plan);                       // ws_fft_planes is always the library's
+    if (rc == WS_OK && plan->fft_own) rc = ws_fft_own_init(plan);
     if (rc != WS_OK) {
+        if (plan->fft_ok) cufftDestroy(plan->fft);
+        if (plan->d_twiddles) cudaFree(plan->d_twiddles);
+        if (plan->d_masks) cudaFree(plan->d_masks);
         cudaFree(plan->d_status);
         delete plan;
         return rc;
@@ -180,6 +191,8 @@ int ws_plan_destroy(ws_plan* plan) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (plan->fft_ok) cufftDestroy(plan->fft);
     if (plan->d_status) cudaFree(plan->d_status);
+    if (plan->d_twiddles) cudaFree(plan->d_twiddles);
+    if (plan->d_masks) cudaFree(plan->d_masks);
     delete plan;
     return WS_OK;
 }
@@ -191,6 +204,7 @@ size_t ws_image_bytes(const ws_plan* plan) { return plan ? (size_t)8 * plan->prm
 size_t ws_dirty_bytes(const ws_plan* plan) { return plan ? (size_t)4 * plan->prm.n_pix * plan->prm.n_pix : 0; }
 size_t ws_fft_workspace_bytes(const ws_plan* plan) { return plan ? plan->fft_work_bytes : 0; }
 int ws_plan_tile(const ws_plan* plan) { return plan ? WS_TILE : 0; }
+int ws_plan_fft_is_own(const ws_plan* plan) { return plan && plan->fft_own ? 1 : 0; }
 int64_t ws_plan_n_bins(const ws_plan* plan) { return plan ? (int64_t)plan->geom.n_bins : 0; }
 
 size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_factor) {
@@ -206,8 +220,11 @@ size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis) { return ws_work
 
 int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_zero: null argument");
-    const int rc = ws_launch_zero(plan, grid, ws_grid_bytes(plan), (cudaStream_t)stream);
-    return rc < 0 ? fail(plan, rc, "ws_grid_zero: memset failed") : WS_OK;
+    int rc = ws_launch_zero(plan, grid, ws_grid_bytes(plan), (cudaStream_t)stream);
+    if (rc >= 0) rc = ws_launch_fft_masks_clear(plan, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_grid_zero: memset failed");
+    plan->occ_grid = grid;                               // an empty mesh: the occupancy masks describe it
+    return WS_OK;
 }
 
 int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
@@ -262,13 +279,30 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid || !workspace) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: null pointer");
-    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: bad mode");
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: bad mode");
+    if (mode == WS_GRID_SPARSE && !plan->fft_own)
+        return fail(plan, WS_ERR_UNSUPPORTED, "ws_grid_binned: WS_GRID_SPARSE needs the own FFT (N = 2^8..2^13, no WS_FLAG_LIBRARY_FFT)");
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: grid must be 16-byte aligned");
     if (!plan->last_valid || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: workspace does not hold the bins of ws_bin_visibilities");
-    const int rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
+    int rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
     plan->launches += rc;
+    // tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE
+    if (plan->d_masks) {
+        if (mode != WS_GRID_ACCUMULATE) {
+            if (ws_launch_fft_masks_clear(plan, (cudaStream_t)stream) < 0) return fail(plan, WS_ERR_CUDA, "ws_grid_binned: mask clear failed");
+            plan->occ_grid = grid;
+        }
+        if (plan->occ_grid == grid) {
+            rc = ws_launch_fft_masks(plan, (const uint32_t*)((char*)workspace + plan->last_layout.off_rec_start), (cudaStream_t)stream);
+            if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
+            plan->launches += rc;
+        } else {
+            plan->occ_grid = nullptr;                    // accumulation onto a mesh this plan has no record of
+        }
+    }
     return WS_OK;
 }
 
@@ -277,7 +311,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
                          void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
-    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE)
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: bad mode");
     const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
@@ -286,6 +320,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
 
 int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_planes: null argument");
+    if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_planes: grid must be 16-byte aligned");
     if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
         return fail(plan, WS_ERR_WORKSPACE, "ws_fft_planes: workspace smaller than ws_fft_workspace_bytes");
     if (cufftSetStream(plan->fft, (cudaStream_t)stream) != CUFFT_SUCCESS)
@@ -313,6 +348,56 @@ int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32
     if (rc < 0) return fail(plan, rc, "ws_wcorrect_accumulate: launch failed");
     plan->launches += rc;
     return WS_OK;
+}
+
+// 0 = dense, 1 = sparse, negative = error
+static int fft_sparse_flag(ws_plan* plan, const void* grid, uint32_t fft_flags, const char* who) {
+    if (fft_flags & ~(uint32_t)WS_FFT_USE_OCCUPANCY) return fail(plan, WS_ERR_INVALID_ARG, who);
+    if (!(fft_flags & WS_FFT_USE_OCCUPANCY)) return 0;
+    if (!plan->d_masks || plan->occ_grid != grid) return fail(plan, WS_ERR_INVALID_ARG, who);
+    return 1;
+}
+
+int ws_fft_columns(ws_plan* plan, void* grid, uint32_t fft_flags, void* stream) {
+    if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_columns: null argument");
+    if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_columns: grid must be 16-byte aligned");
+    if (!plan->fft_own) return fail(plan, WS_ERR_UNSUPPORTED, "ws_fft_columns: this plan uses the library FFT");
+    const int sparse = fft_sparse_flag(plan, grid, fft_flags, "ws_fft_columns: bad fft_flags, or no occupancy recorded for this mesh");
+    if (sparse < 0) return sparse;
+    const int rc = ws_launch_fft_cols(plan, (float2*)grid, sparse != 0, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_fft_columns: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t accumulate, float* dirty,
+                         uint32_t fft_flags, void* stream) {
+    if (!plan || !grid || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_rows_wcorrect: null argument");
+    if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_rows_wcorrect: bad flag");
+    if (((uintptr_t)grid | (uintptr_t)image | (uintptr_t)dirty) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_rows_wcorrect: pointers must be 16-byte aligned");
+    if (!plan->fft_own) return fail(plan, WS_ERR_UNSUPPORTED, "ws_fft_rows_wcorrect: this plan uses the library FFT");
+    const int sparse = fft_sparse_flag(plan, grid, fft_flags, "ws_fft_rows_wcorrect: bad fft_flags, or no occupancy recorded for this mesh");
+    if (sparse < 0) return sparse;
+    const int rc = ws_launch_fft_rows(plan, (const float2*)grid, (float2*)image, dirty, accumulate, sparse != 0,
+                                      (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_fft_rows_wcorrect: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_fft_wcorrect(ws_plan* plan, void* grid, void* image, int32_t accumulate, float* dirty, uint32_t fft_flags,
+                    void* workspace, size_t workspace_bytes, void* stream) {
+    if (!plan || !grid || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_wcorrect: null argument");
+    if (!plan->fft_own) {     // library FFT (needs a fully written mesh), then the stand-alone a4 pass
+        if (fft_flags & ~(uint32_t)WS_FFT_USE_OCCUPANCY) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_wcorrect: bad fft_flags");
+        const int rc = ws_fft_planes(plan, grid, workspace, workspace_bytes, stream);
+        if (rc != WS_OK) return rc;
+        return ws_wcorrect_accumulate(plan, grid, image, accumulate, dirty, stream);
+    }
+    const int rc = ws_fft_columns(plan, grid, fft_flags, stream);
+    if (rc != WS_OK) return rc;
+    return ws_fft_rows_wcorrect(plan, grid, image, accumulate, dirty, fft_flags, stream);
 }
 
 int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream) {
@@ -348,11 +433,13 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
         (e = cudaMemcpyAsync(vis_d, vis_h, b_vis, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(wt_d, weights_h, b_wt, cudaMemcpyHostToDevice, st)) != cudaSuccess)
         return cuda_fail(plan, e, "ws_image_from_host: H2D copy");
-    int rc = ws_grid_visibilities(plan, uvw_d, vis_d, wt_d, freq_hz, n_rows, n_chan, grid, WS_GRID_OVERWRITE, workspace,
-                                  workspace_bytes, stream);
+    // the mesh is never cleared nor completely written where the own FFT can skip what the gridder left empty
+    int rc = ws_grid_visibilities(plan, uvw_d, vis_d, wt_d, freq_hz, n_rows, n_chan, grid,
+                                  plan->fft_own ? WS_GRID_SPARSE : WS_GRID_OVERWRITE, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
-    if ((rc = ws_fft_planes(plan, grid, workspace, workspace_bytes, stream)) != WS_OK) return rc;
-    if ((rc = ws_wcorrect_accumulate(plan, grid, image, 0, dirty_d, stream)) != WS_OK) return rc;
+    if ((rc = ws_fft_wcorrect(plan, grid, image, 0, dirty_d, plan->fft_own ? WS_FFT_USE_OCCUPANCY : 0u, workspace,
+                              workspace_bytes, stream)) != WS_OK)
+        return rc;
     if ((e = cudaMemcpyAsync(dirty_h, dirty_d, ws_dirty_bytes(plan), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(plan, e, "ws_image_from_host: D2H copy");
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(plan, e, "ws_image_from_host: synchronize");
@@ -399,6 +486,33 @@ int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_ke
     if (n_dropped) *n_dropped = plan->last_n_vis - (int64_t)s.n_kept;
     if (n_records) *n_records = (int64_t)s.n_records;
     if (s.overflow) return fail(plan, WS_ERR_WORKSPACE, "record capacity of the workspace exceeded: gridding was skipped");
+    return WS_OK;
+}
+
+int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!plan->d_masks || !plan->occ_grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_occupancy: no occupancy recorded");
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_occupancy: synchronize");
+    std::vector<uint32_t> m(plan->mask_words);
+    e = cudaMemcpy(m.data(), plan->d_masks, m.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_occupancy: copy");
+    const size_t nw = (size_t)plan->prm.n_wplanes, nt = (size_t)plan->geom.nt, n_class = nw * nt * 8;
+    size_t t = 0, c = 0, b = 0, p = 0;
+    for (size_t i = 0; i < n_class; ++i) {
+        t += (size_t)__builtin_popcount(m[i]);
+        c += m[i] != 0;
+    }
+    for (size_t k = 0; k < nw; ++k) {
+        size_t nb = 0;
+        for (int i = 0; i < 8; ++i) nb += (size_t)__builtin_popcount(m[n_class + k * 8 + i]);
+        b += nb;
+        p += nb != 0;
+    }
+    if (tiles) *tiles = (double)t / (double)(nw * nt * nt);
+    if (classes) *classes = (double)c / (double)n_class;
+    if (bands) *bands = (double)b / (double)(nw * nt);
+    if (planes) *planes = (double)p / (double)nw;
     return WS_OK;
 }
 

@@ -177,7 +177,7 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
         uint32_t o = base + inc - chunks;
         for (uint32_t lo = s; lo < s + cnt; lo += WS_CHUNK) items[o++] = make_uint4(b, lo, min(lo + WS_CHUNK, s + cnt), 0u);
     }
-    if (mode == WS_GRID_OVERWRITE) {
+    if (mode != WS_GRID_ACCUMULATE) {
         for (unsigned m = hm; m; m &= m - 1) {
             const uint32_t hb = (b - lane) + (__ffs(m) - 1);
             store_zero_tile(tile_origin(g, grid, hb), (size_t)g.n_pix, lane);
@@ -233,7 +233,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         }
         zero_tile<S>(sm.tile, lane);
         accumulate<S>(g, records, s, e, sm, lane);
-        if (mode == WS_GRID_OVERWRITE) {
+        if (mode != WS_GRID_ACCUMULATE) {
 #pragma unroll 4
             for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, sm.tile[y * C::P + lane]);
         } else {

@@ -71,6 +71,13 @@ struct ws_plan {
     bool sorted_keys_valid;
     int sticky_status;
     WsStatus* d_status;                         // plan-owned 64-byte device block: totals and the overflow flag
+    // own FFT (ws_fft.cu): available for N = 2^8 .. 2^13 unless WS_FLAG_LIBRARY_FFT is set
+    bool fft_own;
+    void* d_twiddles;                           // plan-owned inter-stage twiddle tables (fp64-computed, < 140 KB)
+    size_t tw_off_a, tw_off_b;                  // entry offsets of the pass 1a / 1b tables
+    void* d_masks;                              // plan-owned tile-occupancy masks of the mesh (class masks, band masks)
+    size_t mask_words;
+    const void* occ_grid;                       // mesh the masks describe (NULL: none)
 };
 
 static inline size_t ws_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -84,3 +91,10 @@ int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int a
                        cudaStream_t st);
 int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, cudaStream_t st);
 int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);
+bool ws_fft_own_supported(int n_pix);
+int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error
+int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st);
+int ws_launch_fft_rows(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
+                       cudaStream_t st);
+int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st);
+int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, cudaStream_t st);

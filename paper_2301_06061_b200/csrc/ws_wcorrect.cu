@@ -9,29 +9,11 @@
 // phi0, delta and GROUP*delta are formed and range-reduced in fp64 (|w (n-1)| reaches ~10^2 turns, where an
 // fp32 product is 1e-5 rad off), n - 1 as -r^2 / (1 + sqrt(1 - r^2)); only the fraction goes to sincospif.
 #include "ws_internal.h"
+#include "ws_phase.cuh"
 
 namespace {
 
 constexpr int G = WS_WC_GROUP;
-
-struct WcParams {
-    int32_t n_pix, n_wplanes;
-    double cell, w0, dw;      // w0 = w_min + dw/2
-};
-
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
-}
-// acc * r + p
-__device__ __forceinline__ float2 horner(float2 acc, float2 r, float px, float py) {
-    return make_float2(fmaf(acc.x, r.x, fmaf(-acc.y, r.y, px)), fmaf(acc.x, r.y, fmaf(acc.y, r.x, py)));
-}
-__device__ __forceinline__ float2 expi_turns(double turns) {
-    const float f = (float)(turns - rint(turns));   // fraction in [-1/2, 1/2], reduced in fp64
-    float s, c;
-    sincospif(2.0f * f, &s, &c);
-    return make_float2(c, s);
-}
 
 struct PixelPhase {
     float2 e0, r, R;
@@ -39,15 +21,11 @@ struct PixelPhase {
 };
 __device__ __forceinline__ PixelPhase pixel_phase(const WcParams& prm, int q, int p) {
     PixelPhase o;
-    const int half = prm.n_pix >> 1;
-    const double l = (double)(p - half) * prm.cell, m = (double)(q - half) * prm.cell;
-    const double r2 = l * l + m * m;
-    o.inside = r2 < 1.0;
-    const double t = o.inside ? -r2 / (1.0 + sqrt(1.0 - r2)) : 0.0;   // n - 1, never by subtraction
+    const double t = ws_n_minus_1(prm, q, p, &o.inside);   // n - 1, never by subtraction
     const double delta = prm.dw * t;
-    o.e0 = expi_turns(prm.w0 * t);
-    o.r = expi_turns(delta);
-    o.R = expi_turns((double)G * delta);
+    o.e0 = ws_expi_turns(prm.w0 * t);
+    o.r = ws_expi_turns(delta);
+    o.R = ws_expi_turns((double)G * delta);
     return o;
 }
 
@@ -77,14 +55,14 @@ k_wcorrect(const __grid_constant__ WcParams prm, const float4* __restrict__ plan
         float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
 #pragma unroll
         for (int j = G - 1; j >= 0; --j) {
-            hA = horner(hA, A.r, v[j].x, v[j].y);
-            hB = horner(hB, B.r, v[j].z, v[j].w);
+            hA = ws_horner(hA, A.r, v[j].x, v[j].y);
+            hB = ws_horner(hB, B.r, v[j].z, v[j].w);
         }
-        dA = horner(dA, A.R, hA.x, hA.y);
-        dB = horner(dB, B.R, hB.x, hB.y);
+        dA = ws_horner(dA, A.R, hA.x, hA.y);
+        dB = ws_horner(dB, B.R, hB.x, hB.y);
     }
-    dA = cmul(dA, A.e0);
-    dB = cmul(dB, B.e0);
+    dA = ws_cmul(dA, A.e0);
+    dB = ws_cmul(dB, B.e0);
     if (!A.inside) dA = make_float2(0.f, 0.f);   // R14
     if (!B.inside) dB = make_float2(0.f, 0.f);
     float4* dst = image + tid;                    // centred image, row q, pixels p, p+1

@@ -12,12 +12,15 @@ from . import build as _build
 
 WS_GRID_ACCUMULATE = 0
 WS_GRID_OVERWRITE = 1
+WS_FLAG_LIBRARY_FFT = 1
+WS_GRID_SPARSE = 2
+WS_FFT_USE_OCCUPANCY = 1
 
 EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_dirty_image", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count",
 ]
 
@@ -66,6 +69,11 @@ def lib():
         "ws_grid_binned": (C.c_int, [vp, vp, i32, vp, sz, vp]),
         "ws_fft_planes": (C.c_int, [vp, vp, vp, sz, vp]),
         "ws_wcorrect_accumulate": (C.c_int, [vp, vp, vp, i32, vp, vp]),
+        "ws_fft_wcorrect": (C.c_int, [vp, vp, vp, i32, vp, u32, vp, sz, vp]),
+        "ws_fft_columns": (C.c_int, [vp, vp, u32, vp]),
+        "ws_fft_rows_wcorrect": (C.c_int, [vp, vp, vp, i32, vp, u32, vp]),
+        "ws_plan_fft_is_own": (C.c_int, [vp]),
+        "ws_get_occupancy": (C.c_int, [vp] + [C.POINTER(C.c_double)] * 4 + [vp]),
         "ws_dirty_image": (C.c_int, [vp, vp, vp, u32, vp]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
@@ -102,9 +110,9 @@ class Plan:
     """An imaging plan (ws_plan).  All buffers are torch CUDA tensors owned by the caller."""
 
     def __init__(self, n_pix: int, n_wplanes: int, support: int, cell_rad: float, w_min: float, w_max: float,
-                 sigma: float = 1.0, tile: int = 0, device: int = 0):
+                 sigma: float = 1.0, tile: int = 0, device: int = 0, flags: int = 0):
         self._h = C.c_void_p()
-        prm = _Params(n_pix, n_wplanes, support, 0, sigma, cell_rad, w_min, w_max, tile, device, 0)
+        prm = _Params(n_pix, n_wplanes, support, 0, sigma, cell_rad, w_min, w_max, tile, device, flags)
         rc = lib().ws_plan_create(C.byref(prm), C.byref(self._h))
         if rc != 0:
             self._h = C.c_void_p()
@@ -146,6 +154,10 @@ class Plan:
         if dup_factor is None:
             return lib().ws_workspace_bytes(self._h, max_vis)
         return lib().ws_workspace_bytes_for(self._h, max_vis, dup_factor)
+
+    @property
+    def fft_is_own(self) -> bool:
+        return bool(lib().ws_plan_fft_is_own(self._h))
 
     def fft_workspace_bytes(self) -> int:
         return lib().ws_fft_workspace_bytes(self._h)
@@ -205,6 +217,22 @@ class Plan:
                                                  _dev(image, torch.complex64, "image"), int(accumulate), d,
                                                  _stream(stream)))
 
+    def fft_wcorrect(self, grid, image, workspace, accumulate: bool = False, dirty=None, fft_flags: int = 0, stream=None):
+        """a3 + a4 in one call (the mesh is destroyed)."""
+        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
+        self._check(lib().ws_fft_wcorrect(self._h, _dev(grid, torch.complex64, "grid"),
+                                          _dev(image, torch.complex64, "image"), int(accumulate), d, fft_flags,
+                                          _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def fft_columns(self, grid, fft_flags: int = 0, stream=None):
+        self._check(lib().ws_fft_columns(self._h, _dev(grid, torch.complex64, "grid"), fft_flags, _stream(stream)))
+
+    def fft_rows_wcorrect(self, grid, image, accumulate: bool = False, dirty=None, fft_flags: int = 0, stream=None):
+        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
+        self._check(lib().ws_fft_rows_wcorrect(self._h, _dev(grid, torch.complex64, "grid"),
+                                               _dev(image, torch.complex64, "image"), int(accumulate), d, fft_flags,
+                                               _stream(stream)))
+
     def dirty_image(self, image, dirty, stream=None):
         self._check(lib().ws_dirty_image(self._h, _dev(image, torch.complex64, "image"),
                                          _dev(dirty, torch.float32, "dirty"), 0, _stream(stream)))
@@ -223,6 +251,12 @@ class Plan:
             _dev(dev_inputs, torch.uint8, "dev_inputs"), dev_inputs.numel(), _dev(grid, torch.complex64, "grid"),
             _dev(image, torch.complex64, "image"), _dev(dirty_d, torch.float32, "dirty_d"), dirty_h.data_ptr(),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def occupancy(self, stream=None) -> dict:
+        """Fractions of the mesh marked non-empty by the gridding calls: tiles, classes, bands, planes."""
+        v = [C.c_double() for _ in range(4)]
+        self._check(lib().ws_get_occupancy(self._h, *[C.byref(x) for x in v], _stream(stream)))
+        return dict(zip(("tiles", "classes", "bands", "planes"), (x.value for x in v)))
 
     def async_status(self, stream=None):
         self._check(lib().ws_async_status(self._h, _stream(stream)))

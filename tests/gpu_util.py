@@ -22,7 +22,11 @@ def logical(grid_stored: torch.Tensor) -> np.ndarray:
 
 
 def run_chain(d, plan=None, want_bins=True, dup_factor=None):
-    """grid (logical order, numpy complex64), image (numpy complex64), dirty, bins of the GPU path."""
+    """The GPU path through the C ABI.  Returns grid (logical order, numpy complex64, from an OVERWRITE gridding),
+    bins, and three images of the same inputs: `image` = the configuration bench.py times (WS_GRID_SPARSE onto a
+    NaN-filled mesh, own FFT with fused w-correction skipping what the gridder left empty; the library path where
+    the plan has no own FFT), `image_library` = cuFFT + stand-alone w-correction + ws_dirty_image, `image_dense` =
+    own FFT without occupancy.  `dirty` belongs to `image`."""
     import paper_2301_06061_b200 as ws
     dev = d.to("cuda")
     plan = plan or make_plan(d)
@@ -33,11 +37,28 @@ def run_chain(d, plan=None, want_bins=True, dup_factor=None):
     bins = plan.get_bins() if want_bins else None
     plan.async_status()
     g = logical(grid)
+    out = dict(grid=g, bins=bins, plan=plan)
+    if plan.fft_is_own:
+        image_d = plan.alloc_image()
+        plan.fft_wcorrect(grid, image_d, wsp, accumulate=False, dirty=None, fft_flags=0)
+        out["image_dense"] = image_d.cpu().numpy()
+        grid.fill_(float("nan"))
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_OVERWRITE)
     plan.fft_planes(grid, wsp)
-    plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=None)
-    plan.dirty_image(image, dirty)
+    image_l, dirty_l = plan.alloc_image(), plan.alloc_dirty()
+    plan.wcorrect_accumulate(grid, image_l, accumulate=False, dirty=None)
+    plan.dirty_image(image_l, dirty_l)
+    out["image_library"], out["dirty_library"] = image_l.cpu().numpy(), dirty_l.cpu().numpy()
+    if plan.fft_is_own:
+        grid.fill_(float("nan"))  # WS_GRID_SPARSE leaves empty tiles alone; the FFT must never read them
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_SPARSE)
+        plan.fft_wcorrect(grid, image, wsp, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+        plan.async_status()
+        out["image"], out["dirty"] = image.cpu().numpy(), dirty.cpu().numpy()
+    else:
+        out["image"], out["dirty"] = out["image_library"], out["dirty_library"]
     torch.cuda.synchronize()
-    return dict(grid=g, image=image.cpu().numpy(), dirty=dirty.cpu().numpy(), bins=bins, plan=plan)
+    return out
 
 
 def errors(x: np.ndarray, ref: np.ndarray):

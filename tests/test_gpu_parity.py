@@ -22,12 +22,16 @@ def _full_check(oracle, d, **kw):
     eg = U.assert_close(out["grid"], G, "grid")
     ei = U.assert_close(out["image"], D, "image")
     assert np.array_equal(out["dirty"], out["image"].real)
+    U.assert_close(out["image_library"], D, "image (cuFFT + stand-alone w-correction)")
+    assert np.array_equal(out["dirty_library"], out["image_library"].real)
+    if "image_dense" in out:
+        U.assert_close(out["image_dense"], D, "image (own FFT, no occupancy)")
     return out, eg, ei
 
 
 def test_library_loaded_is_the_cuda_one():
     import paper_2301_06061_b200 as ws
-    assert ws.lib().ws_version() == 100
+    assert ws.lib().ws_version() == 110
     assert torch.cuda.is_available()
 
 
@@ -36,6 +40,7 @@ def test_tiny_config(oracle):
     out, eg, ei = _full_check(oracle, d)
     print("tiny grid/image errors", eg, ei)
     assert out["plan"].launch_count() >= 9
+    assert out["plan"].fft_is_own
 
 
 @pytest.mark.parametrize("support", [1, 3, 5, 7, 9, 11, 13, 15])
@@ -111,6 +116,73 @@ def test_wcorrect_accumulate_flag_and_fused_dirty(oracle):
     U.assert_close(image.cpu().numpy(), 2 * ref, "w-correction, accumulate")
 
 
+@pytest.mark.parametrize("n_pix,n_wplanes", [(256, 3), (512, 2), (1024, 2), (2048, 3), (256, 70), (512, 130)])
+def test_own_fft_fused_wcorrect_on_arbitrary_planes(oracle, n_pix, n_wplanes):
+    # a3 + a4 of the own FFT (dense: any mesh contents) against the oracle's transform + w-correction, every
+    # supported stage plan that fits a quick test; 70 and 130 planes cross the 64-plane Horner chains
+    d = make_random_dataset(20 + n_wplanes, 10, 1, n_pix, n_wplanes, 7, w_span=250.0, cell_rad=0.6 / n_pix)
+    plan = U.make_plan(d)
+    assert plan.fft_is_own
+    rng = np.random.default_rng(n_pix + n_wplanes)
+    G = (rng.standard_normal((n_wplanes, n_pix, n_pix)) + 1j * rng.standard_normal((n_wplanes, n_pix, n_pix))).astype(np.complex64)
+    prm = U.oracle_params(oracle, d, plan.tile)
+    ref = np.zeros((n_pix, n_pix), np.complex128)
+    for k in range(n_wplanes):
+        oracle.wcorrect(prm, oracle.transform(G[k].astype(np.complex128))[None], k, ref)
+    stored = torch.fft.ifftshift(torch.from_numpy(G).cuda(), dim=(-2, -1)).contiguous()
+    keep = stored.clone()
+    image, dirty = plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(16)
+    plan.fft_wcorrect(stored, image, wsp, accumulate=False, dirty=dirty)
+    print("own fft + wcorrect", n_pix, n_wplanes, U.assert_close(image.cpu().numpy(), ref, "fused image"))
+    assert np.array_equal(dirty.cpu().numpy(), image.cpu().numpy().real)
+    stored.copy_(keep)
+    plan.fft_columns(stored)                       # the two halves as separate calls, accumulating
+    plan.fft_rows_wcorrect(stored, image, accumulate=True, dirty=dirty)
+    U.assert_close(image.cpu().numpy(), 2 * ref, "fused image, accumulate")
+    assert np.array_equal(dirty.cpu().numpy(), image.cpu().numpy().real)
+
+
+def test_library_fft_flag_and_occupancy_rules(oracle):
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(31, 3000, 1, 256, 4, 7, fill=0.7, w_span=30.0, cell_rad=2e-3)
+    lib = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, flags=ws.WS_FLAG_LIBRARY_FFT)
+    assert not lib.fft_is_own
+    out = U.run_chain(d, plan=lib)
+    prm = U.oracle_params(oracle, d, lib.tile)
+    U.assert_close(out["image"], oracle.dirty_image(prm, *_np(d)), "image, library FFT plan")
+    dev = d.to("cuda")
+    grid, image, wsp = lib.alloc_grid(), lib.alloc_image(), lib.alloc_workspace(d.n_vis)
+    with pytest.raises(ws.WStackError):            # a sparse mesh is only meaningful to the own FFT
+        lib.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_SPARSE)
+    with pytest.raises(ws.WStackError):
+        lib.fft_columns(grid)
+    lib.fft_wcorrect(grid, image, wsp)             # falls back to the two library calls
+    own = U.make_plan(d)
+    other = own.alloc_grid()
+    own.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_SPARSE)
+    with pytest.raises(ws.WStackError):            # occupancy was recorded for `grid`, not for `other`
+        own.fft_wcorrect(other, image, wsp, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    occ = own.occupancy()
+    assert 0 < occ["tiles"] <= occ["classes"] <= occ["bands"] <= occ["planes"] <= 1
+
+
+def test_chunked_accumulate_keeps_occupancy_of_all_chunks(oracle):
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(32, 8000, 2, 512, 6, 7, wavelengths=False, fill=0.95, w_span=60.0, cell_rad=1e-3)
+    plan = U.make_plan(d)
+    dev = d.to("cuda")
+    grid, image = plan.alloc_grid(), plan.alloc_image()
+    wsp = plan.alloc_workspace(d.n_vis)
+    for i, (lo, hi) in enumerate(((0, 3000), (3000, 8000))):      # rows sorted by nothing: chunks touch different tiles
+        plan.grid_visibilities(dev.uvw[lo:hi].contiguous(), dev.vis[lo:hi].contiguous(), dev.weights[lo:hi].contiguous(),
+                               d.freqs_hz, grid, wsp, mode=ws.WS_GRID_OVERWRITE if i == 0 else ws.WS_GRID_ACCUMULATE)
+    plan.fft_wcorrect(grid, image, wsp, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    plan.async_status()
+    prm = U.oracle_params(oracle, d, plan.tile)
+    U.assert_close(image.cpu().numpy(), oracle.dirty_image(prm, *_np(d)), "image from two chunks, occupancy-aware FFT")
+
+
 def test_fft_planes_matches_oracle_transform(oracle):
     d = make_random_dataset(13, 10, 1, 256, 3, 7)
     plan = U.make_plan(d)
@@ -145,7 +217,8 @@ def test_small_workspace_reports_overflow(oracle):
 
 def test_argument_validation():
     import paper_2301_06061_b200 as ws
-    for bad in (dict(n_pix=250), dict(support=8), dict(support=17), dict(w_max=-5.0), dict(cell_rad=0.0), dict(tile=64)):
+    for bad in (dict(n_pix=250), dict(support=8), dict(support=17), dict(w_max=-5.0), dict(cell_rad=0.0), dict(tile=64),
+                dict(flags=8)):
         kw = dict(n_pix=256, n_wplanes=4, support=7, cell_rad=1e-3, w_min=-1.0, w_max=1.0)
         kw.update(bad)
         with pytest.raises(ws.WStackError):
