@@ -168,7 +168,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
         return WS_ERR_CUDA;
     }
     // a3: the FFT of ws_fft.cu where it exists (N = 2^8 .. 2^13), else (or on request) the library's
-    plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix);
+    plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix, p->n_wplanes);
     plan->d_twiddles = nullptr;
     plan->d_masks = nullptr;
     plan->mask_words = 0;

@@ -31,21 +31,26 @@
 
 namespace {
 
-constexpr int FT = 256;            // threads per CTA
-constexpr int EPT = 32;            // points per thread
-constexpr int PTS = FT * EPT;      // points per CTA
+constexpr int CT = 256;            // threads per CTA of the column kernels
+constexpr int FT = 512;            // threads per CTA of the row kernel: two groups of 8 warps
+constexpr int GT = 256;            // threads per group
+constexpr int PT = 128;            // the producer's warpgroup (one warp of it works): register re-allocation is per warpgroup
+constexpr int EPT = 16;            // points per thread
+constexpr int PTS = FT * EPT;      // points per CTA (8192)
+constexpr int MAX_PLANES = 4096;   // w-planes the row kernel's per-plane occupancy bits provide for
 constexpr int WC_SPAN = 64;        // planes per Horner chain of the fused w-correction (exact restart between chains)
 
-// ---- stage plan: N = prod R_s ------------------------------------------------------------------------------
-__host__ __device__ constexpr int n_stages(int logn) { return logn <= 10 ? 2 : 3; }
+// ---- stage plan of the row transform: N = prod R_s ---------------------------------------------------------------
+__host__ __device__ constexpr int n_stages(int logn) { return logn == 8 ? 2 : 3; }
 __host__ __device__ constexpr int log2r(int logn, int s) {
+    if (s >= n_stages(logn)) return 0;
     switch (logn) {
-        case 8: return s < 2 ? 4 : 0;                       // 16 16
-        case 9: return s == 0 ? 5 : (s == 1 ? 4 : 0);       // 32 16
-        case 10: return s < 2 ? 5 : 0;                      // 32 32
-        case 11: return s < 2 ? 4 : (s == 2 ? 3 : 0);       // 16 16 8
-        case 12: return s < 3 ? 4 : 0;                      // 16 16 16
-        case 13: return s == 0 ? 5 : (s < 3 ? 4 : 0);       // 32 16 16
+        case 8: return 4;                                   // 16 16
+        case 9: return s < 2 ? 4 : 1;                       // 16 16 2
+        case 10: return s < 2 ? 4 : 2;                      // 16 16 4
+        case 11: return s < 2 ? 4 : 3;                      // 16 16 8
+        case 12: return 4;                                  // 16 16 16
+        case 13: return s == 0 ? 5 : 4;                     // 32 16 16 (the radix-32 butterflies are split over two threads)
     }
     return 0;
 }
@@ -84,6 +89,7 @@ __device__ __forceinline__ int freq_of(int n) {
     }
     return f;
 }
+
 
 // ---- complex helpers -------------------------------------------------------------------------------------------
 __device__ __forceinline__ float2 eadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -140,90 +146,6 @@ __device__ __forceinline__ void bfly(E* x) {
     }
 }
 
-// ---- one stage of the CTA-wide transform -------------------------------------------------------------------
-// Stage with sub-transform length L = 2^LOGL and radix R = 2^LOGR (Q = L / R): butterfly b of the CTA
-// (b = t + 256 i, i < 32 / R) takes the points base + m Q, m < R, base = (b / Q) L + (b mod Q), and leaves
-// Y[m'] W_L^(j m') at base + m' Q (j = b mod Q): in place, so consecutive stages need one barrier only.
-template <int LOGL, int LOGR>
-__device__ __forceinline__ int stage_base(int b) {
-    constexpr int LOGQ = LOGL - LOGR;
-    return ((b >> LOGQ) << LOGL) + (b & ((1 << LOGQ) - 1));
-}
-
-template <typename E, int LOGL, int LOGR, bool PADDED>
-__device__ __forceinline__ void stage_load(E* x, const E* __restrict__ src, int t) {
-    constexpr int R = 1 << LOGR, LOGQ = LOGL - LOGR;
-#pragma unroll
-    for (int i = 0; i < EPT / R; ++i) {
-        const int base = stage_base<LOGL, LOGR>(t + FT * i);
-#pragma unroll
-        for (int m = 0; m < R; ++m) {
-            const int p = base + (m << LOGQ);
-            x[i * R + m] = src[PADDED ? pad(p) : p];
-        }
-    }
-}
-
-template <typename E, int LOGL, int LOGR>
-__device__ __forceinline__ void stage_compute(E* x, const float2* __restrict__ tw, int t) {
-    constexpr int R = 1 << LOGR, LOGQ = LOGL - LOGR, Q = 1 << LOGQ;
-#pragma unroll
-    for (int i = 0; i < EPT / R; ++i) {
-        bfly<E, LOGR>(x + i * R);
-        if (LOGQ > 0) {
-            const int j = (t + FT * i) & (Q - 1);
-#pragma unroll
-            for (int r = 1; r < R; ++r) {
-                const float2 w = tw[(brev(r, LOGR) - 1) * Q + j];
-                x[i * R + r] = emul(x[i * R + r], w.x, w.y);
-            }
-        }
-    }
-}
-
-template <typename E, int LOGL, int LOGR>
-__device__ __forceinline__ void stage_store(const E* x, E* __restrict__ dst, int t) {
-    constexpr int R = 1 << LOGR, LOGQ = LOGL - LOGR;
-#pragma unroll
-    for (int i = 0; i < EPT / R; ++i) {
-        const int base = stage_base<LOGL, LOGR>(t + FT * i);
-#pragma unroll
-        for (int r = 0; r < R; ++r) dst[pad(base + (brev(r, LOGR) << LOGQ))] = x[i * R + r];
-    }
-}
-
-// Stages 1 .. S-1 on the padded work buffer; the first stage's results must already be in `work` (not yet
-// synchronised).  On return x[] holds the transform: register i*R + r of thread t is position
-// ((t + 256 i) R + brev(r)) of the CTA, R the radix of the last stage.
-template <typename E, int LOGN>
-__device__ __forceinline__ void later_stages(E* x, E* work, const float2* tw, int t) {
-    constexpr int S = n_stages(LOGN);
-    __syncthreads();
-    if (S == 3) {
-        constexpr int L1 = log2l(LOGN, 1), R1 = log2r(LOGN, 1);
-        stage_load<E, L1, R1, true>(x, work, t);
-        stage_compute<E, L1, R1>(x, tw + tw_offset(LOGN, 1), t);
-        stage_store<E, L1, R1>(x, work, t);
-        __syncthreads();
-    }
-    constexpr int LL = log2l(LOGN, S - 1), RL = log2r(LOGN, S - 1);
-    static_assert(LL == RL, "last stage must have Q = 1");
-    stage_load<E, LL, RL, true>(x, work, t);
-    stage_compute<E, LL, RL>(x, tw, t);
-}
-
-// CTA position of register slot `slot` after later_stages()
-template <int LOGN>
-__device__ __forceinline__ int final_pos(int slot, int t) {
-    constexpr int RL = log2r(LOGN, n_stages(LOGN) - 1), R = 1 << RL;
-    return ((t + FT * (slot / R)) << RL) + brev(slot % R, RL);
-}
-
-__device__ __forceinline__ void load_twiddles(float2* tw_s, const float2* __restrict__ tw_g, int n, int t) {
-    for (int i = t; i < n; i += FT) tw_s[i] = tw_g[i];
-}
-
-
 // ---- occupancy masks -----------------------------------------------------------------------------------------
 // Storage (FFT-native) tile coordinates.  class_mask[(k nt + tx) 8 + c]: bit m set <=> tile (ty = c + 8 m, tx) of
 // plane k holds visibilities (the R0 inputs of pass 1a's butterflies on the rows of class c = (row mod 256) / 32).
@@ -254,7 +176,7 @@ k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_c
 // Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
 // row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
 template <int LOGN>
-__global__ void __launch_bounds__(FT)
+__global__ void __launch_bounds__(CT)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ class_mask,
            uint32_t n_items) {
     constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32;
@@ -285,7 +207,7 @@ k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 // Item = (plane, column band tx, block m0 of 256 rows).  Warp w, lane = column.  Stage 1: j in {w, w + 8}, rows
 // j + 16 m; stage 2: blocks b in {w, w + 8}, rows 16 b + m; frequency f = b + 16 m' is stored at row 256 m0 + f.
 template <int LOGN>
-__global__ void __launch_bounds__(FT, 2)
+__global__ void __launch_bounds__(CT, 2)
 k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ class_mask,
            uint32_t n_items) {
     constexpr int N = 1 << LOGN, R0 = 1 << (LOGN - 8), NT = N / 32;
@@ -369,8 +291,16 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // `pos` holds v-frequency (pos >> 8) + R0 (pos & 255) (pass 1b).  Planes are visited from the top one down so that
 // the phase screen is applied by Horner's rule: h <- h r + P_k, r = exp(2 pi i dw t); every WC_SPAN planes the
 // chain is closed with the exactly evaluated phase of its lowest plane and restarted.
+//
+// 512 threads x 16 points.  Stage s, radix R: butterfly b takes the points base + m Q (Q = L / R, base =
+// (b / Q) L + b mod Q) and leaves Y[m'] W_L^(j m') at base + m' Q: in place.  For N >= 4096 the CTA is two groups
+// of 8 warps that share nothing but the landing buffer, each with its own named barrier, so that one group's
+// exchanges overlap the other's arithmetic: N = 4096: a group per row; N = 8192: the first stage is radix 32 with
+// each butterfly split over the two groups by the parity of its outputs (both read its 32 inputs; the even half
+// is the 16-point transform of a + b, the odd half that of (a - b) W_32^m), after which the blocks of even and
+// odd first digit are separate problems.
 // band_mask (or NULL = dense): only the non-empty 32-column bands of a plane are copied in, as maximal runs; a
-// band that is empty now but was filled by the previous copy is cleared by the CTA; a plane without any is skipped.
+// band that is empty now but was filled by the previous copy is cleared first; a plane without any is skipped.
 struct BandMask {
     uint32_t w[8];
 };
@@ -380,7 +310,7 @@ __device__ __forceinline__ BandMask load_bands(const uint32_t* __restrict__ band
     for (int i = 0; i < 8; ++i) {
         const int lo = 32 * i;
         const uint32_t full = nt >= lo + 32 ? 0xFFFFFFFFu : (nt > lo ? (1u << (nt - lo)) - 1u : 0u);
-        b.w[i] = band_mask ? (__ldg(band_mask + k * 8 + i) & full) : full;
+        b.w[i] = band_mask ? (band_mask[k * 8 + i] & full) : full;
     }
     return b;
 }
@@ -390,68 +320,294 @@ __device__ __forceinline__ bool any_band(const BandMask& b) {
     for (int i = 0; i < 8; ++i) o |= b.w[i];
     return o != 0;
 }
+template <int LOGN>
+struct RowCfg {
+    static constexpr int N = 1 << LOGN, ROWS = PTS / N, NT = N / 32, R0 = 1 << (LOGN - 8);
+    static constexpr int S = n_stages(LOGN);
+    static constexpr bool GROUPED = LOGN >= 12;       // two independent 8-warp groups
+    static constexpr bool SPLIT32 = LOGN == 13;       // first stage: radix 32 split over the groups
+    static constexpr int LRL = log2r(LOGN, S - 1);    // last stage
+};
+
+// butterfly i of thread u in stage s (s >= 1, or any stage when not SPLIT32)
+template <int LOGN>
+__device__ __forceinline__ int bfly_id(int u, int i) {
+    if constexpr (RowCfg<LOGN>::SPLIT32) return (((u & 255) >> 4) << 5) | ((u >> 8) << 4) | (u & 15);   // first digit parity = group
+    return u + FT * i;
+}
+template <int LOGL, int LOGR>
+__device__ __forceinline__ int stage_base(int b) {
+    constexpr int LOGQ = LOGL - LOGR;
+    return ((b >> LOGQ) << LOGL) + (b & ((1 << LOGQ) - 1));
+}
+
+// generic stage on the padded work buffer (or, FIRST, from the unpadded landing buffer): load, butterfly, and unless
+// LAST twiddle + store.  After the LAST stage x[i R + r] is position (bfly_id(u, i) << LOGR) + brev(r).
+template <int LOGN, int STAGE, bool FIRST, bool LAST>
+__device__ __forceinline__ void row_stage(float2* x, const float2* __restrict__ src, float2* __restrict__ work,
+                                          const float2* __restrict__ tw, int u) {
+    constexpr int LOGL = log2l(LOGN, STAGE), LOGR = log2r(LOGN, STAGE), LOGQ = LOGL - LOGR, R = 1 << LOGR, Q = 1 << LOGQ;
+#pragma unroll
+    for (int i = 0; i < EPT / R; ++i) {
+        const int b = bfly_id<LOGN>(u, i), base = stage_base<LOGL, LOGR>(b);
+        float2* xi = x + i * R;
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            const int p = base + (m << LOGQ);
+            xi[m] = src[FIRST ? p : pad(p)];
+        }
+    }
+    if constexpr (!FIRST) {  // (FIRST: the caller releases the landing buffer before the arithmetic)
+#pragma unroll
+    for (int i = 0; i < EPT / R; ++i) {
+        const int b = bfly_id<LOGN>(u, i), base = stage_base<LOGL, LOGR>(b);
+        float2* xi = x + i * R;
+        bfly<float2, LOGR>(xi);
+        if (!LAST) {
+            const int j = b & (Q - 1);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                float2 v = xi[r];
+                if (r) {
+                    const float2 w = tw[tw_offset(LOGN, STAGE) + (brev(r, LOGR) - 1) * Q + j];
+                    v = emul(v, w.x, w.y);
+                }
+                work[pad(base + (brev(r, LOGR) << LOGQ))] = v;
+            }
+        }
+    }
+    }
+}
+// arithmetic + store of a first stage whose inputs are already in x[]
+template <int LOGN>
+__device__ __forceinline__ void first_stage_finish(float2* x, float2* __restrict__ work, const float2* __restrict__ tw, int u) {
+    constexpr int LOGL = LOGN, LOGR = log2r(LOGN, 0), LOGQ = LOGL - LOGR, R = 1 << LOGR, Q = 1 << LOGQ;
+    static_assert(R == EPT, "first stage: one radix-16 butterfly per thread");
+    const int b = u, base = stage_base<LOGL, LOGR>(b), j = b & (Q - 1);
+    bfly<float2, LOGR>(x);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        float2 v = x[r];
+        if (r) {
+            const float2 w = tw[(brev(r, LOGR) - 1) * Q + j];
+            v = emul(v, w.x, w.y);
+        }
+        work[pad(base + (brev(r, LOGR) << LOGQ))] = v;
+    }
+}
+
+// row (within the super-row) and frequency of register slot `slot` after the last stage
+template <int LOGN>
+__device__ __forceinline__ int final_pos(int slot, int u);
+template <int LOGN>
+__device__ __forceinline__ int slot_row(int slot, int u) {
+    if constexpr (LOGN == 13) return 0;
+    else if constexpr (LOGN == 12) return u >> 8;
+    else return final_pos<LOGN>(slot, u) >> LOGN;
+}
+template <int LOGN>
+__device__ __forceinline__ int slot_freq(int slot, int u) {
+    const int ug = u & 255, g = u >> 8;
+    if constexpr (LOGN == 13) return (2 * (ug >> 4) + g) + 32 * (ug & 15) + 512 * brev(slot, 4);
+    else if constexpr (LOGN == 12) return (ug >> 4) + 16 * (ug & 15) + 256 * brev(slot, 4);
+    else return freq_of<LOGN>(final_pos<LOGN>(slot, u) & ((1 << LOGN) - 1));
+}
+// CTA position of register slot `slot` after the last stage (generic path)
+template <int LOGN>
+__device__ __forceinline__ int final_pos(int slot, int u) {
+    constexpr int LRL = RowCfg<LOGN>::LRL, R = 1 << LRL;
+    return (bfly_id<LOGN>(u, slot / R) << LRL) + brev(slot % R, LRL);
+}
+
+// ---- the two-group path (N = 4096, 8192) with every shared-memory address in the form base + constant ---------
+// Padded index of position blk * 256 + x (x < 256) is blk * 272 + x + (x >> 4).  Group g, thread ug < 256:
+//   first stage   j = ug: 32 (N = 8192) or 16 (N = 4096, row g) inputs j + 256 m from `landing`; output digit d goes
+//                 to block d (N = 8192: d = 2 brev(r) + g; N = 4096: block 16 g + brev(r)) at x = j;
+//   second stage  block blk = (N = 8192: 2 (ug >> 4) + g; N = 4096: 16 g + (ug >> 4)), jj = ug & 15, points jj + 16 m;
+//   third stage   points 16 jj + m of the same block: they were written by the 16 lanes that share blk, so the
+//                 exchange between the last two stages needs a warp barrier only.
+template <int LOGN>
+struct Grouped {
+    static constexpr bool SPLIT32 = LOGN == 13;
+    __device__ static __forceinline__ int blk(int ug, int g) { return SPLIT32 ? 2 * (ug >> 4) + g : 16 * g + (ug >> 4); }
+    // frequency of register r after the third stage
+    __device__ static __forceinline__ int freq(int ug, int g, int r) {
+        return SPLIT32 ? (2 * (ug >> 4) + g) + 32 * (ug & 15) + 512 * brev(r, 4) : (ug >> 4) + 16 * (ug & 15) + 256 * brev(r, 4);
+    }
+    __device__ static __forceinline__ void load_first(float2* x, const float2* __restrict__ landing, int ug, int g) {
+        if constexpr (SPLIT32) {
+            const float2* in = landing + ug;
+            if (g == 0) {
+#pragma unroll
+                for (int m = 0; m < 16; ++m) x[m] = eadd(in[256 * m], in[256 * (m + 16)]);
+            } else {
+#pragma unroll
+                for (int m = 0; m < 16; ++m) x[m] = mul_w32(esub(in[256 * m], in[256 * (m + 16)]), m);
+            }
+        } else {
+            const float2* in = landing + g * 4096 + ug;
+#pragma unroll
+            for (int m = 0; m < 16; ++m) x[m] = in[256 * m];
+        }
+    }
+    __device__ static __forceinline__ void finish_first(float2* x, float2* __restrict__ work, const float2* __restrict__ tw,
+                                                        int ug, int g) {
+        bfly<float2, 4>(x);
+        if constexpr (SPLIT32) {
+            float2* out = work + g * 272 + ug + (ug >> 4);
+            const float2* t = tw + ug + (g - 1) * 256;              // tw[(d - 1) 256 + j], d = 2 brev(r) + g
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                float2 v = x[r];
+                if (r) {
+                    const float2 w = t[brev(r, 4) * 512];
+                    v = emul(v, w.x, w.y);
+                } else if (g) {
+                    const float2 w = t[0];
+                    v = emul(v, w.x, w.y);
+                }
+                out[brev(r, 4) * 544] = v;
+            }
+        } else {
+            float2* out = work + g * (16 * 272) + ug + (ug >> 4);
+            const float2* t = tw + ug - 256;                        // tw[(m' - 1) 256 + j]
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                float2 v = x[r];
+                if (r) {
+                    const float2 w = t[brev(r, 4) * 256];
+                    v = emul(v, w.x, w.y);
+                }
+                out[brev(r, 4) * 272] = v;
+            }
+        }
+    }
+    __device__ static __forceinline__ void second_third(float2* x, float2* __restrict__ work, const float2* __restrict__ tw,
+                                                        int ug, int g) {
+        const int jj = ug & 15;
+        float2* b1 = work + blk(ug, g) * 272 + jj;
+        const float2* t = tw + tw_offset(LOGN, 1) + jj - 16;        // tw1[(m' - 1) 16 + jj]
+#pragma unroll
+        for (int m = 0; m < 16; ++m) x[m] = b1[17 * m];
+        bfly<float2, 4>(x);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            float2 v = x[r];
+            if (r) {
+                const float2 w = t[brev(r, 4) * 16];
+                v = emul(v, w.x, w.y);
+            }
+            b1[17 * brev(r, 4)] = v;
+        }
+        __syncwarp();
+        const float2* b2 = work + blk(ug, g) * 272 + 17 * jj;
+#pragma unroll
+        for (int m = 0; m < 16; ++m) x[m] = b2[m];
+        bfly<float2, 4>(x);
+    }
+};
 
 template <int LOGN>
-__global__ void __launch_bounds__(FT, 1)
+__global__ void __launch_bounds__(FT + PT, 1)
 k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ planes, float2* __restrict__ image,
            float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g,
            const uint32_t* __restrict__ band_mask, uint32_t n_super) {
-    constexpr int N = 1 << LOGN, ROWS = PTS / N, NT = N / 32, R0 = 1 << (LOGN - 8);
-    constexpr int L0 = LOGN, LR0 = log2r(LOGN, 0);
+    using C = RowCfg<LOGN>;
+    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* landing = (float2*)smem_raw;
     float2* work = landing + PTS;
     float2* tw = work + PAD_PTS;
-    uint64_t* bar = (uint64_t*)(tw + ((tw_entries(LOGN) + 1) & ~1));
-    const int t = threadIdx.x;
+    uint64_t* full = (uint64_t*)(tw + ((tw_entries(LOGN) + 1) & ~1));   // the copy of a plane has landed
+    uint64_t* empty = full + 1;                                         // every group has consumed it
+    uint32_t* s_any = (uint32_t*)(empty + 1);                           // bit k: plane k has a non-empty band
+    const int u = threadIdx.x, g = u >> 8;
     const int nw = prm.n_wplanes;
     const size_t plane_elems = (size_t)N * N;
-    load_twiddles(tw, tw_g, tw_entries(LOGN), t);
-#pragma unroll
-    for (int i = 0; i < EPT; ++i) landing[t + FT * i] = make_float2(0.f, 0.f);
+    for (int i = u; i < tw_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
+    for (int i = u; i < PTS; i += FT + PT) landing[i] = make_float2(0.f, 0.f);
+    for (int k0 = 0; k0 < nw; k0 += FT + PT) {       // (FT + PT is a multiple of 32: one ballot per mask word)
+        const int k = k0 + u;
+        bool any = false;
+        if (k < nw) any = any_band(load_bands(band_mask, k, NT));
+        const uint32_t bits = __ballot_sync(0xffffffffu, any);
+        if ((u & 31) == 0 && k < nw) s_any[k >> 5] = bits;
+    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    if (t == 0) mbar_init(bar, 1);
+    if (u == 0) {
+        mbar_init(full, 1);
+        mbar_init(empty, C::GROUPED ? 2 : 1);
+    }
     __syncthreads();
     if (blockIdx.x >= n_super) return;
 
-    // Lane 0 of warp w brings the non-empty bands of word w (32 bands, 8 KB per row) of super-row sr of plane k into
-    // `landing`, one bulk copy per maximal run; thread 0 posts the byte count (the copies of the other warps may
-    // complete before it does: the phase cannot, it needs this arrival).
-    auto issue = [&](uint32_t sr, int k, const BandMask& bm) {
-        if (t & 31) return;
-        if (t == 0) {
-            uint32_t n_bands = 0;
+    if (u >= FT) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (u >= FT + 32) return;
+        // ---- producer warp: clears the bands of `landing` that the last copy filled and the next one will not, then
+        // brings the non-empty bands of the next plane in.  Lane wi < 8 owns mask word wi (32 bands = 8 KB per row)
+        // and issues one bulk copy per maximal run of set bits.
+        const int lane = u & 31;
+        uint32_t was = 0, e_parity = 0;
+        bool first = true;
+        for (uint32_t sr = blockIdx.x; sr < n_super; sr += gridDim.x) {
+            for (int k = nw - 1; k >= 0; --k) {
+                if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
+                uint32_t now = 0;
+                if (lane < 8) {
+                    const int lo = 32 * lane;
+                    const uint32_t fullw = NT >= lo + 32 ? 0xFFFFFFFFu : (NT > lo ? (1u << (NT - lo)) - 1u : 0u);
+                    now = band_mask ? (__ldg(band_mask + k * 8 + lane) & fullw) : fullw;
+                }
+                // what needs neither `landing` nor the barrier happens before the wait for the consumers
+                uint32_t n_bands = __popc(now);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) n_bands += __popc(bm.w[i]);
-            mbar_expect_tx(bar, n_bands * 256u * ROWS);
-        }
-        const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * PTS);
-        uint32_t m = 0;
+                for (int d = 16; d >= 1; d >>= 1) n_bands += __shfl_xor_sync(0xffffffffu, n_bands, d);
+                const uint32_t stale = was & ~now;
+                const bool any_stale = __any_sync(0xffffffffu, stale != 0);
+                if (!first) {
+                    while (!mbar_try_wait(empty, e_parity)) {}
+                    e_parity ^= 1u;
+                }
+                first = false;
+                if (lane == 0) mbar_expect_tx(full, n_bands * 256u * ROWS);     // (the previous phase is complete now)
+                if (any_stale) {
 #pragma unroll
-        for (int wi = 0; wi < 8; ++wi) m = (t >> 5) == wi ? bm.w[wi] : m;
-        while (m) {
-            const int b0 = __ffs(m) - 1;
-            const uint32_t inv = ~(m >> b0);
-            const int len = inv ? __ffs(inv) - 1 : 32;
-            m &= ~((len == 32 ? 0xFFFFFFFFu : (1u << len) - 1u) << b0);
-            const size_t off = (size_t)((t >> 5) * 32 + b0) * 256;
-            for (int r = 0; r < ROWS; ++r)
-                bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, bar);
+                    for (int wi = 0; wi < 8; ++wi) {
+                        uint32_t z = __shfl_sync(0xffffffffu, stale, wi);
+                        while (z) {
+                            const int b = wi * 32 + __ffs(z) - 1;
+                            z &= z - 1;
+                            for (int r = 0; r < ROWS; ++r) landing[r * N + b * 32 + lane] = make_float2(0.f, 0.f);
+                        }
+                    }
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncwarp();
+                }
+                const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * PTS);
+                uint32_t m = now;
+                while (m) {
+                    const int b0 = __ffs(m) - 1;
+                    const uint32_t inv = ~(m >> b0);
+                    const int len = inv ? __ffs(inv) - 1 : 32;
+                    m &= ~((len == 32 ? 0xFFFFFFFFu : (1u << len) - 1u) << b0);
+                    const size_t off = (size_t)(lane * 32 + b0) * 256;
+                    for (int r = 0; r < ROWS; ++r)
+                        bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, full);
+                }
+                was = now;
+            }
         }
-    };
-    // first plane (from the top) of this CTA's super-row that has data; -1 if none
-    auto next_plane = [&](int k, BandMask& bm) {
-        for (; k >= 0; --k) {
-            bm = load_bands(band_mask, k, NT);
-            if (any_band(bm)) return k;
-        }
-        return -1;
-    };
+        return;
+    }
 
-    BandMask cur, nxt;                 // invariant: the non-zero bands of `landing` are a subset of `cur`
-    int k_cur = next_plane(nw - 1, cur);
-    uint32_t sr_cur = blockIdx.x;
-    if (k_cur >= 0) issue(blockIdx.x, k_cur, cur);
+    // ---- the 16 compute warps (they take over the registers the producer's warpgroup gave back)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    auto cta_sync = [&]() { asm volatile("bar.sync 3, %0;" ::"r"(FT) : "memory"); };     // (the producer is not part of it)
+    auto group_sync = [&]() {
+        if (C::GROUPED) asm volatile("bar.sync %0, %1;" ::"r"(1 + g), "r"(GT) : "memory");
+        else cta_sync();
+    };
     uint32_t parity = 0;
     const int top_span_lo = ((nw - 1) / WC_SPAN) * WC_SPAN;
 
@@ -459,10 +615,9 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         float2 rot[EPT], h[EPT];
 #pragma unroll
         for (int s = 0; s < EPT; ++s) {
-            const int P = final_pos<LOGN>(s, t);
-            const int pos = (int)sr * ROWS + (P >> LOGN);
+            const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
             const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-            const int p = (freq_of<LOGN>(P & (N - 1)) + N / 2) & (N - 1);
+            const int p = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
             bool inside;
             const double tt = ws_n_minus_1(prm, q, p, &inside);
             rot[s] = ws_expi_turns(prm.dw * tt);
@@ -470,39 +625,29 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         }
         for (int k = nw - 1; k >= 0; --k) {
             float2 x[EPT];
-            if (k == k_cur && sr == sr_cur) { // CTA-uniform: this plane has data and its copy is in flight
-                while (!mbar_try_wait(bar, parity)) {}
+            if ((s_any[k >> 5] >> (k & 31)) & 1u) {      // CTA-uniform: the plane has data, its copy is under way
+                while (!mbar_try_wait(full, parity)) {}
                 parity ^= 1u;
-                stage_load<float2, L0, LR0, false>(x, landing, t);
-                __syncthreads();       // landing consumed (and the previous plane's last stage has read `work`)
-                // next copy: the next non-empty plane of this super-row, else the first one of the next super-row
-                int k_nxt = next_plane(k - 1, nxt);
-                uint32_t sr_nxt = sr;
-                if (k_nxt < 0 && sr + gridDim.x < n_super) {
-                    sr_nxt = sr + gridDim.x;
-                    k_nxt = next_plane(nw - 1, nxt);
-                }
-                if (k_nxt >= 0) {
-                    uint32_t stale = 0;                    // bands the last copy filled and the next one will not
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) stale |= cur.w[i] & ~nxt.w[i];
-                    if (stale) {
-#pragma unroll
-                        for (int i = 0; i < EPT; ++i) {
-                            const int wi = ((8 * i) & (NT - 1)) >> 5;      // band of point t + 256 i: (t >> 5) + 8 i
-                            const int bit = ((t >> 5) + 8 * i) & 31;
-                            if (((cur.w[wi] & ~nxt.w[wi]) >> bit) & 1u) landing[t + FT * i] = make_float2(0.f, 0.f);
-                        }
-                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                // ---- first stage: inputs from the landing buffer
+                if constexpr (C::GROUPED) Grouped<LOGN>::load_first(x, landing, u & 255, g);
+                else row_stage<LOGN, 0, true, false>(x, landing, work, tw, u);
+                group_sync();          // this group is done with `landing` (and with last plane's reads of `work`)
+                if ((u & 255) == 0 && (C::GROUPED || g == 0))
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty)) : "memory");
+                // ---- arithmetic, twiddles, exchanges
+                if constexpr (C::GROUPED) {
+                    Grouped<LOGN>::finish_first(x, work, tw, u & 255, g);
+                    group_sync();
+                    Grouped<LOGN>::second_third(x, work, tw, u & 255, g);
+                } else {
+                    first_stage_finish<LOGN>(x, work, tw, u);
+                    group_sync();
+                    if constexpr (C::S == 3) {
+                        row_stage<LOGN, 1, false, false>(x, work, work, tw, u);
+                        group_sync();
                     }
-                    issue(sr_nxt, k_nxt, nxt);
+                    row_stage<LOGN, C::S - 1, false, true>(x, work, work, tw, u);
                 }
-                cur = nxt;
-                k_cur = k_nxt;
-                sr_cur = sr_nxt;
-                stage_compute<float2, L0, LR0>(x, tw, t);
-                stage_store<float2, L0, LR0>(x, work, t);
-                later_stages<float2, LOGN>(x, work, tw, t);
 #pragma unroll
                 for (int s = 0; s < EPT; ++s) h[s] = ws_horner(h[s], rot[s], x[s].x, x[s].y);
             } else {                          // empty plane: P_k = 0
@@ -513,27 +658,24 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
             // close the chain: x <- E h, E = exp(2 pi i (w0 + k dw) t) evaluated exactly
 #pragma unroll
             for (int s = 0; s < EPT; ++s) {
-                const int P = final_pos<LOGN>(s, t);
-                const int pos = (int)sr * ROWS + (P >> LOGN);
+                const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
                 const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-                const int p = (freq_of<LOGN>(P & (N - 1)) + N / 2) & (N - 1);
+                const int p = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
                 bool inside;
                 const double tt = ws_n_minus_1(prm, q, p, &inside);
                 x[s] = ws_cmul(h[s], ws_expi_turns((prm.w0 + (double)k * prm.dw) * tt));
                 if (!inside) x[s] = make_float2(0.f, 0.f);
                 h[s] = make_float2(0.f, 0.f);
             }
-            // un-permute through `work`: natural order along the rows of the centred image
-            __syncthreads();
+            // un-permute through `work`: natural order along the rows of the centred image (both groups)
+            cta_sync();
 #pragma unroll
-            for (int s = 0; s < EPT; ++s) {
-                const int P = final_pos<LOGN>(s, t);
-                work[pad((P & ~(N - 1)) + ((freq_of<LOGN>(P & (N - 1)) + N / 2) & (N - 1)))] = x[s];
-            }
-            __syncthreads();
+            for (int s = 0; s < EPT; ++s)
+                work[pad(slot_row<LOGN>(s, u) * N + ((slot_freq<LOGN>(s, u) + N / 2) & (N - 1)))] = x[s];
+            cta_sync();
 #pragma unroll
             for (int i = 0; i < EPT / 2; ++i) {
-                const int e = (t + FT * i) * 2;
+                const int e = (u + FT * i) * 2;
                 const float2 a = work[pad(e)], b = work[pad(e) + 1];
                 float4 v = make_float4(a.x, a.y, b.x, b.y);
                 const int pos = (int)sr * ROWS + (e >> LOGN);
@@ -546,16 +688,17 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                 *(float4*)(image + o) = v;
                 if (dirty && k == 0) *(float2*)(dirty + o) = make_float2(v.x, v.z);
             }
-            __syncthreads();       // `work` is free again before the next plane's first stage stores into it
+            cta_sync();            // `work` is free again before the next plane's first stage stores into it
         }
     }
 }
+
 
 // ---- host side ---------------------------------------------------------------------------------------------
 template <int LOGN>
 size_t rows_smem() {
     return (size_t)PTS * sizeof(float2) + (size_t)PAD_PTS * sizeof(float2) +
-           (size_t)((tw_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16;
+           (size_t)((tw_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16 + MAX_PLANES / 8;
 }
 
 float2 unit(long long e, long long L) {      // exp(+2 pi i e / L), fp64 -> fp32
@@ -605,12 +748,12 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
     if (R0 > 1) {
         const uint32_t n_items = nw * NT * 32u;
         const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 8u ? n_items : (uint32_t)plan->sm_count * 8u;
-        k_fft_colA<LOGN><<<ctas, FT, 0, st>>>(grid, tw + plan->tw_off_a, cm, n_items);
+        k_fft_colA<LOGN><<<ctas, CT, 0, st>>>(grid, tw + plan->tw_off_a, cm, n_items);
         ++launches;
     }
     const uint32_t n_items = nw * NT * (uint32_t)R0;
     const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 2u ? n_items : (uint32_t)plan->sm_count * 2u;
-    k_fft_colB<LOGN><<<ctas, FT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_b, cm, n_items);
+    k_fft_colB<LOGN><<<ctas, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_b, cm, n_items);
     ++launches;
     return cudaGetLastError() == cudaSuccess ? launches : WS_ERR_CUDA;
 }
@@ -629,7 +772,7 @@ int launch_rows_n(ws_plan* plan, const float2* grid, float2* image, float* dirty
     const uint32_t n_super = (uint32_t)(((size_t)N * N) / PTS);
     const uint32_t ctas = n_super < (uint32_t)plan->sm_count ? n_super : (uint32_t)plan->sm_count;
     const uint32_t* bm = sparse ? (const uint32_t*)plan->d_masks + (size_t)P.n_wplanes * (N / 32) * 8 : nullptr;
-    k_fft_rows<LOGN><<<ctas, FT, rows_smem<LOGN>(), st>>>(prm, grid, image, dirty, accumulate,
+    k_fft_rows<LOGN><<<ctas, FT + PT, rows_smem<LOGN>(), st>>>(prm, grid, image, dirty, accumulate,
                                                           (const float2*)plan->d_twiddles, bm, n_super);
     return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
 }
@@ -653,7 +796,7 @@ int logn_of(int n_pix) {
     }                                                \
     return WS_ERR_UNSUPPORTED;
 
-bool ws_fft_own_supported(int n_pix) { return logn_of(n_pix) != 0; }
+bool ws_fft_own_supported(int n_pix, int n_wplanes) { return logn_of(n_pix) != 0 && n_wplanes <= MAX_PLANES; }
 
 int ws_fft_own_init(ws_plan* plan) { WS_FFT_DISPATCH(init_n, plan) }
 

@@ -91,7 +91,7 @@ int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int a
                        cudaStream_t st);
 int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, cudaStream_t st);
 int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);
-bool ws_fft_own_supported(int n_pix);
+bool ws_fft_own_supported(int n_pix, int n_wplanes);
 int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error
 int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st);
 int ws_launch_fft_rows(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
