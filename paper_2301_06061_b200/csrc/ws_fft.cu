@@ -92,8 +92,28 @@ __device__ __forceinline__ int freq_of(int n) {
 
 
 // ---- complex helpers -------------------------------------------------------------------------------------------
-__device__ __forceinline__ float2 eadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 esub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 sadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 ssub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// complex add / subtract as ONE packed instruction (add.f32x2 -> FADD2 on sm_100a): same lane throughput as two
+// FADDs, half the issue slots -- the butterflies are mostly additions and the row kernel is issue-bound
+__device__ __forceinline__ float2 eadd(float2 a, float2 b) {
+    unsigned long long ra, rb, rc;
+    float2 c;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rc) : "l"(ra), "l"(rb));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(c.x), "=f"(c.y) : "l"(rc));
+    return c;
+}
+__device__ __forceinline__ float2 esub(float2 a, float2 b) {
+    unsigned long long ra, rb, rc;
+    float2 c;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(rc) : "l"(ra), "l"(rb));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(c.x), "=f"(c.y) : "l"(rc));
+    return c;
+}
 // a * (c + i s)
 __device__ __forceinline__ float2 emul(float2 a, float c, float s) {
     return make_float2(fmaf(a.x, c, -(a.y * s)), fmaf(a.x, s, a.y * c));
@@ -129,7 +149,7 @@ __device__ __forceinline__ E mul_w32(E a, int k) {
 
 // In-register inverse DFT of R = 2^LOGR points, decimation in frequency: on return x[i] = Y[brev(i)],
 // Y[m'] = sum_m x[m] exp(+2 pi i m m' / R).
-template <typename E, int LOGR>
+template <typename E, int LOGR, bool PACKED = true>
 __device__ __forceinline__ void bfly(E* x) {
     constexpr int R = 1 << LOGR;
 #pragma unroll
@@ -139,8 +159,8 @@ __device__ __forceinline__ void bfly(E* x) {
 #pragma unroll
             for (int j = 0; j < half; ++j) {
                 const E a = x[blk + j], b = x[blk + j + half];
-                x[blk + j] = eadd(a, b);
-                x[blk + j + half] = mul_w32(esub(a, b), j * (16 / half));
+                x[blk + j] = PACKED ? eadd(a, b) : sadd(a, b);
+                x[blk + j + half] = mul_w32(PACKED ? esub(a, b) : ssub(a, b), j * (16 / half));
             }
         }
     }
@@ -176,7 +196,7 @@ k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_c
 // Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
 // row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
 template <int LOGN>
-__global__ void __launch_bounds__(CT)
+__global__ void __launch_bounds__(CT, 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ class_mask,
            uint32_t n_items) {
     constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32;
@@ -192,7 +212,7 @@ k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 #pragma unroll
         for (int m = 0; m < R0; ++m)
             x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-        bfly<float2, LR0>(x);
+        bfly<float2, LR0, false>(x);
 #pragma unroll
         for (int r = 1; r < R0; ++r) {
             const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
@@ -237,7 +257,7 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int j = w + 8 * i;
-            bfly<float2, 4>(x + i * 16);
+            bfly<float2, 4, false>(x + i * 16);
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
                 float2 v = x[i * 16 + r];
@@ -254,7 +274,7 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
             const int b = w + 8 * i;
 #pragma unroll
             for (int m = 0; m < 16; ++m) x[i * 16 + m] = blk[(16 * b + m) * 32 + lane];
-            bfly<float2, 4>(x + i * 16);
+            bfly<float2, 4, false>(x + i * 16);
 #pragma unroll
             for (int r = 0; r < 16; ++r) p[(size_t)(b + 16 * brev(r, 4)) * N] = x[i * 16 + r];
         }
