@@ -231,6 +231,7 @@ def main():
     # ---- the library path on the same inputs, for the separate FFT figure (north_star): OVERWRITE gridding,
     # cuFFT per plane, stand-alone w-correction.  Outside the timed region.
     lib_ms = None
+    occ = plan.occupancy() if own else None      # of the timed path's mesh (fractions the FFT passes touch; orientation)
     if own:
         e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         rows = []
@@ -253,7 +254,6 @@ def main():
     mesh_b = 8.0 * d.n_pix ** 2 * d.n_wplanes
     N, NW = d.n_pix, d.n_wplanes
     if own:
-        occ = plan.occupancy()       # fractions of the mesh the passes touch (from the plan's masks)
         # k_grid: records read + non-empty tiles written; pass 1: non-empty tiles read, classes written, then the
         # non-empty bands read and written; pass 2: non-empty bands read once, image + dirty written
         alg = {"k_grid_tiles": 16.0 * n_records + mesh_b * occ["tiles"],

@@ -49,8 +49,10 @@ extern "C" {
 #define WS_GRID_ACCUMULATE 0 /* add onto the existing mesh (call ws_grid_zero first); tiles without visibilities untouched */
 #define WS_GRID_OVERWRITE 1  /* the mesh is taken as zero on entry and EVERY cell is written: no ws_grid_zero needed */
 #define WS_GRID_SPARSE 2     /* as OVERWRITE, but only the 32 x 32 tiles that receive visibilities are written; every
-                                other cell keeps whatever it held.  Only ws_fft_* with WS_FFT_USE_OCCUPANCY can
-                                consume such a mesh (own FFT: N = 2^8..2^13 and no WS_FLAG_LIBRARY_FFT) */
+                                other cell keeps whatever it held, and the layout is PRIVATE: the library stores the
+                                planes transposed ([k][u][v]) when that leaves fewer 32-line bands to transform.  Only
+                                ws_fft_* with WS_FFT_USE_OCCUPANCY can consume such a mesh (own FFT: N = 2^8..2^13
+                                and no WS_FLAG_LIBRARY_FFT), and nothing can be accumulated onto it */
 
 /* fft_flags of ws_fft_wcorrect / ws_fft_columns / ws_fft_rows_wcorrect */
 #define WS_FFT_USE_OCCUPANCY 1u /* skip the tiles / column bands the gridding calls on this plan left empty.  The plan
@@ -61,6 +63,7 @@ extern "C" {
 
 /* ws_params.flags */
 #define WS_FLAG_LIBRARY_FFT 1u /* a3 through cuFFT even where the library's own two-pass FFT exists (N = 2^8..2^13) */
+#define WS_FLAG_NO_TRANSPOSE 2u /* WS_GRID_SPARSE keeps the [k][v][u] orientation (default: it may store the mesh transposed) */
 
 /* kernel_type */
 #define WS_KERNEL_GAUSSIAN 0 /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)) */
@@ -181,8 +184,10 @@ int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_ke
                 int64_t* n_records, void* stream);
 
 /* Fractions of the mesh the recorded occupancy marks non-empty (synchronises `stream`): 32 x 32 tiles; row classes
- * pass 1a of the FFT writes; 32-column bands per plane (what pass 1b writes and pass 2 reads); planes with any. */
-int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, void* stream);
+ * pass 1a of the FFT writes; 32-column bands per plane (what pass 1b writes and pass 2 reads); planes with any;
+ * *transposed = 1 if the WS_GRID_SPARSE mesh is stored [k][u][v] (then "column" means a line along u). */
+int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, int32_t* transposed,
+                     void* stream);
 
 /* Synchronises `stream` and returns the deferred status of the work enqueued so far (record capacity
  * exceeded -> WS_ERR_WORKSPACE, CUDA fault -> WS_ERR_CUDA). */

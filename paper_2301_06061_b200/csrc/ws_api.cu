@@ -124,7 +124,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
     if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
-    if ((p->flags & ~(uint32_t)WS_FLAG_LIBRARY_FFT) != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
+    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE)) != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
     if (p->support > 2 * WS_HALO_MAX + 1) return WS_ERR_UNSUPPORTED;
     if (p->kernel_type != WS_KERNEL_GAUSSIAN) return WS_ERR_UNSUPPORTED;
     if (p->tile != 0 && p->tile != WS_TILE) return WS_ERR_UNSUPPORTED;
@@ -173,6 +173,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->d_masks = nullptr;
     plan->mask_words = 0;
     plan->occ_grid = nullptr;
+    plan->occ_sparse = false;
     int rc = make_fft_plan(plan);                       // ws_fft_planes is always the library's
     if (rc == WS_OK && plan->fft_own) rc = ws_fft_own_init(plan);
     if (rc != WS_OK) {
@@ -224,6 +225,7 @@ int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     if (rc >= 0) rc = ws_launch_fft_masks_clear(plan, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_grid_zero: memset failed");
     plan->occ_grid = grid;                               // an empty mesh: the occupancy masks describe it
+    plan->occ_sparse = false;
     return WS_OK;
 }
 
@@ -286,23 +288,29 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: grid must be 16-byte aligned");
     if (!plan->last_valid || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: workspace does not hold the bins of ws_bin_visibilities");
-    int rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
-    if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
-    plan->launches += rc;
-    // tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE
+    if (mode == WS_GRID_ACCUMULATE && plan->occ_sparse && plan->occ_grid == grid)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written)");
+    // Tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE.  It
+    // comes BEFORE the gridding kernel: a SPARSE mesh is stored in the orientation the masks favour.
+    int rc;
     if (plan->d_masks) {
         if (mode != WS_GRID_ACCUMULATE) {
             if (ws_launch_fft_masks_clear(plan, (cudaStream_t)stream) < 0) return fail(plan, WS_ERR_CUDA, "ws_grid_binned: mask clear failed");
             plan->occ_grid = grid;
+            plan->occ_sparse = mode == WS_GRID_SPARSE;
         }
         if (plan->occ_grid == grid) {
-            rc = ws_launch_fft_masks(plan, (const uint32_t*)((char*)workspace + plan->last_layout.off_rec_start), (cudaStream_t)stream);
+            rc = ws_launch_fft_masks(plan, (const uint32_t*)((char*)workspace + plan->last_layout.off_rec_start),
+                                     mode == WS_GRID_SPARSE ? 1 : (mode == WS_GRID_OVERWRITE ? 0 : -1), (cudaStream_t)stream);
             if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
             plan->launches += rc;
         } else {
             plan->occ_grid = nullptr;                    // accumulation onto a mesh this plan has no record of
         }
     }
+    rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
+    plan->launches += rc;
     return WS_OK;
 }
 
@@ -489,14 +497,17 @@ int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_ke
     return WS_OK;
 }
 
-int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, void* stream) {
+int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, int32_t* transposed,
+                     void* stream) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!plan->d_masks || !plan->occ_grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_occupancy: no occupancy recorded");
     cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_occupancy: synchronize");
-    std::vector<uint32_t> m(plan->mask_words);
-    e = cudaMemcpy(m.data(), plan->d_masks, m.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+    std::vector<uint32_t> all(plan->mask_words);
+    e = cudaMemcpy(all.data(), plan->d_masks, all.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_occupancy: copy");
+    const bool tr = all[2] != 0;
+    const uint32_t* m = all.data() + 8 + (tr ? plan->mask_set_words : 0);      // the set of the orientation in use
     const size_t nw = (size_t)plan->prm.n_wplanes, nt = (size_t)plan->geom.nt, n_class = nw * nt * 8;
     size_t t = 0, c = 0, b = 0, p = 0;
     for (size_t i = 0; i < n_class; ++i) {
@@ -513,6 +524,7 @@ int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* band
     if (classes) *classes = (double)c / (double)n_class;
     if (bands) *bands = (double)b / (double)(nw * nt);
     if (planes) *planes = (double)p / (double)nw;
+    if (transposed) *transposed = tr ? 1 : 0;
     return WS_OK;
 }
 

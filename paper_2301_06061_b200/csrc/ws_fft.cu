@@ -170,36 +170,52 @@ __device__ __forceinline__ void bfly(E* x) {
 // Storage (FFT-native) tile coordinates.  class_mask[(k nt + tx) 8 + c]: bit m set <=> tile (ty = c + 8 m, tx) of
 // plane k holds visibilities (the R0 inputs of pass 1a's butterflies on the rows of class c = (row mod 256) / 32).
 // band_mask[k 8 + tx / 32]: bit tx % 32 set <=> some tile of column band tx of plane k does.
+// Two sets are kept: set 0 for the mesh as the header describes it ([k][v][u]), set 1 for a mesh stored transposed
+// ([k][u][v]: the roles of tx and ty swap).  A WS_GRID_SPARSE mesh is private to this library, so the gridder stores
+// it in whichever orientation leaves fewer bands to transform (ctrl[2]): the uv tracks of an east-west-ish array are
+// squeezed in v by sin(dec), and a band costs 2 N x 256 B of traffic in pass 1b and pass 2.
+// Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; set = class masks, band masks.
 // Masks are OR-ed into (chunked gridding accumulates); ws_fft_masks_clear zeroes them.
+constexpr int MASK_CTRL = 8;
+__device__ __forceinline__ const uint32_t* mask_set(const uint32_t* __restrict__ masks, uint32_t set_words) {
+    return masks + MASK_CTRL + (masks[2] ? set_words : 0u);
+}
 __global__ void __launch_bounds__(256)
-k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_classes, uint32_t* __restrict__ class_mask,
-            uint32_t* __restrict__ band_mask) {
-    const uint32_t id = blockIdx.x * 256u + threadIdx.x;      // (k nt + txs) 8 + c
+k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_classes, uint32_t set_words,
+            uint32_t* __restrict__ masks) {
+    const uint32_t id = blockIdx.x * 256u + threadIdx.x;      // (k nt + band) 8 + c
     if (id >= n_classes) return;
+    const int set = blockIdx.y;
+    uint32_t* class_mask = masks + MASK_CTRL + set * set_words;
+    uint32_t* band_mask = class_mask + n_classes;
     const int c = id & 7;
-    const uint32_t ktx = id >> 3;
-    const int txs = ktx % nt, k = ktx / nt;
-    const int tx = (txs + nt / 2) & (nt - 1);
+    const uint32_t kb = id >> 3;
+    const int bs = kb % nt, k = kb / nt;
+    const int bl = (bs + nt / 2) & (nt - 1);                  // logical tile coordinate of the band
     uint32_t mask = 0;
     for (int m = 0; m < r0; ++m) {
-        const int ty = (c + 8 * m + nt / 2) & (nt - 1);
-        const uint32_t bin = ((uint32_t)k * nt + ty) * nt + tx;
+        const int ol = (c + 8 * m + nt / 2) & (nt - 1);       // the other coordinate: ty (set 0) or tx (set 1)
+        const uint32_t bin = set == 0 ? ((uint32_t)k * nt + ol) * nt + bl : ((uint32_t)k * nt + bl) * nt + ol;
         if (rec_start[bin + 1] > rec_start[bin]) mask |= 1u << m;
     }
     if (mask) {
         atomicOr(class_mask + id, mask);
-        atomicOr(band_mask + k * 8 + (txs >> 5), 1u << (txs & 31));
+        const uint32_t bit = 1u << (bs & 31);
+        if (!(atomicOr(band_mask + k * 8 + (bs >> 5), bit) & bit)) atomicAdd(masks + set, 1u);
     }
 }
+// the orientation of a WS_GRID_SPARSE mesh: transposed iff that leaves fewer bands (allow = 0: as the header says)
+__global__ void k_fft_orient(uint32_t* __restrict__ masks, int allow) { masks[2] = allow && masks[1] < masks[0] ? 1u : 0u; }
 
 // ---- pass 1a: first radix-R0 step of the column transforms ------------------------------------------------------
 // Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
 // row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
 template <int LOGN>
 __global__ void __launch_bounds__(CT, 2)
-k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ class_mask,
-           uint32_t n_items) {
+k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
+           uint32_t set_words, uint32_t n_items) {
     constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32;
+    const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
         const uint32_t jb = item & 31, ktx = item >> 5;            // 32 groups of 8 rows per (plane, band)
@@ -228,9 +244,10 @@ k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 // j + 16 m; stage 2: blocks b in {w, w + 8}, rows 16 b + m; frequency f = b + 16 m' is stored at row 256 m0 + f.
 template <int LOGN>
 __global__ void __launch_bounds__(CT, 2)
-k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ class_mask,
-           uint32_t n_items) {
+k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
+           uint32_t set_words, uint32_t n_items) {
     constexpr int N = 1 << LOGN, R0 = 1 << (LOGN - 8), NT = N / 32;
+    const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -527,13 +544,27 @@ struct Grouped {
     }
 };
 
+// Work item -> super-row.  For N = 8192 (one row position per super-row) items are taken in the order of the
+// FREQUENCY the row position holds, pos = (F mod R0) 256 + F / R0, so that the CTAs running side by side own adjacent
+// lines of the image: when the mesh is transposed their 8-byte pixels share 32-byte sectors and meet in L2.
+template <int LOGN>
+__device__ __forceinline__ uint32_t super_row_of(uint32_t item) {
+    constexpr int LR0 = LOGN - 8;
+    if constexpr (RowCfg<LOGN>::ROWS == 1) return ((item & ((1u << LR0) - 1u)) << 8) | (item >> LR0);
+    else return item;
+}
+
 template <int LOGN>
 __global__ void __launch_bounds__(FT + PT, 1)
 k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ planes, float2* __restrict__ image,
            float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g,
-           const uint32_t* __restrict__ band_mask, uint32_t n_super) {
+           const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_super) {
     using C = RowCfg<LOGN>;
     constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0;
+    // occupancy: the band masks of the orientation the mesh is stored in; transposed: the mesh is [k][u][v], i.e. a
+    // row position is a u-frequency and the image comes out transposed (the phase screen is symmetric in l and m)
+    const uint32_t* band_mask = masks ? mask_set(masks, set_words) + (set_words - 8u * (uint32_t)prm.n_wplanes) : nullptr;
+    const bool transposed = masks && masks[2];
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* landing = (float2*)smem_raw;
     float2* work = landing + PTS;
@@ -570,7 +601,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         const int lane = u & 31;
         uint32_t was = 0, e_parity = 0;
         bool first = true;
-        for (uint32_t sr = blockIdx.x; sr < n_super; sr += gridDim.x) {
+        for (uint32_t it = blockIdx.x; it < n_super; it += gridDim.x) {
+            const uint32_t sr = super_row_of<LOGN>(it);
             for (int k = nw - 1; k >= 0; --k) {
                 if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
                 uint32_t now = 0;
@@ -631,7 +663,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     uint32_t parity = 0;
     const int top_span_lo = ((nw - 1) / WC_SPAN) * WC_SPAN;
 
-    for (uint32_t sr = blockIdx.x; sr < n_super; sr += gridDim.x) {
+    for (uint32_t it = blockIdx.x; it < n_super; it += gridDim.x) {
+        const uint32_t sr = super_row_of<LOGN>(it);
         float2 rot[EPT], h[EPT];
 #pragma unroll
         for (int s = 0; s < EPT; ++s) {
@@ -686,6 +719,23 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                 x[s] = ws_cmul(h[s], ws_expi_turns((prm.w0 + (double)k * prm.dw) * tt));
                 if (!inside) x[s] = make_float2(0.f, 0.f);
                 h[s] = make_float2(0.f, 0.f);
+            }
+            if (transposed) {      // pixel (row position, frequency) belongs at image[frequency][row position]
+#pragma unroll
+                for (int s = 0; s < EPT; ++s) {
+                    const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
+                    const int a = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
+                    const int b = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
+                    const size_t o = (size_t)b * N + a;
+                    float2 v = x[s];
+                    if (accumulate || k != top_span_lo) {
+                        const float2 old = image[o];
+                        v.x += old.x; v.y += old.y;
+                    }
+                    image[o] = v;
+                    if (dirty && k == 0) dirty[o] = v.x;
+                }
+                continue;
             }
             // un-permute through `work`: natural order along the rows of the centred image (both groups)
             cta_sync();
@@ -744,7 +794,8 @@ int init_n(ws_plan* plan) {
     for (int m = 1; m < 16; ++m)
         for (int j = 0; j < 16; ++j) tw.push_back(unit((long long)j * m, 256));
     const size_t n_class = (size_t)plan->prm.n_wplanes * (N / 32) * 8, n_band = (size_t)plan->prm.n_wplanes * 8;
-    plan->mask_words = n_class + n_band;
+    plan->mask_set_words = n_class + n_band;
+    plan->mask_words = MASK_CTRL + 2 * plan->mask_set_words;
     if (cudaMalloc((void**)&plan->d_twiddles, tw.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&plan->d_masks, plan->mask_words * sizeof(uint32_t)) != cudaSuccess)
         return WS_ERR_CUDA;
@@ -763,17 +814,18 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
     constexpr int N = 1 << LOGN, R0 = N / 256, NT = N / 32;
     const float2* tw = (const float2*)plan->d_twiddles;
     const uint32_t* cm = sparse ? (const uint32_t*)plan->d_masks : nullptr;
+    const uint32_t sw = (uint32_t)plan->mask_set_words;
     const uint32_t nw = (uint32_t)plan->prm.n_wplanes;
     int launches = 0;
     if (R0 > 1) {
         const uint32_t n_items = nw * NT * 32u;
         const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 8u ? n_items : (uint32_t)plan->sm_count * 8u;
-        k_fft_colA<LOGN><<<ctas, CT, 0, st>>>(grid, tw + plan->tw_off_a, cm, n_items);
+        k_fft_colA<LOGN><<<ctas, CT, 0, st>>>(grid, tw + plan->tw_off_a, cm, sw, n_items);
         ++launches;
     }
     const uint32_t n_items = nw * NT * (uint32_t)R0;
     const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 2u ? n_items : (uint32_t)plan->sm_count * 2u;
-    k_fft_colB<LOGN><<<ctas, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_b, cm, n_items);
+    k_fft_colB<LOGN><<<ctas, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_b, cm, sw, n_items);
     ++launches;
     return cudaGetLastError() == cudaSuccess ? launches : WS_ERR_CUDA;
 }
@@ -791,9 +843,10 @@ int launch_rows_n(ws_plan* plan, const float2* grid, float2* image, float* dirty
     prm.w0 = P.w_min + 0.5 * prm.dw;
     const uint32_t n_super = (uint32_t)(((size_t)N * N) / PTS);
     const uint32_t ctas = n_super < (uint32_t)plan->sm_count ? n_super : (uint32_t)plan->sm_count;
-    const uint32_t* bm = sparse ? (const uint32_t*)plan->d_masks + (size_t)P.n_wplanes * (N / 32) * 8 : nullptr;
+    const uint32_t* bm = sparse ? (const uint32_t*)plan->d_masks : nullptr;
     k_fft_rows<LOGN><<<ctas, FT + PT, rows_smem<LOGN>(), st>>>(prm, grid, image, dirty, accumulate,
-                                                          (const float2*)plan->d_twiddles, bm, n_super);
+                                                          (const float2*)plan->d_twiddles, bm,
+                                                                    (uint32_t)plan->mask_set_words, n_super);
     return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
 }
 
@@ -834,12 +887,20 @@ int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st) {
     return cudaMemsetAsync(plan->d_masks, 0, plan->mask_words * sizeof(uint32_t), st) == cudaSuccess ? 0 : WS_ERR_CUDA;
 }
 
-// OR the occupancy of the bins (rec_start of ws_bin.cu, logical tile coordinates) into the plan's masks
-int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, cudaStream_t st) {
+// OR the occupancy of the bins (rec_start of ws_bin.cu, logical tile coordinates) into the plan's masks (both
+// orientations); decide: 1 = choose the orientation of the mesh (WS_GRID_SPARSE), 0 = as the header says, -1 = keep
+int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, int decide, cudaStream_t st) {
     if (!plan->d_masks) return 0;
     const int nt = plan->geom.nt, r0 = plan->prm.n_pix / 256;
     const uint32_t n_classes = (uint32_t)plan->prm.n_wplanes * (uint32_t)nt * 8u;
-    uint32_t* cm = (uint32_t*)plan->d_masks;
-    k_fft_masks<<<(n_classes + 255) / 256, 256, 0, st>>>(rec_start, nt, r0, n_classes, cm, cm + n_classes);
-    return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
+    uint32_t* m = (uint32_t*)plan->d_masks;
+    k_fft_masks<<<dim3((n_classes + 255) / 256, 2), 256, 0, st>>>(rec_start, nt, r0, n_classes, (uint32_t)plan->mask_set_words, m);
+    int launches = 1;
+    if (decide >= 0) {
+        k_fft_orient<<<1, 1, 0, st>>>(m, decide && !(plan->prm.flags & WS_FLAG_NO_TRANSPOSE));
+        ++launches;
+    }
+    return cudaGetLastError() == cudaSuccess ? launches : WS_ERR_CUDA;
 }
+
+const uint32_t* ws_fft_orientation_flag(const ws_plan* plan) { return plan->d_masks ? (const uint32_t*)plan->d_masks + 2 : nullptr; }

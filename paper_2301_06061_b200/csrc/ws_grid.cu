@@ -42,8 +42,10 @@ struct TileCfg {
     static constexpr int THREADS = WARPS * 32;
 };
 
-// storage origin (FFT-native order, wstack.h) of tile `bin`: returns the pointer to its first cell
-__device__ __forceinline__ float2* tile_origin(const WsGeom& g, float2* grid, uint32_t bin) {
+// storage origin (FFT-native order, wstack.h) of tile `bin`: returns the pointer to its first cell.  tr: the planes
+// are stored transposed ([k][u][v], the private layout a WS_GRID_SPARSE mesh may take): cell (y, x) of the tile is
+// then at origin + x N + y.
+__device__ __forceinline__ float2* tile_origin(const WsGeom& g, float2* grid, uint32_t bin, bool tr) {
     const uint32_t nt = (uint32_t)g.nt;
     const uint32_t tx = bin % nt, r = bin / nt;
     const uint32_t ty = r % nt, k = r / nt;
@@ -51,7 +53,7 @@ __device__ __forceinline__ float2* tile_origin(const WsGeom& g, float2* grid, ui
     uint32_t sx = tx * T + half, sy = ty * T + half;
     sx = sx >= N ? sx - N : sx;
     sy = sy >= N ? sy - N : sy;
-    return grid + ((size_t)k * N + sy) * N + sx;
+    return tr ? grid + ((size_t)k * N + sx) * N + sy : grid + ((size_t)k * N + sy) * N + sx;
 }
 
 // 32 rows x 256 B of zeros: 16 lanes x 16 B per row, two rows per store instruction
@@ -146,8 +148,10 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
 // Queues the chunks of the heavy bins as work items and (OVERWRITE mode) clears their tiles.
 __global__ void __launch_bounds__(256)
 k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, uint4* __restrict__ items,
-                uint32_t item_capacity, WsStatus* __restrict__ status, float2* __restrict__ grid, int mode) {
+                uint32_t item_capacity, WsStatus* __restrict__ status, float2* __restrict__ grid, int mode,
+                const uint32_t* __restrict__ orient) {
     if (status->overflow) return;
+    const bool tr = orient && *orient;
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
     const int lane = threadIdx.x & 31;
     uint32_t s = 0, cnt = 0;
@@ -180,7 +184,7 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
     if (mode != WS_GRID_ACCUMULATE) {
         for (unsigned m = hm; m; m &= m - 1) {
             const uint32_t hb = (b - lane) + (__ffs(m) - 1);
-            store_zero_tile(tile_origin(g, grid, hb), (size_t)g.n_pix, lane);
+            store_zero_tile(tile_origin(g, grid, hb, tr), (size_t)g.n_pix, lane);
         }
     }
 }
@@ -189,12 +193,14 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
 template <int S>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 2)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint4* __restrict__ items,
-       const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status) {
+       const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
+       const uint32_t* __restrict__ orient) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const WarpSmem<S> sm(smem_raw + (size_t)wid * C::WARP_BYTES);
     if (status->overflow) return;
+    const bool tr = orient && *orient;          // transposed planes: lane = row of the tile, one tile column per store
     const uint32_t n_items = status->n_items;
     const uint32_t n_warps = gridDim.x * C::WARPS;
     const uint32_t gw = blockIdx.x * C::WARPS + wid;
@@ -207,12 +213,12 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
     auto do_item = [&]() {
         const uint4 w = items[it];
         it += n_warps;
-        float2* out = tile_origin(g, grid, w.x);
+        float2* out = tile_origin(g, grid, w.x, tr);
         zero_tile<S>(sm.tile, lane);
         accumulate<S>(g, records, w.y, w.z, sm, lane);
 #pragma unroll 4
         for (int y = 0; y < T; ++y) {
-            const float2 v = sm.tile[y * C::P + lane];
+            const float2 v = tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane];
             if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
         }
         __syncwarp();
@@ -226,7 +232,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         ++since;
         const uint32_t s = rec_start[bin], e = rec_start[bin + 1];
         if (e - s > WS_CHUNK) continue;                     // heavy: its chunks are items
-        float2* out = tile_origin(g, grid, bin);
+        float2* out = tile_origin(g, grid, bin, tr);
         if (s == e) {
             if (mode == WS_GRID_OVERWRITE) store_zero_tile(out, N, lane);
             continue;
@@ -235,7 +241,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         accumulate<S>(g, records, s, e, sm, lane);
         if (mode != WS_GRID_ACCUMULATE) {
 #pragma unroll 4
-            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, sm.tile[y * C::P + lane]);
+            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane]);
         } else {
 #pragma unroll 4
             for (int y = 0; y < T; ++y) {
@@ -254,6 +260,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
 
 template <int S>
 int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
+    const uint32_t* orient = mode == WS_GRID_SPARSE ? ws_fft_orientation_flag(plan) : nullptr;
     using C = TileCfg<S>;
     const size_t smem = C::WARP_BYTES * C::WARPS;
     static bool attr_set = false;
@@ -268,8 +275,8 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode);
-    k_grid<S><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status);
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient);
+    k_grid<S><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }

@@ -76,8 +76,9 @@ struct ws_plan {
     void* d_twiddles;                           // plan-owned inter-stage twiddle tables (fp64-computed, < 140 KB)
     size_t tw_off_a, tw_off_b;                  // entry offsets of the pass 1a / 1b tables
     void* d_masks;                              // plan-owned tile-occupancy masks of the mesh (class masks, band masks)
-    size_t mask_words;
+    size_t mask_words, mask_set_words;          // whole buffer; one set (class masks + band masks) of the two orientations
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
+    bool occ_sparse;                            // ... and it was written by WS_GRID_SPARSE (private layout, empty tiles unwritten)
 };
 
 static inline size_t ws_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -97,4 +98,5 @@ int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st
 int ws_launch_fft_rows(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
                        cudaStream_t st);
 int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st);
-int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, cudaStream_t st);
+int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, int decide, cudaStream_t st);
+const uint32_t* ws_fft_orientation_flag(const ws_plan* plan);   // device word: 1 = the sparse mesh is stored transposed

@@ -13,6 +13,7 @@ from . import build as _build
 WS_GRID_ACCUMULATE = 0
 WS_GRID_OVERWRITE = 1
 WS_FLAG_LIBRARY_FFT = 1
+WS_FLAG_NO_TRANSPOSE = 2
 WS_GRID_SPARSE = 2
 WS_FFT_USE_OCCUPANCY = 1
 
@@ -73,7 +74,7 @@ def lib():
         "ws_fft_columns": (C.c_int, [vp, vp, u32, vp]),
         "ws_fft_rows_wcorrect": (C.c_int, [vp, vp, vp, i32, vp, u32, vp]),
         "ws_plan_fft_is_own": (C.c_int, [vp]),
-        "ws_get_occupancy": (C.c_int, [vp] + [C.POINTER(C.c_double)] * 4 + [vp]),
+        "ws_get_occupancy": (C.c_int, [vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(i32), vp]),
         "ws_dirty_image": (C.c_int, [vp, vp, vp, u32, vp]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
@@ -255,8 +256,11 @@ class Plan:
     def occupancy(self, stream=None) -> dict:
         """Fractions of the mesh marked non-empty by the gridding calls: tiles, classes, bands, planes."""
         v = [C.c_double() for _ in range(4)]
-        self._check(lib().ws_get_occupancy(self._h, *[C.byref(x) for x in v], _stream(stream)))
-        return dict(zip(("tiles", "classes", "bands", "planes"), (x.value for x in v)))
+        tr = C.c_int32()
+        self._check(lib().ws_get_occupancy(self._h, *[C.byref(x) for x in v], C.byref(tr), _stream(stream)))
+        out = dict(zip(("tiles", "classes", "bands", "planes"), (x.value for x in v)))
+        out["transposed"] = bool(tr.value)
+        return out
 
     def async_status(self, stream=None):
         self._check(lib().ws_async_status(self._h, _stream(stream)))

@@ -167,6 +167,27 @@ def test_library_fft_flag_and_occupancy_rules(oracle):
     assert 0 < occ["tiles"] <= occ["classes"] <= occ["bands"] <= occ["planes"] <= 1
 
 
+@pytest.mark.parametrize("squeeze_axis,flags,expect_transposed", [(1, 0, True), (0, 0, False), (1, 2, False)])
+def test_sparse_mesh_orientation_follows_the_uv_coverage(oracle, squeeze_axis, flags, expect_transposed):
+    # uv coverage squeezed along v (axis 1) leaves fewer row bands than column bands: the sparse mesh is then stored
+    # transposed (unless WS_FLAG_NO_TRANSPOSE = 2); squeezed along u it is not.  The image is the same either way.
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(40, 20000, 1, 512, 5, 7, fill=0.9, w_span=50.0, cell_rad=1e-3)
+    d.uvw[:, squeeze_axis] *= 0.2
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, flags=flags)
+    out = U.run_chain(d, plan=plan)
+    occ = plan.occupancy()
+    assert occ["transposed"] == expect_transposed, occ
+    prm = U.oracle_params(oracle, d, plan.tile)
+    U.assert_close(out["image"], oracle.dirty_image(prm, *_np(d)), "image from a sparse mesh")
+    assert np.array_equal(out["dirty"], out["image"].real)
+    dev = d.to("cuda")
+    grid, wsp = plan.alloc_grid(), plan.alloc_workspace(d.n_vis)
+    plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_SPARSE)
+    with pytest.raises(ws.WStackError):        # nothing can be accumulated onto a sparse mesh
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_ACCUMULATE)
+
+
 def test_chunked_accumulate_keeps_occupancy_of_all_chunks(oracle):
     import paper_2301_06061_b200 as ws
     d = make_random_dataset(32, 8000, 2, 512, 6, 7, wavelengths=False, fill=0.95, w_span=60.0, cell_rad=1e-3)
@@ -218,7 +239,7 @@ def test_small_workspace_reports_overflow(oracle):
 def test_argument_validation():
     import paper_2301_06061_b200 as ws
     for bad in (dict(n_pix=250), dict(support=8), dict(support=17), dict(w_max=-5.0), dict(cell_rad=0.0), dict(tile=64),
-                dict(flags=8)):
+                dict(flags=16)):
         kw = dict(n_pix=256, n_wplanes=4, support=7, cell_rad=1e-3, w_min=-1.0, w_max=1.0)
         kw.update(bad)
         with pytest.raises(ws.WStackError):
