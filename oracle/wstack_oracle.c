@@ -23,6 +23,14 @@
  *                      pinned against orc_dft2_naive and numpy in tests/test_oracle_pins.py.
  *   orc_wcorrect       PAPER.md:68 Eq. 2 / :86 "phase shift and reduction of the w-planes":
  *                      D(l,m) = sum_k exp(2 pi i w_k (sqrt(1-l^2-m^2)-1)) P_k(l,m).
+ *   orc_kernel1d       the 1-D convolution function: the paper's Gaussian or the Kaiser-Bessel
+ *                      window the paper names as the production kernel and as its next step (:82, :459),
+ *                      I0 by its power series; unit integral (reading R2 / R28).
+ *   orc_taper1d        the continuous Fourier transform of that function (closed forms), i.e. the image-plane
+ *                      response the convolution leaves behind ("aliasing response in image space", :82).
+ *   orc_sum_weights    sum of the weights of the kept visibilities (the normalisation of the direct sum).
+ *   orc_dirty          PAPER.md:68 Eq. 2 solved for I: the factor n = sqrt(1-l^2-m^2) of its left side, the
+ *                      division by the taper and by the sum of weights (readings R12 / R29).
  *   orc_image_samples  the composition orc_grid -> DFT -> orc_wcorrect evaluated at single pixels
  *                      with the order of the (finite, linear) sums exchanged: visibility outermost.
  *                      Used where a full fp64 plane stack would not fit; pinned against the chain.
@@ -57,6 +65,8 @@ typedef struct {
     double cell_rad;    /* image pixel size, radians                           */
     double w_min;       /* w range covered by the planes, wavelengths (R6)     */
     double w_max;
+    int32_t kernel_type; /* 0: Gaussian, `sigma` = sigma in cells; 1: Kaiser-Bessel, `sigma` = beta (R28) */
+    int32_t pad_;
 } orc_params;
 
 /* ---- O1: per-channel scalar constants (O1) ------------------------- */
@@ -151,9 +161,48 @@ int64_t orc_bins(const uint32_t *key, int64_t n_vis, int64_t n_bins, uint32_t *b
     return dropped;
 }
 
-/* ---- O5: Gaussian taps (unit integral; readings R1, R2) ---------------------------------- */
-static inline double orc_g(double x, double sigma) {
-    return exp(-(x * x) / (2.0 * sigma * sigma)) / (sigma * sqrt(2.0 * ORC_PI));
+/* ---- O5: 1-D convolution function, unit integral (readings R1, R2, R28) ------------------- */
+/* Modified Bessel function of the first kind, order 0, by its defining power series            */
+/* I0(x) = sum_k (x^2/4)^k / (k!)^2 (all terms positive: no cancellation).                       */
+double orc_i0(double x) {
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 1000; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-18 * sum) break;
+    }
+    return sum;
+}
+
+/* Gaussian: g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)).                  */
+/* Kaiser-Bessel (Jackson et al. 1991), width S cells, shape beta:             */
+/*   g(x) = I0(beta sqrt(1 - (2x/S)^2)) * beta / (S sinh(beta))   for |x| <= S/2, else 0,         */
+/* whose integral over [-S/2, S/2] is 1 because int_{-1}^{1} I0(beta sqrt(1-t^2)) dt = 2 sinh(beta)/beta. */
+double orc_kernel1d(const orc_params *p, double x) {
+    if (p->kernel_type == 1) {
+        const double S = (double)p->support, beta = p->sigma;
+        double y = 1.0 - (2.0 * x / S) * (2.0 * x / S);
+        if (y < 0.0) return 0.0;
+        return orc_i0(beta * sqrt(y)) * beta / (S * sinh(beta));
+    }
+    return exp(-(x * x) / (2.0 * p->sigma * p->sigma)) / (p->sigma * sqrt(2.0 * ORC_PI));
+}
+
+/* Continuous Fourier transform ghat(xi) = int g(x) e^{2 pi i x xi} dx, xi in cycles per cell.    */
+/* Gaussian (untruncated): exp(-2 pi^2 sigma^2 xi^2).  Kaiser-Bessel: with a = pi S xi,            */
+/* (beta / sinh beta) sinh(sqrt(beta^2 - a^2)) / sqrt(beta^2 - a^2), continued as sin(.)/. for a > beta. */
+double orc_taper1d(const orc_params *p, double xi) {
+    if (p->kernel_type == 1) {
+        const double beta = p->sigma, a = ORC_PI * (double)p->support * xi;
+        const double d = beta * beta - a * a;
+        double f;
+        if (d > 1e-12) { double r = sqrt(d); f = sinh(r) / r; }
+        else if (d < -1e-12) { double r = sqrt(-d); f = sin(r) / r; }
+        else f = 1.0;
+        return f * beta / sinh(beta);
+    }
+    return exp(-2.0 * ORC_PI * ORC_PI * p->sigma * p->sigma * xi * xi);
 }
 
 /* ---- O6: gridding, Eq. 3 ------------------------------------------------------------------ */
@@ -178,8 +227,8 @@ void orc_grid(const orc_params *p, const float *uvw, const float *vis /* re,im *
                 int64_t m = r * n_chan + c;
                 double vr = (double)wt[m] * (double)vis[2 * m], vi = (double)wt[m] * (double)vis[2 * m + 1];
                 for (int a = -h; a <= h; ++a) {
-                    gu[a + h] = orc_g((double)a - fu, p->sigma);
-                    gv[a + h] = orc_g((double)a - fv, p->sigma);
+                    gu[a + h] = orc_kernel1d(p, (double)a - fu);
+                    gv[a + h] = orc_kernel1d(p, (double)a - fv);
                 }
                 for (int b = -h; b <= h; ++b)
                     for (int a = -h; a <= h; ++a) {
@@ -378,8 +427,8 @@ void orc_image_samples(const orc_params *p, const float *uvw, const float *vis, 
                 int64_t mi = r * n_chan + c;
                 double vr = (double)wt[mi] * (double)vis[2 * mi], vi = (double)wt[mi] * (double)vis[2 * mi + 1];
                 for (int a = -h; a <= h; ++a) {
-                    gu[a + h] = orc_g((double)a - fu, p->sigma);
-                    gv[a + h] = orc_g((double)a - fv, p->sigma);
+                    gu[a + h] = orc_kernel1d(p, (double)a - fu);
+                    gv[a + h] = orc_kernel1d(p, (double)a - fv);
                 }
                 for (int s = 0; s < n_samp; ++s) {
                     double xr = 0, xi = 0, yr = 0, yi = 0;
@@ -404,6 +453,43 @@ void orc_image_samples(const orc_params *p, const float *uvw, const float *vis, 
         D[2 * s] = sr; D[2 * s + 1] = si;
     }
     free(part); free(wph); free(E); free(su); free(sw);
+}
+
+/* ---- normalisation of the image (Eq. 2 solved for I; readings R12, R29) ------------------- */
+/* Sum of the weights of the kept visibilities (O3), in input order.                             */
+double orc_sum_weights(const orc_params *p, const float *uvw, const float *wt, const double *freq_hz,
+                       int64_t n_rows, int32_t n_chan) {
+    double *su = malloc(sizeof(double) * n_chan), *sw = malloc(sizeof(double) * n_chan), ow, sum = 0.0;
+    orc_channel_constants(p, freq_hz, n_chan, su, sw, &ow);
+    for (int64_t r = 0; r < n_rows; ++r) {
+        double u = (double)uvw[3 * r], v = (double)uvw[3 * r + 1], w = (double)uvw[3 * r + 2];
+        for (int c = 0; c < n_chan; ++c) {
+            int32_t i0, j0, k; double fu, fv;
+            if (orc_place(p, u, v, w, su[c], sw[c], ow, &i0, &j0, &k, &fu, &fv)) sum += (double)wt[r * n_chan + c];
+        }
+    }
+    free(su); free(sw);
+    return sum;
+}
+
+/* dirty[q][p] = Re D[q][p] * f, f the product of the factors `flags` selects:                    */
+/*   1 (SUMWT): 1 / sum_wt        -- the direct sum I = sum wt V e^{..} becomes a weighted mean    */
+/*   2 (N):     n = sqrt(1-l^2-m^2) -- the 1/n on the left side of Eq. 2              */
+/*   4 (TAPER): 1 / (ghat(xi_p) ghat(xi_q)), xi = (p - N/2)/N -- undoes the image-plane response    */
+/*              of the convolution function.  Pixels with l^2+m^2 >= 1 stay 0 (R14).                */
+void orc_dirty(const orc_params *p, const double *D, uint32_t flags, double sum_wt, double *dirty) {
+    const int N = p->n_pix;
+    for (int q = 0; q < N; ++q)
+        for (int pp = 0; pp < N; ++pp) {
+            double f = 1.0;
+            double l = (double)(pp - N / 2) * p->cell_rad, m = (double)(q - N / 2) * p->cell_rad;
+            double r2 = l * l + m * m;
+            if (flags & 1u) f /= sum_wt;
+            if (flags & 2u) f *= r2 < 1.0 ? sqrt(1.0 - r2) : 0.0;
+            if (flags & 4u)
+                f /= orc_taper1d(p, (double)(pp - N / 2) / (double)N) * orc_taper1d(p, (double)(q - N / 2) / (double)N);
+            dirty[(size_t)q * N + pp] = D[2 * ((size_t)q * N + pp)] * f;
+        }
 }
 
 int32_t orc_num_threads(void) {

@@ -20,7 +20,13 @@ _lib = None
 
 class _Params(C.Structure):
     _fields_ = [("n_pix", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.c_int32), ("tile", C.c_int32),
-                ("sigma", C.c_double), ("cell_rad", C.c_double), ("w_min", C.c_double), ("w_max", C.c_double)]
+                ("sigma", C.c_double), ("cell_rad", C.c_double), ("w_min", C.c_double), ("w_max", C.c_double),
+                ("kernel_type", C.c_int32), ("pad_", C.c_int32)]
+
+
+KERNEL_GAUSSIAN = 0
+KERNEL_KAISER_BESSEL = 1
+NORM_SUMWT, NORM_N, NORM_TAPER = 1, 2, 4
 
 
 @dataclass
@@ -31,12 +37,13 @@ class OracleParams:
     cell_rad: float
     w_min: float
     w_max: float
-    sigma: float = 1.0
+    sigma: float = 1.0          # Gaussian: sigma in cells; Kaiser-Bessel: beta
     tile: int = 32
+    kernel_type: int = 0
 
     def c(self) -> _Params:
         return _Params(self.n_pix, self.n_wplanes, self.support, self.tile, self.sigma, self.cell_rad,
-                       self.w_min, self.w_max)
+                       self.w_min, self.w_max, self.kernel_type, 0)
 
     @property
     def n_bins(self) -> int:
@@ -51,6 +58,8 @@ def lib():
         _lib.orc_bins.restype = C.c_int64
         _lib.orc_fft2.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int32
+        for f in ("orc_i0", "orc_kernel1d", "orc_taper1d", "orc_sum_weights"):
+            getattr(_lib, f).restype = C.c_double
     return _lib
 
 
@@ -117,6 +126,36 @@ def grid(prm: OracleParams, uvw, vis, wt, freq=None, plane_lo: int = 0, plane_hi
                    _p(fr, C.c_double), C.c_int64(uvw.shape[0]), C.c_int32(vis.shape[1]),
                    C.c_int32(plane_lo), C.c_int32(plane_hi), _p(G.view(np.float64), C.c_double))
     return G
+
+
+def i0(x: float) -> float:
+    return float(lib().orc_i0(C.c_double(x)))
+
+
+def kernel1d(prm: OracleParams, x: float) -> float:
+    """The 1-D convolution function g(x), x in cells (O5)."""
+    return float(lib().orc_kernel1d(C.byref(prm.c()), C.c_double(x)))
+
+
+def taper1d(prm: OracleParams, xi: float) -> float:
+    """Continuous Fourier transform of g at xi cycles per cell."""
+    return float(lib().orc_taper1d(C.byref(prm.c()), C.c_double(xi)))
+
+
+def sum_weights(prm: OracleParams, uvw, wt, freq=None) -> float:
+    uvw, _, _, fr = _inputs(uvw, freq=freq)
+    wt = np.ascontiguousarray(wt, dtype=np.float32)
+    return float(lib().orc_sum_weights(C.byref(prm.c()), _p(uvw, C.c_float), _p(wt, C.c_float), _p(fr, C.c_double),
+                                       C.c_int64(uvw.shape[0]), C.c_int32(wt.shape[1])))
+
+
+def dirty(prm: OracleParams, D: np.ndarray, flags: int = 0, sum_wt: float = 1.0) -> np.ndarray:
+    """a5: Re D times the normalisation factors `flags` selects (NORM_SUMWT | NORM_N | NORM_TAPER)."""
+    D = np.ascontiguousarray(D, dtype=np.complex128)
+    out = np.empty(D.shape, np.float64)
+    lib().orc_dirty(C.byref(prm.c()), _p(D.view(np.float64), C.c_double), C.c_uint32(flags), C.c_double(sum_wt),
+                    _p(out, C.c_double))
+    return out
 
 
 def dft2_naive(plane: np.ndarray) -> np.ndarray:

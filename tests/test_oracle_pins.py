@@ -206,8 +206,10 @@ def test_naive_dft_non_power_of_two_and_asymmetry(oracle):
 
 
 # --------------------------------------------------------------------------- P1: closed form, no mesh, no DFT
-def _closed_form_image(d):
-    """D(l,m) per visibility with numpy: wt V e^{2 pi i w_k t} [sum_a gu e^{2 pi i (i0+a-N/2) du l}] [same in v]."""
+def _closed_form_image(d, tap=None):
+    """D(l,m) per visibility with numpy: wt V e^{2 pi i w_k t} [sum_a gu e^{2 pi i (i0+a-N/2) du l}] [same in v].
+    `tap`: the 1-D convolution function (default: the Gaussian of PAPER.md:82)."""
+    tap = tap or (lambda x: _gauss(x, d.sigma_cells))
     N, h = d.n_pix, (d.support - 1) // 2
     pu, pv, pw = _independent_positions(d, d.n_chan)
     i0, j0 = np.floor(pu + 0.5), np.floor(pv + 0.5)
@@ -224,8 +226,8 @@ def _closed_form_image(d):
     D = np.zeros((N, N), np.complex128)
     a = np.arange(-h, h + 1)
     for n in np.flatnonzero(keep):
-        gu = _gauss(a - (pu[n] - i0[n]), d.sigma_cells)
-        gv = _gauss(a - (pv[n] - j0[n]), d.sigma_cells)
+        gu = tap(a - (pu[n] - i0[n]))
+        gv = tap(a - (pv[n] - j0[n]))
         fx = (gu[:, None] * np.exp(2j * np.pi * np.outer((i0[n] + a - N // 2) * du, x))).sum(0)   # [N] over l
         fy = (gv[:, None] * np.exp(2j * np.pi * np.outer((j0[n] + a - N // 2) * du, x))).sum(0)   # [N] over m
         D += val[n] * np.exp(2j * np.pi * wk[n] * t) * np.outer(fy, fx)
