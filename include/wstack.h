@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 110
+#define WS_VERSION 120
 
 /* error codes */
 #define WS_OK 0
@@ -65,8 +65,22 @@ extern "C" {
 #define WS_FLAG_LIBRARY_FFT 1u /* a3 through cuFFT even where the library's own two-pass FFT exists (N = 2^8..2^13) */
 #define WS_FLAG_NO_TRANSPOSE 2u /* WS_GRID_SPARSE keeps the [k][v][u] orientation (default: it may store the mesh transposed) */
 
-/* kernel_type */
-#define WS_KERNEL_GAUSSIAN 0 /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)) */
+#define WS_FLAG_TRACK_SUMWT 4u  /* every gridding call also sums the weights of the visibilities it kept (one extra
+                                   reduction kernel); needed by WS_NORM_SUMWT.  The sum restarts with ws_grid_zero and
+                                   with an OVERWRITE / SPARSE call and grows with ACCUMULATE calls */
+
+/* kernel_type: the separable 1-D convolution function g(x), x in cells, unit integral (R2, R28) */
+#define WS_KERNEL_GAUSSIAN 0      /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)), kernel_param = sigma */
+#define WS_KERNEL_KAISER_BESSEL 1 /* g(x) = I0(beta sqrt(1 - (2x/S)^2)) beta / (S sinh beta) on |x| <= S/2, kernel_param =
+                                     beta in (0, 24]; the production kernel PAPER.md:82 and :459 name (Jackson et al. 1991).
+                                     I0 is evaluated in registers from its power series, not from a table */
+
+/* norm_flags of ws_dirty_image: dirty = Re(image) times the product of the selected factors (R29) */
+#define WS_NORM_SUMWT 1u /* 1 / (sum of the weights of the gridded visibilities); plan needs WS_FLAG_TRACK_SUMWT          */
+#define WS_NORM_N 2u     /* n = sqrt(1 - l^2 - m^2): the 1/n on the left side of Eq. 2; 0 where l^2+m^2 >= 1 */
+#define WS_NORM_TAPER 4u /* 1 / (ghat(xi_p) ghat(xi_q)), xi = (p - N/2)/N, ghat the continuous Fourier transform of g:
+                            Gaussian exp(-2 pi^2 sigma^2 xi^2); Kaiser-Bessel (beta / sinh beta) sinh(r)/r,
+                            r = sqrt(beta^2 - (pi S xi)^2) (sin(r')/r' with r' = sqrt(-(..)) beyond) */
 
 typedef struct ws_plan ws_plan; /* opaque */
 
@@ -74,8 +88,8 @@ typedef struct ws_params {
     int32_t n_pix;        /* N: mesh and image side; multiple of 2*tile                                   */
     int32_t n_wplanes;    /* N_w >= 1                                                                      */
     int32_t support;      /* S: odd, 1..15; full S x S footprint ("kernel size of 7 cells")    */
-    int32_t kernel_type;  /* WS_KERNEL_GAUSSIAN                                                            */
-    double kernel_param;  /* Gaussian sigma in cells (> 0); 1.0 is the default reading R1                  */
+    int32_t kernel_type;  /* WS_KERNEL_GAUSSIAN or WS_KERNEL_KAISER_BESSEL                                 */
+    double kernel_param;  /* Gaussian: sigma in cells (> 0), 1.0 is the default reading R1; KB: beta        */
     double cell_rad;      /* image pixel size in radians (> 0)                                             */
     double w_min, w_max;  /* w range covered by the planes, wavelengths; w_max > w_min.  Plane k covers    */
                           /* [w_min + k dw, w_min + (k+1) dw), dw = (w_max-w_min)/N_w, value = midpoint     */
@@ -161,8 +175,15 @@ int ws_fft_columns(ws_plan* plan, void* grid, uint32_t fft_flags, void* stream);
 int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t accumulate, float* dirty,
                          uint32_t fft_flags, void* stream);
 
-/* ---- a5: dirty[q][p] = Re image[q][p]; norm_flags must be 0 ---------------------------- */
+/* ---- a5: dirty[q][p] = Re image[q][p] x normalisation (PAPER.md:86-88; Eq. 2 solved for I, :68) ---------- */
+/* norm_flags = 0: the plain real part.  Otherwise an OR of WS_NORM_*: with all three set and a Kaiser-Bessel
+ * kernel the result is the weighted-mean brightness, comparable to the direct sum
+ * n / sum(wt) * Re sum_k wt_k V_k exp(2 pi i (u l + v m + w (n - 1))) in the inner half of the field.
+ * WS_NORM_SUMWT without WS_FLAG_TRACK_SUMWT, or unknown bits: WS_ERR_INVALID_ARG. */
 int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream);
+
+/* Sum of the weights of the visibilities gridded so far (plan with WS_FLAG_TRACK_SUMWT; synchronises `stream`). */
+int ws_get_sum_weights(ws_plan* plan, double* sum_weights, void* stream);
 
 /* ---- the whole path from HOST buffers (end-to-end entry) ----------------------------------------------- */
 /* uvw_h, vis_h, weights_h, dirty_h are HOST pointers (pinned memory gives asynchronous copies); dev_inputs

@@ -97,6 +97,51 @@ int make_fft_plan(ws_plan* plan) {
     return WS_ERR_CUFFT;
 }
 
+// Continuous Fourier transform of the 1-D convolution function at xi cycles per cell (WS_NORM_TAPER, wstack.h).
+double kernel_taper(const ws_params& p, double xi) {
+    if (p.kernel_type == WS_KERNEL_KAISER_BESSEL) {
+        const double beta = p.kernel_param, a = PI * (double)p.support * xi, d = beta * beta - a * a;
+        double f = 1.0;
+        if (d > 1e-12) f = std::sinh(std::sqrt(d)) / std::sqrt(d);
+        else if (d < -1e-12) f = std::sin(std::sqrt(-d)) / std::sqrt(-d);
+        return f * beta / std::sinh(beta);
+    }
+    return std::exp(-2.0 * PI * PI * p.kernel_param * p.kernel_param * xi * xi);
+}
+
+// Tap constants of the gridder.  Gaussian: g(x) = norm1 2^(tap_c x^2).  Kaiser-Bessel: I0(beta sqrt(y)) as its power
+// series in y = 1 - (2x/S)^2, scaled by 1/I0(beta) so that the fp32 Horner sum stays in (0, 1]; every coefficient is
+// positive, so the sum has no cancellation.  Terms are kept until the tail is below 1e-9 of the peak.
+int make_taps(const ws_params& p, WsGeom& g) {
+    std::memset(g.kb_c, 0, sizeof(g.kb_c));
+    g.kb_terms = 0;
+    g.kb_y = 0.f;
+    if (p.kernel_type == WS_KERNEL_GAUSSIAN) {
+        const double sigma = p.kernel_param;
+        g.tap_c = (float)(-1.4426950408889634 / (2.0 * sigma * sigma));
+        g.norm2 = (float)(1.0 / (2.0 * PI * sigma * sigma));
+        return WS_OK;
+    }
+    const double beta = p.kernel_param, q = 0.25 * beta * beta, S = (double)p.support;
+    if (beta > 24.0) return WS_ERR_UNSUPPORTED;
+    double c[WS_KB_MAX_TERMS + 64], sum = 0.0;
+    const int n_all = WS_KB_MAX_TERMS + 64;
+    c[0] = 1.0;
+    for (int k = 1; k < n_all; ++k) c[k] = c[k - 1] * q / ((double)k * (double)k);
+    for (int k = 0; k < n_all; ++k) sum += c[k];          // = I0(beta) to fp64 accuracy (k up to 112 >> beta)
+    double tail = 0.0;
+    int terms = n_all;
+    while (terms > 1 && tail + c[terms - 1] < 1e-9 * sum) tail += c[--terms];
+    if (terms > WS_KB_MAX_TERMS) return WS_ERR_UNSUPPORTED;
+    for (int k = 0; k < terms; ++k) g.kb_c[k] = (float)(c[k] / sum);
+    g.kb_terms = terms;
+    g.kb_y = (float)(4.0 / (S * S));
+    g.tap_c = 0.f;
+    const double norm1 = beta / (S * std::sinh(beta)) * sum;   // g(x) = norm1 * (series / I0(beta))
+    g.norm2 = (float)(norm1 * norm1);
+    return WS_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -124,9 +169,11 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
     if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
-    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE)) != 0 || p->device < 0) return WS_ERR_INVALID_ARG;
+    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE | WS_FLAG_TRACK_SUMWT)) != 0 || p->device < 0)
+        return WS_ERR_INVALID_ARG;
+    if (!std::isfinite(p->kernel_param)) return WS_ERR_INVALID_ARG;
     if (p->support > 2 * WS_HALO_MAX + 1) return WS_ERR_UNSUPPORTED;
-    if (p->kernel_type != WS_KERNEL_GAUSSIAN) return WS_ERR_UNSUPPORTED;
+    if (p->kernel_type != WS_KERNEL_GAUSSIAN && p->kernel_type != WS_KERNEL_KAISER_BESSEL) return WS_ERR_UNSUPPORTED;
     if (p->tile != 0 && p->tile != WS_TILE) return WS_ERR_UNSUPPORTED;
     if (p->n_pix % (2 * WS_TILE) != 0 || p->n_pix > 32768) return WS_ERR_INVALID_ARG;
     const uint64_t nt = (uint64_t)p->n_pix / WS_TILE;
@@ -146,10 +193,15 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     g.halo = (p->support - 1) / 2;
     g.nt = (int32_t)nt;
     g.n_bins = (uint32_t)(nt * nt * (uint64_t)p->n_wplanes);
-    const double sigma = p->kernel_param;
-    g.tap_c = (float)(-1.4426950408889634 / (2.0 * sigma * sigma));
-    g.norm2 = (float)(1.0 / (2.0 * PI * sigma * sigma));
+    const int taps_rc = make_taps(*p, g);
+    if (taps_rc != WS_OK) {
+        delete plan;
+        return taps_rc;
+    }
     plan->fft_ok = false;
+    plan->d_sumwt = nullptr;
+    plan->d_taper = nullptr;
+    plan->last_weights = nullptr;
     plan->launches = 0;
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
@@ -162,10 +214,21 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->sm_count = prop.multiProcessorCount;
     plan->d_status = nullptr;
     plan->last_ws = nullptr;
-    if (cudaMalloc((void**)&plan->d_status, sizeof(WsStatus)) != cudaSuccess ||
-        cudaMemset(plan->d_status, 0, sizeof(WsStatus)) != cudaSuccess) {
-        delete plan;
-        return WS_ERR_CUDA;
+    {   // 1 / ghat per image column (= per row: the kernel is separable and the image square), fp64 on the host
+        std::vector<float> inv_taper((size_t)p->n_pix);
+        for (int i = 0; i < p->n_pix; ++i)
+            inv_taper[(size_t)i] = (float)(1.0 / kernel_taper(*p, (double)(i - p->n_pix / 2) / (double)p->n_pix));
+        if (cudaMalloc((void**)&plan->d_status, sizeof(WsStatus)) != cudaSuccess ||
+            cudaMemset(plan->d_status, 0, sizeof(WsStatus)) != cudaSuccess ||
+            cudaMalloc((void**)&plan->d_sumwt, 16) != cudaSuccess || cudaMemset(plan->d_sumwt, 0, 16) != cudaSuccess ||
+            cudaMalloc((void**)&plan->d_taper, inv_taper.size() * 4) != cudaSuccess ||
+            cudaMemcpy(plan->d_taper, inv_taper.data(), inv_taper.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+            if (plan->d_status) cudaFree(plan->d_status);
+            if (plan->d_sumwt) cudaFree(plan->d_sumwt);
+            if (plan->d_taper) cudaFree(plan->d_taper);
+            delete plan;
+            return WS_ERR_CUDA;
+        }
     }
     // a3: the FFT of ws_fft.cu where it exists (N = 2^8 .. 2^13), else (or on request) the library's
     plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix, p->n_wplanes);
@@ -181,6 +244,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
         if (plan->d_twiddles) cudaFree(plan->d_twiddles);
         if (plan->d_masks) cudaFree(plan->d_masks);
         cudaFree(plan->d_status);
+        cudaFree(plan->d_sumwt);
+        cudaFree(plan->d_taper);
         delete plan;
         return rc;
     }
@@ -192,6 +257,8 @@ int ws_plan_destroy(ws_plan* plan) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (plan->fft_ok) cufftDestroy(plan->fft);
     if (plan->d_status) cudaFree(plan->d_status);
+    if (plan->d_sumwt) cudaFree(plan->d_sumwt);
+    if (plan->d_taper) cudaFree(plan->d_taper);
     if (plan->d_twiddles) cudaFree(plan->d_twiddles);
     if (plan->d_masks) cudaFree(plan->d_masks);
     delete plan;
@@ -223,6 +290,7 @@ int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_zero: null argument");
     int rc = ws_launch_zero(plan, grid, ws_grid_bytes(plan), (cudaStream_t)stream);
     if (rc >= 0) rc = ws_launch_fft_masks_clear(plan, (cudaStream_t)stream);
+    if (rc >= 0 && cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), (cudaStream_t)stream) != cudaSuccess) rc = WS_ERR_CUDA;
     if (rc < 0) return fail(plan, rc, "ws_grid_zero: memset failed");
     plan->occ_grid = grid;                               // an empty mesh: the occupancy masks describe it
     plan->occ_sparse = false;
@@ -274,6 +342,7 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
     plan->last_ws = workspace;
     plan->last_layout = L;
     plan->last_n_vis = n_vis;
+    plan->last_weights = weights;
     plan->last_valid = true;
     return WS_OK;
 }
@@ -307,6 +376,14 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
         } else {
             plan->occ_grid = nullptr;                    // accumulation onto a mesh this plan has no record of
         }
+    }
+    if (plan->prm.flags & WS_FLAG_TRACK_SUMWT) {
+        if (mode != WS_GRID_ACCUMULATE && cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), (cudaStream_t)stream) != cudaSuccess)
+            return fail(plan, WS_ERR_CUDA, "ws_grid_binned: memset failed");
+        rc = ws_launch_sum_weights(plan, plan->last_layout, (char*)workspace, plan->last_weights, plan->last_n_vis,
+                                   (cudaStream_t)stream);
+        if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
+        plan->launches += rc;
     }
     rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
@@ -410,12 +487,26 @@ int ws_fft_wcorrect(ws_plan* plan, void* grid, void* image, int32_t accumulate, 
 
 int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream) {
     if (!plan || !image || !dirty) return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: null argument");
-    if (norm_flags != 0) return fail(plan, WS_ERR_UNSUPPORTED, "ws_dirty_image: norm_flags must be 0");
+    if (norm_flags & ~(uint32_t)(WS_NORM_SUMWT | WS_NORM_N | WS_NORM_TAPER))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: unknown norm_flags");
+    if ((norm_flags & WS_NORM_SUMWT) && !(plan->prm.flags & WS_FLAG_TRACK_SUMWT))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: WS_NORM_SUMWT needs a plan created with WS_FLAG_TRACK_SUMWT");
     if (((uintptr_t)image | (uintptr_t)dirty) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: pointers must be 16-byte aligned");
-    const int rc = ws_launch_dirty(plan, (const float2*)image, dirty, (cudaStream_t)stream);
+    const int rc = ws_launch_dirty(plan, (const float2*)image, dirty, norm_flags, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_dirty_image: launch failed");
     plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_get_sum_weights(ws_plan* plan, double* sum_weights, void* stream) {
+    if (!plan || !sum_weights) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_sum_weights: null argument");
+    if (!(plan->prm.flags & WS_FLAG_TRACK_SUMWT))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_get_sum_weights: plan was not created with WS_FLAG_TRACK_SUMWT");
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_sum_weights: synchronize");
+    e = cudaMemcpy(sum_weights, plan->d_sumwt, sizeof(double), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(plan, e, "ws_get_sum_weights: copy");
     return WS_OK;
 }
 

@@ -4,6 +4,8 @@
 // key), exclusive prefix scan (warp shuffles), and a scatter that writes, per bin, contiguous 16-byte records
 // the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
 // it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
+#include <algorithm>
+
 #include "ws_internal.h"
 
 namespace {
@@ -307,7 +309,34 @@ k_sorted_keys(const uint32_t* __restrict__ bin_start, uint32_t n_bins, uint32_t*
     for (uint32_t i = s + lane; i < e; i += 32) sorted_keys[i] = w;
 }
 
+// ---- WS_FLAG_TRACK_SUMWT: sum of the weights of the kept visibilities (keys[] != 0xFFFFFFFF), fp64 --------------
+__global__ void __launch_bounds__(256)
+k_sum_weights(const uint32_t* __restrict__ keys, const float* __restrict__ wt, uint32_t n_vis, double* __restrict__ sum) {
+    __shared__ double s_part[8];
+    double acc = 0.0;
+    for (uint32_t m = blockIdx.x * 256u + threadIdx.x; m < n_vis; m += gridDim.x * 256u)
+        if (__ldcs(keys + m) != 0xFFFFFFFFu) acc += (double)__ldcs(wt + m);
+#pragma unroll
+    for (int d = 16; d; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) t += s_part[i];
+        atomicAdd(sum, t);
+    }
+}
+
 }  // namespace
+
+int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, cudaStream_t st) {
+    if (n_vis <= 0) return 0;
+    const unsigned blocks = (unsigned)std::min<int64_t>((n_vis + 255) / 256, (int64_t)plan->sm_count * 8);
+    k_sum_weights<<<blocks, 256, 0, st>>>((const uint32_t*)(ws + L.off_keys), wt, (uint32_t)n_vis, plan->d_sumwt);
+    if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+    return 1;
+}
 
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {

@@ -9,7 +9,8 @@
 //     collisions and no atomics), and writes it ONCE with coalesced stores -- in WS_GRID_OVERWRITE mode the
 //     tile (zeros included) is simply stored, so the mesh needs no memset and no read-modify-write;
 //   * taps are evaluated in registers, 32 visibilities at a time (lane r evaluates the 2 S taps of record r
-//     with ex2.approx and parks them in shared memory), then lane (a, b) of the warp applies tap (a, b) of
+//     -- Gaussian: ex2.approx; Kaiser-Bessel: the power series of I0 by Horner's rule, all 2 S
+//     taps side by side -- and parks them in shared memory), then lane (a, b) of the warp applies tap (a, b) of
 //     one record after the other;
 //   * a bin with more than WS_CHUNK records ("heavy": the dense core of the uv plane) is cut
 //     into chunks that become work items of their own; k_prepare_heavy queues them and clears their tiles,
@@ -79,14 +80,50 @@ struct WarpSmem {
     }
 };
 
+// The 2 S taps of one record: gu[i] = g(i - h - fx) / norm1, gv likewise (norm1^2 is folded into weight * vis).
+template <int S, bool KB>
+__device__ __forceinline__ void eval_taps(const WsGeom& g, float fx, float fy, float* gu, float* gv) {
+    constexpr int H = (S - 1) / 2;
+    if constexpr (!KB) {
+        const float tap_c = g.tap_c;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const float dx = (float)(i - H) - fx, dy = (float)(i - H) - fy;
+            gu[i] = ex2_approx(tap_c * dx * dx);
+            gv[i] = ex2_approx(tap_c * dy * dy);
+        }
+    } else {
+        // I0(beta sqrt(y)) / I0(beta) = sum_k c_k y^k, y = 1 - (2x/S)^2 in [0, 1], c_k > 0: Horner without cancellation
+        float yu[S], yv[S];
+        const float ky = g.kb_y;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const float dx = (float)(i - H) - fx, dy = (float)(i - H) - fy;
+            yu[i] = fmaxf(fmaf(-ky * dx, dx, 1.0f), 0.0f);
+            yv[i] = fmaxf(fmaf(-ky * dy, dy, 1.0f), 0.0f);
+        }
+        int k = g.kb_terms - 1;
+        const float top = g.kb_c[k];
+#pragma unroll
+        for (int i = 0; i < S; ++i) gu[i] = gv[i] = top;
+        for (--k; k >= 0; --k) {
+            const float c = g.kb_c[k];
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                gu[i] = fmaf(gu[i], yu[i], c);
+                gv[i] = fmaf(gv[i], yv[i], c);
+            }
+        }
+    }
+}
+
 // Accumulates records [lo, hi) into the warp's shared tile.
-template <int S>
+template <int S, bool KB>
 __device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
                                            const WarpSmem<S>& sm, int lane) {
     using C = TileCfg<S>;
     const int a = lane % S, br = lane / S;
     const bool active = br < C::R;
-    const float tap_c = g.tap_c;
     const int lane_idx = br * C::P + a;            // tap (a, br) relative to the footprint's first cell
     float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lo + lane < hi) nxt = __ldcs(records + lo + lane);
@@ -97,11 +134,12 @@ __device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __rest
             const int cxp = ((int)X >> 24) - C::H, cyp = ((int)Y >> 24) - C::H;   // footprint's first cell, tile frame
             const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
             const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
+            float gu[S], gv[S];
+            eval_taps<S, KB>(g, fx, fy, gu, gv);
 #pragma unroll
             for (int i = 0; i < S; ++i) {
-                const float dx = (float)(i - C::H) - fx, dy = (float)(i - C::H) - fy;
-                sm.gu[lane * S + i] = ex2_approx(tap_c * dx * dx);
-                sm.gv[lane * S + i] = ex2_approx(tap_c * dy * dy);
+                sm.gu[lane * S + i] = gu[i];
+                sm.gv[lane * S + i] = gv[i];
             }
             sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cxp & 0xFFFF) | (cyp << 16)),
                                         __int_as_float(cyp * C::P + cxp));
@@ -190,7 +228,7 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
 }
 
 // Persistent kernel: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
-template <int S>
+template <int S, bool KB>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 2)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint4* __restrict__ items,
        const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
@@ -215,7 +253,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         it += n_warps;
         float2* out = tile_origin(g, grid, w.x, tr);
         zero_tile<S>(sm.tile, lane);
-        accumulate<S>(g, records, w.y, w.z, sm, lane);
+        accumulate<S, KB>(g, records, w.y, w.z, sm, lane);
 #pragma unroll 4
         for (int y = 0; y < T; ++y) {
             const float2 v = tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane];
@@ -238,7 +276,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
             continue;
         }
         zero_tile<S>(sm.tile, lane);
-        accumulate<S>(g, records, s, e, sm, lane);
+        accumulate<S, KB>(g, records, s, e, sm, lane);
         if (mode != WS_GRID_ACCUMULATE) {
 #pragma unroll 4
             for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane]);
@@ -258,14 +296,14 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
     while (it < n_items) do_item();
 }
 
-template <int S>
+template <int S, bool KB>
 int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
     const uint32_t* orient = mode == WS_GRID_SPARSE ? ws_fft_orientation_flag(plan) : nullptr;
     using C = TileCfg<S>;
     const size_t smem = C::WARP_BYTES * C::WARPS;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_grid<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_grid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return WS_ERR_CUDA;
         attr_set = true;
     }
@@ -276,7 +314,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
     k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient);
-    k_grid<S><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient);
+    k_grid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }
@@ -284,15 +322,16 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 }  // namespace
 
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
+    const bool kb = plan->geom.kb_terms > 0;
     switch (plan->geom.support) {
-        case 1: return launch_s<1>(plan, L, ws, grid, mode, st);
-        case 3: return launch_s<3>(plan, L, ws, grid, mode, st);
-        case 5: return launch_s<5>(plan, L, ws, grid, mode, st);
-        case 7: return launch_s<7>(plan, L, ws, grid, mode, st);
-        case 9: return launch_s<9>(plan, L, ws, grid, mode, st);
-        case 11: return launch_s<11>(plan, L, ws, grid, mode, st);
-        case 13: return launch_s<13>(plan, L, ws, grid, mode, st);
-        case 15: return launch_s<15>(plan, L, ws, grid, mode, st);
+        case 1: return kb ? launch_s<1, true>(plan, L, ws, grid, mode, st) : launch_s<1, false>(plan, L, ws, grid, mode, st);
+        case 3: return kb ? launch_s<3, true>(plan, L, ws, grid, mode, st) : launch_s<3, false>(plan, L, ws, grid, mode, st);
+        case 5: return kb ? launch_s<5, true>(plan, L, ws, grid, mode, st) : launch_s<5, false>(plan, L, ws, grid, mode, st);
+        case 7: return kb ? launch_s<7, true>(plan, L, ws, grid, mode, st) : launch_s<7, false>(plan, L, ws, grid, mode, st);
+        case 9: return kb ? launch_s<9, true>(plan, L, ws, grid, mode, st) : launch_s<9, false>(plan, L, ws, grid, mode, st);
+        case 11: return kb ? launch_s<11, true>(plan, L, ws, grid, mode, st) : launch_s<11, false>(plan, L, ws, grid, mode, st);
+        case 13: return kb ? launch_s<13, true>(plan, L, ws, grid, mode, st) : launch_s<13, false>(plan, L, ws, grid, mode, st);
+        case 15: return kb ? launch_s<15, true>(plan, L, ws, grid, mode, st) : launch_s<15, false>(plan, L, ws, grid, mode, st);
     }
     return WS_ERR_UNSUPPORTED;
 }

@@ -12,6 +12,7 @@
 #define WS_MAX_CHAN 128       // per-channel constants travel as a kernel parameter
 #define WS_CHUNK 1024         // records a warp accumulates in shared memory before it flushes
 #define WS_HALO_MAX 7         // (S-1)/2 for S <= 15
+#define WS_KB_MAX_TERMS 48    // terms of the I0 power series kept for the Kaiser-Bessel taps (beta <= 24)
 #define WS_WC_GROUP 8          // planes per Horner block in the w-correction (exact restart between blocks)
 
 // Per-channel position constants (O1): fp64, computed on the host exactly as the header states.
@@ -28,7 +29,11 @@ struct WsGeom {
     int32_t nt;                                 // N / T
     uint32_t n_bins;                            // N_w nt^2
     float tap_c;                                // -log2(e) / (2 sigma^2): g(x) = norm1 * 2^(tap_c x^2)
-    float norm2;                                // 1 / (2 pi sigma^2): product of the two 1-D normalisations
+    float norm2;                                // product of the two 1-D normalisations (folded into weight * vis once)
+    // Kaiser-Bessel: g(x) / norm1 = sum_k kb_c[k] y^k, y = 1 - kb_y x^2, kb_c[k] = (beta^2/4)^k / (k!)^2 / I0(beta)
+    int32_t kb_terms;                           // 0: Gaussian
+    float kb_y;                                 // 4 / S^2
+    float kb_c[WS_KB_MAX_TERMS];
 };
 
 // Workspace carve-up for one ws_grid_visibilities call (all offsets 256-byte aligned).
@@ -77,6 +82,9 @@ struct ws_plan {
     size_t tw_off_a, tw_off_b;                  // entry offsets of the pass 1a / 1b tables
     void* d_masks;                              // plan-owned tile-occupancy masks of the mesh (class masks, band masks)
     size_t mask_words, mask_set_words;          // whole buffer; one set (class masks + band masks) of the two orientations
+    double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)
+    float* d_taper;                             // plan-owned [N]: 1 / ghat((p - N/2)/N), fp64-computed on the host
+    const float* last_weights;                  // weights of the last ws_bin_visibilities call
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
     bool occ_sparse;                            // ... and it was written by WS_GRID_SPARSE (private layout, empty tiles unwritten)
 };
@@ -90,7 +98,8 @@ int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int
 int ws_launch_sorted_keys(ws_plan* plan, const WsLayout& L, char* ws, cudaStream_t st);
 int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
                        cudaStream_t st);
-int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, cudaStream_t st);
+int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, uint32_t norm_flags, cudaStream_t st);
+int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, cudaStream_t st);
 int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);
 bool ws_fft_own_supported(int n_pix, int n_wplanes);
 int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error

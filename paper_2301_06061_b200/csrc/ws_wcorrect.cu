@@ -84,6 +84,33 @@ k_dirty(const float4* __restrict__ image, float2* __restrict__ dirty, uint64_t n
     dirty[tid] = make_float2(v.x, v.z);
 }
 
+// a5 with normalisation (wstack.h WS_NORM_*; Eq. 2 solved for I): Re(image) times 1 / sum of weights,
+// n = sqrt(1 - l^2 - m^2) (fp64, 0 outside the unit circle) and 1 / (ghat(xi_p) ghat(xi_q)) from the plan's table.
+__global__ void __launch_bounds__(256)
+k_dirty_norm(const float4* __restrict__ image, float2* __restrict__ dirty, uint32_t N, double cell, uint32_t flags,
+             const double* __restrict__ sum_wt, const float* __restrict__ inv_taper) {
+    const uint32_t pairs = N >> 1;
+    const uint64_t tid = (uint64_t)blockIdx.x * 256u + threadIdx.x;
+    if (tid >= (uint64_t)N * pairs) return;
+    const uint32_t q = (uint32_t)(tid / pairs), p = (uint32_t)(tid - (uint64_t)q * pairs) * 2u;
+    const float4 v = __ldcs(image + tid);
+    double fa = 1.0, fb = 1.0;
+    if (flags & WS_NORM_SUMWT) fa = fb = 1.0 / *sum_wt;
+    if (flags & WS_NORM_N) {
+        const int half = (int)(N >> 1);
+        const double m = (double)((int)q - half) * cell, la = (double)((int)p - half) * cell, lb = (double)((int)p + 1 - half) * cell;
+        const double ra = la * la + m * m, rb = lb * lb + m * m;
+        fa *= ra < 1.0 ? sqrt(1.0 - ra) : 0.0;
+        fb *= rb < 1.0 ? sqrt(1.0 - rb) : 0.0;
+    }
+    if (flags & WS_NORM_TAPER) {
+        const double tq = (double)inv_taper[q];
+        fa *= tq * (double)inv_taper[p];
+        fb *= tq * (double)inv_taper[p + 1];
+    }
+    dirty[tid] = make_float2((float)((double)v.x * fa), (float)((double)v.z * fb));
+}
+
 }  // namespace
 
 int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
@@ -102,8 +129,15 @@ int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int a
     return 1;
 }
 
-int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, cudaStream_t st) {
+int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, uint32_t norm_flags, cudaStream_t st) {
     const uint64_t n_pairs = (uint64_t)plan->prm.n_pix * (uint64_t)(plan->prm.n_pix / 2);
+    if (norm_flags) {
+        k_dirty_norm<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>((const float4*)image, (float2*)dirty,
+                                                                        (uint32_t)plan->prm.n_pix, plan->prm.cell_rad, norm_flags,
+                                                                        plan->d_sumwt, plan->d_taper);
+        if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+        return 1;
+    }
     k_dirty<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>((const float4*)image, (float2*)dirty, n_pairs);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;

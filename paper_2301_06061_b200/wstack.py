@@ -16,12 +16,16 @@ WS_FLAG_LIBRARY_FFT = 1
 WS_FLAG_NO_TRANSPOSE = 2
 WS_GRID_SPARSE = 2
 WS_FFT_USE_OCCUPANCY = 1
+WS_FLAG_TRACK_SUMWT = 4
+WS_KERNEL_GAUSSIAN = 0
+WS_KERNEL_KAISER_BESSEL = 1
+WS_NORM_SUMWT, WS_NORM_N, WS_NORM_TAPER = 1, 2, 4
 
 EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count",
 ]
 
@@ -76,6 +80,7 @@ def lib():
         "ws_plan_fft_is_own": (C.c_int, [vp]),
         "ws_get_occupancy": (C.c_int, [vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(i32), vp]),
         "ws_dirty_image": (C.c_int, [vp, vp, vp, u32, vp]),
+        "ws_get_sum_weights": (C.c_int, [vp, C.POINTER(C.c_double), vp]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
                                   C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
@@ -111,9 +116,12 @@ class Plan:
     """An imaging plan (ws_plan).  All buffers are torch CUDA tensors owned by the caller."""
 
     def __init__(self, n_pix: int, n_wplanes: int, support: int, cell_rad: float, w_min: float, w_max: float,
-                 sigma: float = 1.0, tile: int = 0, device: int = 0, flags: int = 0):
+                 sigma: float = 1.0, tile: int = 0, device: int = 0, flags: int = 0,
+                 kernel_type: int = WS_KERNEL_GAUSSIAN, kernel_param: Optional[float] = None):
+        """kernel_param: Gaussian sigma in cells / Kaiser-Bessel beta; `sigma` is the older name of the same field."""
         self._h = C.c_void_p()
-        prm = _Params(n_pix, n_wplanes, support, 0, sigma, cell_rad, w_min, w_max, tile, device, flags)
+        prm = _Params(n_pix, n_wplanes, support, kernel_type, sigma if kernel_param is None else kernel_param,
+                      cell_rad, w_min, w_max, tile, device, flags)
         rc = lib().ws_plan_create(C.byref(prm), C.byref(self._h))
         if rc != 0:
             self._h = C.c_void_p()
@@ -234,9 +242,14 @@ class Plan:
                                                _dev(image, torch.complex64, "image"), int(accumulate), d, fft_flags,
                                                _stream(stream)))
 
-    def dirty_image(self, image, dirty, stream=None):
+    def dirty_image(self, image, dirty, norm_flags: int = 0, stream=None):
         self._check(lib().ws_dirty_image(self._h, _dev(image, torch.complex64, "image"),
-                                         _dev(dirty, torch.float32, "dirty"), 0, _stream(stream)))
+                                         _dev(dirty, torch.float32, "dirty"), norm_flags, _stream(stream)))
+
+    def sum_weights(self, stream=None) -> float:
+        v = C.c_double()
+        self._check(lib().ws_get_sum_weights(self._h, C.byref(v), _stream(stream)))
+        return v.value
 
     def image_from_host(self, uvw_h, vis_h, weights_h, freq_hz, dev_inputs, grid, image, dirty_d, dirty_h, workspace,
                         stream=None):
