@@ -79,9 +79,19 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+KERNEL = "gaussian"     # --kernel: "gaussian" (the headline workload) or "kb" (Kaiser-Bessel, :459)
+
+
+def kb_beta(support, alpha=2.0):
+    """Kaiser-Bessel shape for a window of `support` cells and the inner 1/alpha of the field (Beatty et al.)."""
+    return float(np.pi * np.sqrt((support / alpha) ** 2 * (alpha - 0.5) ** 2 - 0.8))
+
+
 def oracle_params(orc, d, tile=32):
+    kb = KERNEL == "kb"
     return orc.OracleParams(n_pix=d.n_pix, n_wplanes=d.n_wplanes, support=d.support, cell_rad=d.cell_rad,
-                            w_min=d.w_min, w_max=d.w_max, sigma=d.sigma_cells, tile=tile)
+                            w_min=d.w_min, w_max=d.w_max, sigma=kb_beta(d.support) if kb else d.sigma_cells, tile=tile,
+                            kernel_type=1 if kb else 0)
 
 
 def cpu_baseline(d, n_sample_planes=2):
@@ -123,7 +133,8 @@ def run_reference(args, d, cfg_name):
 
 def workload_config(d, cfg_name):
     return {"workload": f"{cfg_name}: {d.n_vis} visibilities ({d.n_rows} rows x {d.n_chan} channels), "
-                        f"{d.n_pix}x{d.n_pix} complex64 mesh, {d.n_wplanes} w-planes, Gaussian support {d.support}",
+                        f"{d.n_pix}x{d.n_pix} complex64 mesh, {d.n_wplanes} w-planes, "
+                        + ("Kaiser-Bessel (beta %.2f)" % kb_beta(d.support) if KERNEL == "kb" else "Gaussian") + f" support {d.support}",
             "n_vis": d.n_vis, "n_pix": d.n_pix, "n_wplanes": d.n_wplanes, "support": d.support,
             "l2": "inputs (%.2f GB) and mesh (%.1f GB) larger than the 126 MB L2; no flush needed" %
                   ((12 * d.n_rows + 12 * d.n_vis) / 1e9, 8.0 * d.n_pix ** 2 * d.n_wplanes / 1e9)}
@@ -136,9 +147,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="large")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel", default="gaussian", choices=["gaussian", "kb"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
+    global KERNEL
+    KERNEL = args.kernel
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     rank = int(os.environ.get("RANK", "0"))
@@ -164,7 +178,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
 
     d = make_dataset(cfg, device=f"cuda:{local_rank}")
-    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank)
+    if KERNEL == "kb":
+        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, device=local_rank,
+                       kernel_type=ws.WS_KERNEL_KAISER_BESSEL, kernel_param=kb_beta(d.support))
+    else:
+        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank)
     grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
     wsp = plan.alloc_workspace(d.n_vis)
 

@@ -31,6 +31,11 @@
  *   orc_sum_weights    sum of the weights of the kept visibilities (the normalisation of the direct sum).
  *   orc_dirty          PAPER.md:68 Eq. 2 solved for I: the factor n = sqrt(1-l^2-m^2) of its left side, the
  *                      division by the taper and by the sum of weights (readings R12 / R29).
+ *   orc_wscreen_fwd    degridding, step 1 ("the degridding procedure (transforming from the image to
+ *                      the visibility space)"; Eq. 1 at :59): model image times exp(-2 pi i w_k (n-1)).
+ *   orc_degrid         degridding, step 3: every visibility reads its S x S footprint of the forward-transformed
+ *                      plane k through the same convolution function (the transpose of Eq. 3, :80).
+ *                      Step 2, the forward DFT, is conj(orc_dft2(conj(.))) in oracle/wstack_oracle.py.
  *   orc_image_samples  the composition orc_grid -> DFT -> orc_wcorrect evaluated at single pixels
  *                      with the order of the (finite, linear) sums exchanged: visibility outermost.
  *                      Used where a full fp64 plane stack would not fit; pinned against the chain.
@@ -453,6 +458,62 @@ void orc_image_samples(const orc_params *p, const float *uvw, const float *vis, 
         D[2 * s] = sr; D[2 * s + 1] = si;
     }
     free(part); free(wph); free(E); free(su); free(sw);
+}
+
+/* ---- degridding: image -> visibilities (Eq. 1 :59 discretised; reading R30) ---------- */
+/* Step 1: Q[q][p] = M[q][p] exp(-2 pi i w_k t), t = n - 1 as in O8; pixels with r^2 >= 1 give 0 (R14).   */
+void orc_wscreen_fwd(const orc_params *p, const double *M, int32_t k, double *Q) {
+    const int N = p->n_pix;
+    const double dw = (p->w_max - p->w_min) / (double)p->n_wplanes;
+    const double wk = p->w_min + ((double)k + 0.5) * dw;
+#pragma omp parallel for
+    for (int q = 0; q < N; ++q)
+        for (int pp = 0; pp < N; ++pp) {
+            size_t idx = 2 * ((size_t)q * N + pp);
+            double l = (double)(pp - N / 2) * p->cell_rad, m = (double)(q - N / 2) * p->cell_rad;
+            double r2 = l * l + m * m;
+            if (r2 >= 1.0) { Q[idx] = 0.0; Q[idx + 1] = 0.0; continue; }
+            double t = -r2 / (1.0 + sqrt(1.0 - r2));
+            double ph = -2.0 * ORC_PI * wk * t;
+            double c = cos(ph), s = sin(ph);
+            Q[idx] = c * M[idx] - s * M[idx + 1];
+            Q[idx + 1] = s * M[idx] + c * M[idx + 1];
+        }
+}
+
+/* Step 3: V_m = sum_{a,b} g(a - fu) g(b - fv) H[(k - plane_lo)][j0 + b][i0 + a] for every kept visibility   */
+/* whose plane lies in [plane_lo, plane_hi); others are left untouched (the caller starts from zeros, so a    */
+/* dropped visibility predicts 0).  H: forward-transformed planes, logical centred layout.  out: re,im.       */
+void orc_degrid(const orc_params *p, const float *uvw, const double *freq_hz, int64_t n_rows, int32_t n_chan,
+                int32_t plane_lo, int32_t plane_hi, const double *H, double *out) {
+    const int N = p->n_pix, S = p->support, h = (S - 1) / 2;
+    double *su = malloc(sizeof(double) * n_chan), *sw = malloc(sizeof(double) * n_chan), ow;
+    orc_channel_constants(p, freq_hz, n_chan, su, sw, &ow);
+#pragma omp parallel for
+    for (int64_t r = 0; r < n_rows; ++r) {
+        double gu[32], gv[32];
+        double u = (double)uvw[3 * r], v = (double)uvw[3 * r + 1], w = (double)uvw[3 * r + 2];
+        for (int c = 0; c < n_chan; ++c) {
+            int32_t i0, j0, k; double fu, fv;
+            if (!orc_place(p, u, v, w, su[c], sw[c], ow, &i0, &j0, &k, &fu, &fv) || k < plane_lo || k >= plane_hi) continue;
+            const double *Hk = H + (size_t)(k - plane_lo) * (size_t)N * (size_t)N * 2;
+            for (int a = -h; a <= h; ++a) {
+                gu[a + h] = orc_kernel1d(p, (double)a - fu);
+                gv[a + h] = orc_kernel1d(p, (double)a - fv);
+            }
+            double sr = 0.0, si = 0.0;
+            for (int b = -h; b <= h; ++b)
+                for (int a = -h; a <= h; ++a) {
+                    double t = gu[a + h] * gv[b + h];
+                    size_t cell = ((size_t)(j0 + b) * (size_t)N + (size_t)(i0 + a)) * 2;
+                    sr += t * Hk[cell];
+                    si += t * Hk[cell + 1];
+                }
+            out[2 * (r * n_chan + c)] = sr;
+            out[2 * (r * n_chan + c) + 1] = si;
+        }
+    }
+    free(su); free(sw);
 }
 
 /* ---- normalisation of the image (Eq. 2 solved for I; readings R12, R29) ------------------- */

@@ -191,6 +191,45 @@ def wcorrect(prm: OracleParams, planes: np.ndarray, plane_lo: int = 0, out: Opti
     return D
 
 
+def transform_fwd(plane: np.ndarray, naive_max: int = 512) -> np.ndarray:
+    """Forward un-normalised centred DFT (sign -): the conjugate of the inverse one of the conjugate."""
+    return np.conj(transform(np.conj(np.asarray(plane, dtype=np.complex128)), naive_max))
+
+
+def wscreen_fwd(prm: OracleParams, model: np.ndarray, k: int) -> np.ndarray:
+    """Degridding step 1: model image times exp(-2 pi i w_k (n - 1))."""
+    model = np.ascontiguousarray(model, dtype=np.complex128)
+    out = np.empty_like(model)
+    lib().orc_wscreen_fwd(C.byref(prm.c()), _p(model.view(np.float64), C.c_double), C.c_int32(k),
+                          _p(out.view(np.float64), C.c_double))
+    return out
+
+
+def degrid(prm: OracleParams, uvw, n_chan: int, freq, planes: np.ndarray, plane_lo: int = 0,
+           out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Degridding step 3 for the visibilities of planes [plane_lo, plane_lo + len(planes)): complex128 [n_rows, n_chan]."""
+    uvw, _, _, fr = _inputs(uvw, freq=freq)
+    planes = np.ascontiguousarray(planes, dtype=np.complex128)
+    V = np.zeros((uvw.shape[0], n_chan), np.complex128) if out is None else out
+    lib().orc_degrid(C.byref(prm.c()), _p(uvw, C.c_float), _p(fr, C.c_double), C.c_int64(uvw.shape[0]), C.c_int32(n_chan),
+                     C.c_int32(plane_lo), C.c_int32(plane_lo + planes.shape[0]), _p(planes.view(np.float64), C.c_double),
+                     _p(V.view(np.float64), C.c_double))
+    return V
+
+
+def predict(prm: OracleParams, model: np.ndarray, uvw, n_chan: int, freq=None, return_planes: bool = False,
+            naive_max: int = 512):
+    """The degridding chain, plane-streamed: w-screen -> forward transform -> gather.  complex128 [n_rows, n_chan]."""
+    V = np.zeros((np.asarray(uvw).shape[0], n_chan), np.complex128)
+    stack = [] if return_planes else None
+    for k in range(prm.n_wplanes):
+        H = transform_fwd(wscreen_fwd(prm, model, k), naive_max)
+        if return_planes:
+            stack.append(H)
+        degrid(prm, uvw, n_chan, freq, H[None], k, V)
+    return (V, np.stack(stack)) if return_planes else V
+
+
 def image_samples(prm: OracleParams, uvw, vis, wt, freq, q: Sequence[int], p: Sequence[int]) -> np.ndarray:
     """The whole chain at pixels (q[s], p[s]), visibility-outermost; complex128 [n_samp]."""
     uvw, vis, wt, fr = _inputs(uvw, vis, wt, freq)
