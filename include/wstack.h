@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 120
+#define WS_VERSION 130
 
 /* error codes */
 #define WS_OK 0
@@ -184,6 +184,24 @@ int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm
 
 /* Sum of the weights of the visibilities gridded so far (plan with WS_FLAG_TRACK_SUMWT; synchronises `stream`). */
 int ws_get_sum_weights(ws_plan* plan, double* sum_weights, void* stream);
+
+/* ---- degridding: model image -> predicted visibilities (Eq. 1 at :59) -------------------- */
+/* The adjoint of ws_grid_visibilities (unit weights) -> ws_fft_planes -> ws_wcorrect_accumulate, in two calls:
+ *   ws_predict_planes       planes[k] = forward un-normalised 2-D DFT of model_image x exp(-2 pi i w_k (n - 1)),
+ *                           k = 0..N_w-1, FFT-native storage order like the mesh (cuFFT; needs `workspace` >=
+ *                           ws_fft_workspace_bytes).  model_image: complex64 [N][N], centred, the APPARENT sky
+ *                           (Eq. 1's I / n), already divided by the kernel taper ghat(xi_p) ghat(xi_q) if calibrated
+ *                           visibilities are wanted; pixels with l^2 + m^2 >= 1 are ignored.
+ *   ws_degrid_visibilities  vis_out[row][chan] (complex64) = [accumulate ? vis_out : 0] + scale x
+ *                           sum_{a,b} g(a - fu) g(b - fv) planes[k][j0 + b][i0 + a], positions by the rule of
+ *                           ws_grid_visibilities; a dropped visibility predicts 0.  scale = -1 with accumulate = 1 turns
+ *                           measured visibilities into residuals.  Bins the positions into `workspace` first (same
+ *                           size rules as ws_grid_visibilities; ws_get_bins works afterwards, ws_grid_binned does not). */
+int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void* workspace, size_t workspace_bytes,
+                      void* stream);
+int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_hz, int64_t n_rows, int32_t n_chan,
+                           const void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
+                           size_t workspace_bytes, void* stream);
 
 /* ---- the whole path from HOST buffers (end-to-end entry) ----------------------------------------------- */
 /* uvw_h, vis_h, weights_h, dirty_h are HOST pointers (pinned memory gives asynchronous copies); dev_inputs

@@ -202,6 +202,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->d_sumwt = nullptr;
     plan->d_taper = nullptr;
     plan->last_weights = nullptr;
+    plan->last_has_values = false;
     plan->launches = 0;
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
@@ -297,15 +298,16 @@ int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     return WS_OK;
 }
 
-int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
-                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
-                        size_t workspace_bytes, void* stream) {
+// a1 for the gridder (with_values) and for the degridder (positions only: vis and weights are not read)
+static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const float* weights, const double* freq_hz,
+                    int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (n_rows < 0 || n_chan <= 0) return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad n_rows / n_chan");
     if (n_chan > WS_MAX_CHAN) return fail(plan, WS_ERR_UNSUPPORTED, "ws_bin_visibilities: n_chan > 128");
     if (n_rows > MAX_VIS || n_rows * n_chan > MAX_VIS)
         return fail(plan, WS_ERR_UNSUPPORTED, "ws_bin_visibilities: more than 2^30 visibilities in one call");
-    if (!workspace || (n_rows > 0 && (!uvw || !vis || !weights)))
+    if (!with_values) vis = nullptr, weights = nullptr;
+    if (!workspace || (n_rows > 0 && (!uvw || (with_values && (!vis || !weights)))))
         return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: null pointer");
     if (((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)workspace) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: pointers must be 16-byte aligned");
@@ -343,8 +345,15 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
     plan->last_layout = L;
     plan->last_n_vis = n_vis;
     plan->last_weights = weights;
+    plan->last_has_values = with_values;
     plan->last_valid = true;
     return WS_OK;
+}
+
+int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+    return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true);
 }
 
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
@@ -355,7 +364,7 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
     if (mode == WS_GRID_SPARSE && !plan->fft_own)
         return fail(plan, WS_ERR_UNSUPPORTED, "ws_grid_binned: WS_GRID_SPARSE needs the own FFT (N = 2^8..2^13, no WS_FLAG_LIBRARY_FFT)");
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: grid must be 16-byte aligned");
-    if (!plan->last_valid || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
+    if (!plan->last_valid || !plan->last_has_values || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: workspace does not hold the bins of ws_bin_visibilities");
     if (mode == WS_GRID_ACCUMULATE && plan->occ_sparse && plan->occ_grid == grid)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written)");
@@ -403,7 +412,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
     return ws_grid_binned(plan, grid, mode, workspace, workspace_bytes, stream);
 }
 
-int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream) {
+static int fft_planes_dir(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream, int direction) {
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_planes: null argument");
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_planes: grid must be 16-byte aligned");
     if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
@@ -417,9 +426,48 @@ int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_b
     const size_t plane = (size_t)plan->prm.n_pix * plan->prm.n_pix;
     for (int k = 0; k < plan->prm.n_wplanes; k += plan->fft_batch) {
         cufftComplex* p = (cufftComplex*)grid + (size_t)k * plane;
-        if (cufftExecC2C(plan->fft, p, p, CUFFT_INVERSE) != CUFFT_SUCCESS)
+        if (cufftExecC2C(plan->fft, p, p, direction) != CUFFT_SUCCESS)
             return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftExecC2C");
     }
+    return WS_OK;
+}
+
+int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream) {
+    return fft_planes_dir(plan, grid, workspace, workspace_bytes, stream, CUFFT_INVERSE);
+}
+
+int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void* workspace, size_t workspace_bytes,
+                      void* stream) {
+    if (!plan || !model_image || !planes) return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_planes: null argument");
+    if (((uintptr_t)model_image | (uintptr_t)planes) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_planes: pointers must be 16-byte aligned");
+    if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
+        return fail(plan, WS_ERR_WORKSPACE, "ws_predict_planes: workspace smaller than ws_fft_workspace_bytes");
+    if (plan->occ_grid == planes) plan->occ_grid = nullptr;      // no longer a mesh the gridder filled
+    const int rc = ws_launch_wscreen_fwd(plan, (const float2*)model_image, (float2*)planes, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_predict_planes: launch failed");
+    plan->launches += rc;
+    return fft_planes_dir(plan, planes, workspace, workspace_bytes, stream, CUFFT_FORWARD);
+}
+
+int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_hz, int64_t n_rows, int32_t n_chan,
+                           const void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
+                           size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!planes || (n_rows > 0 && !vis_out)) return fail(plan, WS_ERR_INVALID_ARG, "ws_degrid_visibilities: null pointer");
+    if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_degrid_visibilities: bad flag");
+    if (((uintptr_t)planes | (uintptr_t)vis_out) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_degrid_visibilities: pointers must be 16-byte aligned");
+    int rc = bin_impl(plan, uvw, nullptr, nullptr, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, false);
+    if (rc != WS_OK) return rc;
+    if (n_rows == 0) return WS_OK;
+    if (!accumulate &&
+        cudaMemsetAsync(vis_out, 0, (size_t)n_rows * n_chan * 8, (cudaStream_t)stream) != cudaSuccess)   // dropped ones predict 0
+        return fail(plan, WS_ERR_CUDA, "ws_degrid_visibilities: memset failed");
+    rc = ws_launch_degrid(plan, plan->last_layout, (char*)workspace, (const float2*)planes, (float2*)vis_out, scale,
+                          accumulate, (cudaStream_t)stream);
+    if (rc < 0) return fail(plan, rc, "ws_degrid_visibilities: launch failed");
+    plan->launches += rc;
     return WS_OK;
 }
 

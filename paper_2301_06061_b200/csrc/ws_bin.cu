@@ -254,8 +254,10 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
     float2 v = make_float2(0.f, 0.f);
     float w = 0.f;
     if (kept) {
-        v = __ldcs(vis + m);
-        w = __ldcs(wt + m);
+        if (vis) {                                  // NULL: bins for the degridder, the records carry positions only
+            v = __ldcs(vis + m);
+            w = __ldcs(wt + m);
+        }
         tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
         lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
         home = bin_of(g, k, ty, tx);

@@ -1,0 +1,230 @@
+// Degridding: model image -> predicted visibilities ("the degridding procedure (transforming from the
+// image to the visibility space)"; Eq. 1 at :59 discretised the way Eq. 2 / Eq. 3 discretise the imaging direction).
+// With unit weights it is the exact adjoint of a1..a4:
+//   D1  Q_k(l, m) = M(l, m) exp(-2 pi i w_k (sqrt(1 - l^2 - m^2) - 1))          k_wscreen_fwd
+//   D2  H_k = forward un-normalised 2-D DFT of Q_k, per plane                     cuFFT (ws_api.cu)
+//   D3  V_m = sum_{a,b} g(a - fu) g(b - fv) H_k[j0 + b][i0 + a]                    k_degrid
+// D3 reuses the bins of ws_bin.cu: the paper expects "the same parallelization strategy" to work, with "a specific
+// implementation ... required by the distribution of the visibilities on the cell back to the single measurements"
+// (:459).  Here a warp owns a tile-plane, stages the tile plus its halo ((T + S - 1)^2 cells) in shared memory once,
+// and each lane then gathers the S x S footprint of one visibility with its taps in registers -- a pure gather, no
+// atomics; the home lists of the bins give each visibility exactly one owner.
+#include "ws_internal.h"
+#include "ws_phase.cuh"
+#include "ws_taps.cuh"
+
+namespace {
+
+constexpr int T = WS_TILE;
+constexpr int G = WS_WC_GROUP;
+
+// ---- D1: the N_w screened copies of the model image, FFT-native storage order -------------------------------
+// A thread owns two adjacent pixels; the phases over the planes are a geometric sequence, advanced by one complex
+// multiply per plane inside a block of G planes and restarted from an exactly reduced (fp64) phase per block.
+__global__ void __launch_bounds__(256)
+k_wscreen_fwd(const __grid_constant__ WcParams prm, const float4* __restrict__ image, float4* __restrict__ planes) {
+    const uint32_t N = (uint32_t)prm.n_pix, halfN = N >> 1, pairs = N >> 1;
+    const uint64_t tid = (uint64_t)blockIdx.x * 256u + threadIdx.x;
+    if (tid >= (uint64_t)N * pairs) return;
+    const uint32_t q = (uint32_t)(tid / pairs), p = (uint32_t)(tid - (uint64_t)q * pairs) * 2u;
+    const uint32_t sq = q >= halfN ? q - halfN : q + halfN;
+    const uint32_t sp = p >= halfN ? p - halfN : p + halfN;
+    const size_t plane_stride = (size_t)N * pairs;                 // in float4 units
+    float4* dst = planes + (size_t)sq * pairs + (sp >> 1);
+    float4 m = __ldcs(image + tid);
+    bool inA, inB;
+    const double tA = ws_n_minus_1(prm, (int)q, (int)p, &inA), tB = ws_n_minus_1(prm, (int)q, (int)p + 1, &inB);
+    if (!inA) m.x = m.y = 0.f;                                      // R14
+    if (!inB) m.z = m.w = 0.f;
+    const float2 rA = ws_expi_turns(-prm.dw * tA), rB = ws_expi_turns(-prm.dw * tB);
+    const int nw = prm.n_wplanes;
+    for (int lo = 0; lo < nw; lo += G) {
+        const double wk = prm.w0 + (double)lo * prm.dw;
+        float2 eA = ws_expi_turns(-wk * tA), eB = ws_expi_turns(-wk * tB);
+#pragma unroll
+        for (int j = 0; j < G; ++j) {
+            if (lo + j < nw) {
+                const float2 a = ws_cmul(make_float2(m.x, m.y), eA), b = ws_cmul(make_float2(m.z, m.w), eB);
+                __stcs(dst + (size_t)(lo + j) * plane_stride, make_float4(a.x, a.y, b.x, b.y));
+                eA = ws_cmul(eA, rA);
+                eB = ws_cmul(eB, rB);
+            }
+        }
+    }
+}
+
+// ---- D3: the gather ------------------------------------------------------------------------------------------
+template <int S>
+struct DgCfg {
+    static constexpr int H = (S - 1) / 2;
+    static constexpr int W = T + 2 * H;             // side of the staged region: the tile and its halo
+    static constexpr int P = W | 1;                 // odd row pitch (in cells)
+    static constexpr size_t WARP_BYTES = ((size_t)W * P * sizeof(float2) + 15) / 16 * 16;
+    static constexpr int WARPS = (113 * 1024) / WARP_BYTES >= 8 ? 8 : (int)((113 * 1024) / WARP_BYTES);
+    static constexpr int THREADS = WARPS * 32;
+};
+
+// Stages logical cells [x0 - H, x0 + T + H) x [y0 - H, y0 + T + H) of plane k (cells off the mesh: 0; no kept
+// visibility reads them, drop rule O3).
+template <int S>
+__device__ __forceinline__ void load_region(const WsGeom& g, const float2* __restrict__ planes, uint32_t bin, float2* region,
+                                            int lane) {
+    using C = DgCfg<S>;
+    const uint32_t nt = (uint32_t)g.nt;
+    const uint32_t tx = bin % nt, r = bin / nt;
+    const uint32_t ty = r % nt, k = r / nt;
+    const int N = g.n_pix, half = N >> 1;
+    const int x0 = (int)tx * T - C::H, y0 = (int)ty * T - C::H;
+    const float2* plane = planes + (size_t)k * (size_t)N * (size_t)N;
+    for (int ry = 0; ry < C::W; ++ry) {
+        const int ly = y0 + ry;
+        const bool oky = (unsigned)ly < (unsigned)N;
+        const int sy = ly >= half ? ly - half : ly + half;
+        for (int rx = lane; rx < C::W; rx += 32) {
+            const int lx = x0 + rx;
+            float2 v = make_float2(0.f, 0.f);
+            if (oky && (unsigned)lx < (unsigned)N) {
+                const int sx = lx >= half ? lx - half : lx + half;
+                v = __ldg(plane + (size_t)sy * N + sx);
+            }
+            region[ry * C::P + rx] = v;
+        }
+    }
+    __syncwarp();
+}
+
+// Home records [lo, hi) (perm slots) of one bin, whose records start `hs` after their perm slots.
+template <int S, bool KB>
+__device__ __forceinline__ void gather(const WsGeom& g, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
+                                       uint32_t lo, uint32_t hi, uint32_t hs, const float2* region, float2* __restrict__ vis_out,
+                                       float scale, int accumulate, int lane) {
+    using C = DgCfg<S>;
+    for (uint32_t slot = lo + lane; slot < hi; slot += 32) {
+        const float4 rec = __ldcs(records + slot + hs);
+        const uint32_t X = __float_as_uint(rec.x), Y = __float_as_uint(rec.y);
+        const int cx = (int)X >> 24, cy = (int)Y >> 24;            // centre cell in the tile frame = first footprint cell in the region
+        const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
+        const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
+        float gu[S], gv[S];
+        eval_taps<S, KB>(g, fx, fy, gu, gv);
+        const float2* base = region + cy * C::P + cx;
+        float ar = 0.f, ai = 0.f;
+#pragma unroll
+        for (int b = 0; b < S; ++b) {
+            float rr = 0.f, ri = 0.f;
+#pragma unroll
+            for (int a = 0; a < S; ++a) {
+                const float2 c = base[b * C::P + a];
+                rr = fmaf(gu[a], c.x, rr);
+                ri = fmaf(gu[a], c.y, ri);
+            }
+            ar = fmaf(gv[b], rr, ar);
+            ai = fmaf(gv[b], ri, ai);
+        }
+        const float f = scale * g.norm2;
+        float2 out = make_float2(ar * f, ai * f);
+        const uint32_t m = __ldcs(perm + slot);
+        if (accumulate) {
+            const float2 old = vis_out[m];
+            out.x += old.x;
+            out.y += old.y;
+        }
+        vis_out[m] = out;
+    }
+    __syncwarp();
+}
+
+// Persistent kernel: warp w takes bins w, w + W, ... and the chunks of the heavy bins (items), interleaved.
+template <int S, bool KB>
+__global__ void __launch_bounds__(DgCfg<S>::THREADS, 2)
+k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
+         const uint4* __restrict__ items, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
+         const float2* __restrict__ planes, float2* __restrict__ vis_out, float scale, int accumulate,
+         const WsStatus* __restrict__ status) {
+    using C = DgCfg<S>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    float2* region = (float2*)(smem_raw + (size_t)wid * C::WARP_BYTES);
+    if (status->overflow) return;
+    const uint32_t n_items = status->n_items;
+    const uint32_t n_warps = gridDim.x * C::WARPS;
+    const uint32_t gw = blockIdx.x * C::WARPS + wid;
+    const uint32_t my_tiles = gw < g.n_bins ? (g.n_bins - gw + n_warps - 1) / n_warps : 0u;
+    const uint32_t my_items = gw < n_items ? (n_items - gw + n_warps - 1) / n_warps : 0u;
+    const uint32_t gap = my_items ? max(1u, my_tiles / my_items) : 0xFFFFFFFFu;
+    uint32_t it = gw, since = 0;
+
+    auto do_item = [&]() {
+        const uint4 w = items[it];
+        it += n_warps;
+        load_region<S>(g, planes, w.x, region, lane);
+        gather<S, KB>(g, records, perm, w.y, w.z, halo_start[w.x], region, vis_out, scale, accumulate, lane);
+    };
+
+    for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
+        if (it < n_items && since >= gap) {
+            do_item();
+            since = 0;
+        }
+        ++since;
+        const uint32_t s = bin_start[bin], e = bin_start[bin + 1];
+        if (s == e || e - s > WS_CHUNK) continue;           // empty, or heavy: its chunks are items
+        load_region<S>(g, planes, bin, region, lane);
+        gather<S, KB>(g, records, perm, s, e, halo_start[bin], region, vis_out, scale, accumulate, lane);
+    }
+    while (it < n_items) do_item();
+}
+
+template <int S, bool KB>
+int launch_s(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale, int accumulate,
+             cudaStream_t st) {
+    using C = DgCfg<S>;
+    const size_t smem = C::WARP_BYTES * C::WARPS;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_degrid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return WS_ERR_CUDA;
+        attr_set = true;
+    }
+    const uint32_t* bin_start = (const uint32_t*)(ws + L.off_counts_home);
+    const uint32_t* halo_start = (const uint32_t*)(ws + L.off_counts_halo);
+    uint4* items = (uint4*)(ws + L.off_items);
+    int rc = ws_launch_items(plan, bin_start, items, L.item_capacity, st);
+    if (rc < 0) return rc;
+    k_degrid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(plan->geom, bin_start, halo_start, items,
+                                                                  (const float4*)(ws + L.off_records),
+                                                                  (const uint32_t*)(ws + L.off_perm), planes, vis_out, scale,
+                                                                  accumulate, plan->d_status);
+    if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+    return rc + 1;
+}
+
+}  // namespace
+
+int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, cudaStream_t st) {
+    const ws_params& P = plan->prm;
+    WcParams prm;
+    prm.n_pix = P.n_pix;
+    prm.n_wplanes = P.n_wplanes;
+    prm.cell = P.cell_rad;
+    prm.dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
+    prm.w0 = P.w_min + 0.5 * prm.dw;
+    const uint64_t n_pairs = (uint64_t)P.n_pix * (uint64_t)(P.n_pix / 2);
+    k_wscreen_fwd<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(prm, (const float4*)image, (float4*)planes);
+    if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+    return 1;
+}
+
+int ws_launch_degrid(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale,
+                     int accumulate, cudaStream_t st) {
+    const bool kb = plan->geom.kb_terms > 0;
+#define WS_DG_CASE(S_)                                                                                        \
+    case S_:                                                                                                  \
+        return kb ? launch_s<S_, true>(plan, L, ws, planes, vis_out, scale, accumulate, st)                   \
+                  : launch_s<S_, false>(plan, L, ws, planes, vis_out, scale, accumulate, st);
+    switch (plan->geom.support) {
+        WS_DG_CASE(1) WS_DG_CASE(3) WS_DG_CASE(5) WS_DG_CASE(7) WS_DG_CASE(9) WS_DG_CASE(11) WS_DG_CASE(13) WS_DG_CASE(15)
+    }
+#undef WS_DG_CASE
+    return WS_ERR_UNSUPPORTED;
+}

@@ -18,16 +18,11 @@
 //     persistent kernel so that the store stream of the (mostly empty) tiles overlaps the arithmetic of the
 //     dense ones.
 #include "ws_internal.h"
+#include "ws_taps.cuh"
 
 namespace {
 
 constexpr int T = WS_TILE;
-
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 template <int S>
 struct TileCfg {
@@ -80,43 +75,6 @@ struct WarpSmem {
     }
 };
 
-// The 2 S taps of one record: gu[i] = g(i - h - fx) / norm1, gv likewise (norm1^2 is folded into weight * vis).
-template <int S, bool KB>
-__device__ __forceinline__ void eval_taps(const WsGeom& g, float fx, float fy, float* gu, float* gv) {
-    constexpr int H = (S - 1) / 2;
-    if constexpr (!KB) {
-        const float tap_c = g.tap_c;
-#pragma unroll
-        for (int i = 0; i < S; ++i) {
-            const float dx = (float)(i - H) - fx, dy = (float)(i - H) - fy;
-            gu[i] = ex2_approx(tap_c * dx * dx);
-            gv[i] = ex2_approx(tap_c * dy * dy);
-        }
-    } else {
-        // I0(beta sqrt(y)) / I0(beta) = sum_k c_k y^k, y = 1 - (2x/S)^2 in [0, 1], c_k > 0: Horner without cancellation
-        float yu[S], yv[S];
-        const float ky = g.kb_y;
-#pragma unroll
-        for (int i = 0; i < S; ++i) {
-            const float dx = (float)(i - H) - fx, dy = (float)(i - H) - fy;
-            yu[i] = fmaxf(fmaf(-ky * dx, dx, 1.0f), 0.0f);
-            yv[i] = fmaxf(fmaf(-ky * dy, dy, 1.0f), 0.0f);
-        }
-        int k = g.kb_terms - 1;
-        const float top = g.kb_c[k];
-#pragma unroll
-        for (int i = 0; i < S; ++i) gu[i] = gv[i] = top;
-        for (--k; k >= 0; --k) {
-            const float c = g.kb_c[k];
-#pragma unroll
-            for (int i = 0; i < S; ++i) {
-                gu[i] = fmaf(gu[i], yu[i], c);
-                gv[i] = fmaf(gv[i], yv[i], c);
-            }
-        }
-    }
-}
-
 // Accumulates records [lo, hi) into the warp's shared tile.
 template <int S, bool KB>
 __device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
@@ -134,12 +92,22 @@ __device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __rest
             const int cxp = ((int)X >> 24) - C::H, cyp = ((int)Y >> 24) - C::H;   // footprint's first cell, tile frame
             const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
             const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
-            float gu[S], gv[S];
-            eval_taps<S, KB>(g, fx, fy, gu, gv);
+            if constexpr (!KB) {
+                const float tap_c = g.tap_c;
 #pragma unroll
-            for (int i = 0; i < S; ++i) {
-                sm.gu[lane * S + i] = gu[i];
-                sm.gv[lane * S + i] = gv[i];
+                for (int i = 0; i < S; ++i) {
+                    const float dx = (float)(i - C::H) - fx, dy = (float)(i - C::H) - fy;
+                    sm.gu[lane * S + i] = ex2_approx(tap_c * dx * dx);
+                    sm.gv[lane * S + i] = ex2_approx(tap_c * dy * dy);
+                }
+            } else {
+                float gu[S], gv[S];
+                eval_taps<S, true>(g, fx, fy, gu, gv);
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    sm.gu[lane * S + i] = gu[i];
+                    sm.gv[lane * S + i] = gv[i];
+                }
             }
             sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cxp & 0xFFFF) | (cyp << 16)),
                                         __int_as_float(cyp * C::P + cxp));
@@ -320,6 +288,16 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 }
 
 }  // namespace
+
+// Work items for the lists of `starts` ([n_bins + 1] offsets) longer than WS_CHUNK: used by the degridder on the home lists.
+int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st) {
+    const WsGeom& g = plan->geom;
+    if (cudaMemsetAsync(&plan->d_status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, items, item_capacity, plan->d_status, nullptr,
+                                                          WS_GRID_ACCUMULATE, nullptr);
+    if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+    return 1;
+}
 
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
     const bool kb = plan->geom.kb_terms > 0;

@@ -85,6 +85,7 @@ struct ws_plan {
     double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)
     float* d_taper;                             // plan-owned [N]: 1 / ghat((p - N/2)/N), fp64-computed on the host
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
+    bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
     bool occ_sparse;                            // ... and it was written by WS_GRID_SPARSE (private layout, empty tiles unwritten)
 };
@@ -95,6 +96,10 @@ static inline size_t ws_align_up(size_t x, size_t a) { return (x + a - 1) / a * 
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);
+int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st);
+int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, cudaStream_t st);
+int ws_launch_degrid(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale,
+                     int accumulate, cudaStream_t st);
 int ws_launch_sorted_keys(ws_plan* plan, const WsLayout& L, char* ws, cudaStream_t st);
 int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
                        cudaStream_t st);

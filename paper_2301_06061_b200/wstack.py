@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count",
 ]
 
@@ -81,6 +81,8 @@ def lib():
         "ws_get_occupancy": (C.c_int, [vp] + [C.POINTER(C.c_double)] * 4 + [C.POINTER(i32), vp]),
         "ws_dirty_image": (C.c_int, [vp, vp, vp, u32, vp]),
         "ws_get_sum_weights": (C.c_int, [vp, C.POINTER(C.c_double), vp]),
+        "ws_predict_planes": (C.c_int, [vp, vp, vp, vp, sz, vp]),
+        "ws_degrid_visibilities": (C.c_int, [vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
                                   C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
@@ -245,6 +247,23 @@ class Plan:
     def dirty_image(self, image, dirty, norm_flags: int = 0, stream=None):
         self._check(lib().ws_dirty_image(self._h, _dev(image, torch.complex64, "image"),
                                          _dev(dirty, torch.float32, "dirty"), norm_flags, _stream(stream)))
+
+    def predict_planes(self, model_image, planes, workspace, stream=None):
+        """Degridding steps 1-2: planes[k] = forward FFT of model_image x exp(-2 pi i w_k (n - 1))."""
+        self._check(lib().ws_predict_planes(self._h, _dev(model_image, torch.complex64, "model_image"),
+                                            _dev(planes, torch.complex64, "planes"),
+                                            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def degrid_visibilities(self, uvw, freq_hz, n_chan: int, planes, vis_out, workspace, scale: float = 1.0,
+                            accumulate: bool = False, stream=None):
+        """Degridding step 3: vis_out (+)= scale x the footprint sums of `planes` at every visibility position."""
+        n_rows = int(uvw.shape[0])
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_degrid_visibilities(
+            self._h, _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan, _dev(planes, torch.complex64, "planes"),
+            _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+        self._ws = workspace
 
     def sum_weights(self, stream=None) -> float:
         v = C.c_double()
