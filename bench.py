@@ -150,6 +150,7 @@ def main():
     ap.add_argument("--kernel", default="gaussian", choices=["gaussian", "kb"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-degrid", action="store_true")
     args = ap.parse_args()
     global KERNEL
     KERNEL = args.kernel
@@ -267,6 +268,29 @@ def main():
         m = np.median(np.array(rows), axis=0)
         lib_ms = {"grid_overwrite": float(m[0]), "fft_cufft": float(m[1]), "wcorrect_standalone": float(m[2])}
 
+    # ---- degridding on the same positions, outside the timed region: model image -> planes
+    # (forward w-screen + cuFFT), then bins + footprint gather
+    degrid_ms = None
+    if not args.no_degrid:
+        model = torch.randn((d.n_pix, d.n_pix), dtype=torch.complex64, device=f"cuda:{local_rank}")
+        pred = torch.empty_like(d.vis)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        rows = []
+        for _ in range(4):
+            e[0].record()
+            plan.predict_planes(model, grid, wsp)
+            e[1].record()
+            plan.degrid_visibilities(d.uvw, d.freqs_hz, d.n_chan, grid, pred, wsp)
+            e[2].record()
+            torch.cuda.synchronize()
+            rows.append([e[i].elapsed_time(e[i + 1]) for i in range(2)])
+        plan.async_status()
+        m = np.median(np.array(rows[1:]), axis=0)
+        degrid_ms = {"predict_planes_wscreen_cufft": float(m[0]), "bin_and_gather": float(m[1]),
+                     "mvis_per_s_degridding": d.n_vis / (m[1] * 1e-3) / 1e6,
+                     "mvis_per_s_whole_prediction": d.n_vis / ((m[0] + m[1]) * 1e-3) / 1e6}
+        del model, pred
+
     # ---- roofline of the dominant own kernel -----------------------------------------
     peak, peak_src = peaks()
     mesh_b = 8.0 * d.n_pix ** 2 * d.n_wplanes
@@ -317,7 +341,7 @@ def main():
            "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
            "stages_ms_median": {n: float(v) for n, v in zip(stage_names, med)},
            "fft": "own two-pass FFT with fused w-correction, occupancy-aware" if own else "cuFFT",
-           "library_path_ms": lib_ms, "occupancy": occ,
+           "library_path_ms": lib_ms, "degridding_ms": degrid_ms, "occupancy": occ,
            "mvis_per_s_gridding": d.n_vis / ((med[0] + med[1]) * 1e-3) / 1e6,
            "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
            "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "kernels": per_kernel,
