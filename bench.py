@@ -310,11 +310,14 @@ def main():
         alg = {"k_grid_tiles": mesh_b + 16.0 * n_records, "k_wcorrect": mesh_b + 12.0 * N * N}
         times = {"k_grid_tiles": med[1], "k_wcorrect": med[3]}
         flops = {}
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures of this command
+    # (profiles/r1m_large_ncu.md) -- Large, Gaussian only
+    ncu_traffic = {"k_fft_rows_wcorrect": 13.967e9 + 1.113e9, "k_fft_columns": (1.437e9 + 11.106e9) + (10.838e9 + 13.589e9)} if (cfg.name == "large" and KERNEL == "gaussian" and own) else {}
     dom = max(times, key=times.get)
     ach = alg[dom] / (times[dom] * 1e-3) / 1e9
     hbm_frac = ach / peak
     roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": hbm_frac,
-            "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
+            "traffic": ncu_traffic.get(dom), "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
             "launch_ms": float(times[dom])}
     if dom in flops:
         # fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x max SM clock (B200_PROFILING.md unit counts and clocks)
@@ -322,11 +325,12 @@ def main():
         tf = flops[dom] / (times[dom] * 1e-3) / 1e12
         if tf / alu_peak > hbm_frac:
             roof = {"bound": "alu", "kernel": dom, "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
-                    "traffic": None, "peak_source": "148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (guide's unit counts and clocks)",
+                    "traffic": ncu_traffic.get(dom), "peak_source": "148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (guide's unit counts and clocks)",
                     "nominal_flops_per_launch": flops[dom], "launch_ms": float(times[dom]),
                     "hbm_view": {"achieved": ach, "peak": peak, "frac": hbm_frac, "algorithmic_bytes_per_launch": alg[dom]}}
     per_kernel = {k: {"ms": float(times[k]), "alg_GB": alg[k] / 1e9, "GBps": alg[k] / (times[k] * 1e-3) / 1e9,
-                      "frac_of_hbm_peak": alg[k] / (times[k] * 1e-3) / 1e9 / peak} for k in times}
+                      "frac_of_hbm_peak": alg[k] / (times[k] * 1e-3) / 1e9 / peak,
+                      "ncu_dram_GB": ncu_traffic[k] / 1e9 if k in ncu_traffic else None} for k in times}
     # B_alg(path) counts every plane cell written once and read once; the sparse path moves less
     b_path = 12.0 * d.n_rows + 12.0 * d.n_vis + 2 * mesh_b + 8.0 * N * N
     t_path = med[0] + med[1] + (lib_ms["wcorrect_standalone"] if lib_ms else med[3])
