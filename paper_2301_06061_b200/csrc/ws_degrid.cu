@@ -76,19 +76,16 @@ __device__ __forceinline__ void load_region(const WsGeom& g, const float2* __res
     const int N = g.n_pix, half = N >> 1;
     const int x0 = (int)tx * T - C::H, y0 = (int)ty * T - C::H;
     const float2* plane = planes + (size_t)k * (size_t)N * (size_t)N;
-    for (int ry = 0; ry < C::W; ++ry) {
-        const int ly = y0 + ry;
-        const bool oky = (unsigned)ly < (unsigned)N;
-        const int sy = ly >= half ? ly - half : ly + half;
-        for (int rx = lane; rx < C::W; rx += 32) {
-            const int lx = x0 + rx;
-            float2 v = make_float2(0.f, 0.f);
-            if (oky && (unsigned)lx < (unsigned)N) {
-                const int sx = lx >= half ? lx - half : lx + half;
-                v = __ldg(plane + (size_t)sy * N + sx);
-            }
-            region[ry * C::P + rx] = v;
+#pragma unroll 8
+    for (int idx = lane; idx < C::W * C::W; idx += 32) {     // independent loads: eight in flight per lane
+        const int ry = idx / C::W, rx = idx - ry * C::W;
+        const int ly = y0 + ry, lx = x0 + rx;
+        float2 v = make_float2(0.f, 0.f);
+        if ((unsigned)ly < (unsigned)N && (unsigned)lx < (unsigned)N) {
+            const int sy = ly >= half ? ly - half : ly + half, sx = lx >= half ? lx - half : lx + half;
+            v = __ldg(plane + (size_t)sy * N + sx);
         }
+        region[ry * C::P + rx] = v;
     }
     __syncwarp();
 }
@@ -99,8 +96,19 @@ __device__ __forceinline__ void gather(const WsGeom& g, const float4* __restrict
                                        uint32_t lo, uint32_t hi, uint32_t hs, const float2* region, float2* __restrict__ vis_out,
                                        float scale, int accumulate, int lane) {
     using C = DgCfg<S>;
+    float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
+    uint32_t m_nxt = 0;
+    if (lo + lane < hi) {
+        nxt = __ldcs(records + lo + lane + hs);
+        m_nxt = __ldcs(perm + lo + lane);
+    }
     for (uint32_t slot = lo + lane; slot < hi; slot += 32) {
-        const float4 rec = __ldcs(records + slot + hs);
+        const float4 rec = nxt;
+        const uint32_t m = m_nxt;
+        if (slot + 32 < hi) {                                       // next batch in flight while this one gathers
+            nxt = __ldcs(records + slot + 32 + hs);
+            m_nxt = __ldcs(perm + slot + 32);
+        }
         const uint32_t X = __float_as_uint(rec.x), Y = __float_as_uint(rec.y);
         const int cx = (int)X >> 24, cy = (int)Y >> 24;            // centre cell in the tile frame = first footprint cell in the region
         const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
@@ -123,7 +131,6 @@ __device__ __forceinline__ void gather(const WsGeom& g, const float4* __restrict
         }
         const float f = scale * g.norm2;
         float2 out = make_float2(ar * f, ai * f);
-        const uint32_t m = __ldcs(perm + slot);
         if (accumulate) {
             const float2 old = vis_out[m];
             out.x += old.x;
