@@ -516,6 +516,63 @@ void orc_degrid(const orc_params *p, const float *uvw, const double *freq_hz, in
     free(su); free(sw);
 }
 
+/* The degridding chain at single visibilities for a SPARSE model (n_src non-zero pixels (sq, sp) with values sval):   */
+/* V_m = sum_s val_s e^{-2 pi i w_k t_s} [sum_a gu[a] e^{-2 pi i (i0+a-N/2)(p_s-N/2)/N}] [sum_b gv[b] e^{-2 pi i (j0+b-N/2)(q_s-N/2)/N}] */
+/* i.e. steps 1-3 with the finite sums re-ordered (visibility outermost); no plane is formed.  Used at sizes where the   */
+/* fp64 plane stack cannot be transformed in reasonable time; pinned against the chain.  samp: flat indices row*n_chan+c. */
+void orc_predict_samples(const orc_params *p, const float *uvw, const double *freq_hz, int32_t n_chan,
+                         int32_t n_src, const int32_t *sq, const int32_t *sp, const double *sval,
+                         int64_t n_samp, const int64_t *samp, double *out) {
+    const int N = p->n_pix, S = p->support, h = (S - 1) / 2, Nw = p->n_wplanes;
+    const double dw = (p->w_max - p->w_min) / (double)Nw;
+    double *su = malloc(sizeof(double) * n_chan), *sw = malloc(sizeof(double) * n_chan), ow;
+    orc_channel_constants(p, freq_hz, n_chan, su, sw, &ow);
+    double *E = malloc(sizeof(double) * 2 * (size_t)N);       /* E[m] = exp(-2 pi i m / N) */
+    for (int m = 0; m < N; ++m) {
+        E[2 * m] = cos(2.0 * ORC_PI * (double)m / (double)N);
+        E[2 * m + 1] = -sin(2.0 * ORC_PI * (double)m / (double)N);
+    }
+    double *ts = malloc(sizeof(double) * n_src);              /* n - 1 per source pixel; NaN marks r^2 >= 1 */
+    for (int s = 0; s < n_src; ++s) {
+        double l = (double)(sp[s] - N / 2) * p->cell_rad, m = (double)(sq[s] - N / 2) * p->cell_rad;
+        double r2 = l * l + m * m;
+        ts[s] = r2 < 1.0 ? -r2 / (1.0 + sqrt(1.0 - r2)) : NAN;
+    }
+#pragma omp parallel for
+    for (int64_t n = 0; n < n_samp; ++n) {
+        double gu[32], gv[32];
+        int64_t r = samp[n] / n_chan; int c = (int)(samp[n] % n_chan);
+        int32_t i0, j0, k; double fu, fv;
+        out[2 * n] = 0.0; out[2 * n + 1] = 0.0;
+        if (!orc_place(p, (double)uvw[3 * r], (double)uvw[3 * r + 1], (double)uvw[3 * r + 2], su[c], sw[c], ow,
+                       &i0, &j0, &k, &fu, &fv)) continue;
+        for (int a = -h; a <= h; ++a) {
+            gu[a + h] = orc_kernel1d(p, (double)a - fu);
+            gv[a + h] = orc_kernel1d(p, (double)a - fv);
+        }
+        const double wk = p->w_min + ((double)k + 0.5) * dw;
+        double vr = 0.0, vi = 0.0;
+        for (int s = 0; s < n_src; ++s) {
+            if (isnan(ts[s])) continue;
+            double xr = 0, xi = 0, yr = 0, yi = 0;
+            for (int a = -h; a <= h; ++a) {
+                int64_t mx = (((int64_t)(i0 + a) - N / 2) * ((int64_t)sp[s] - N / 2)) % N; if (mx < 0) mx += N;
+                int64_t my = (((int64_t)(j0 + a) - N / 2) * ((int64_t)sq[s] - N / 2)) % N; if (my < 0) my += N;
+                xr += gu[a + h] * E[2 * mx]; xi += gu[a + h] * E[2 * mx + 1];
+                yr += gv[a + h] * E[2 * my]; yi += gv[a + h] * E[2 * my + 1];
+            }
+            double fr = xr * yr - xi * yi, fi = xr * yi + xi * yr;
+            double ph = -2.0 * ORC_PI * wk * ts[s];
+            double cr = cos(ph), ci = sin(ph);
+            double gr = fr * cr - fi * ci, gi = fr * ci + fi * cr;
+            vr += sval[2 * s] * gr - sval[2 * s + 1] * gi;
+            vi += sval[2 * s] * gi + sval[2 * s + 1] * gr;
+        }
+        out[2 * n] = vr; out[2 * n + 1] = vi;
+    }
+    free(su); free(sw); free(E); free(ts);
+}
+
 /* ---- normalisation of the image (Eq. 2 solved for I; readings R12, R29) ------------------- */
 /* Sum of the weights of the kept visibilities (O3), in input order.                             */
 double orc_sum_weights(const orc_params *p, const float *uvw, const float *wt, const double *freq_hz,

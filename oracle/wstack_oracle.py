@@ -230,6 +230,21 @@ def predict(prm: OracleParams, model: np.ndarray, uvw, n_chan: int, freq=None, r
     return (V, np.stack(stack)) if return_planes else V
 
 
+def predict_samples(prm: OracleParams, uvw, n_chan: int, freq, src_q, src_p, src_val, samples) -> np.ndarray:
+    """The degridding chain at the visibilities `samples` (flat indices row * n_chan + c) for a sparse model image
+    (pixels (src_q, src_p) with complex values src_val), visibility-outermost; complex128 [n_samples]."""
+    uvw, _, _, fr = _inputs(uvw, freq=freq)
+    sq = np.ascontiguousarray(src_q, dtype=np.int32)
+    sp = np.ascontiguousarray(src_p, dtype=np.int32)
+    sv = np.ascontiguousarray(src_val, dtype=np.complex128)
+    samp = np.ascontiguousarray(samples, dtype=np.int64)
+    out = np.empty(samp.size, np.complex128)
+    lib().orc_predict_samples(C.byref(prm.c()), _p(uvw, C.c_float), _p(fr, C.c_double), C.c_int32(n_chan),
+                              C.c_int32(sq.size), _p(sq, C.c_int32), _p(sp, C.c_int32), _p(sv.view(np.float64), C.c_double),
+                              C.c_int64(samp.size), _p(samp, C.c_int64), _p(out.view(np.float64), C.c_double))
+    return out
+
+
 def image_samples(prm: OracleParams, uvw, vis, wt, freq, q: Sequence[int], p: Sequence[int]) -> np.ndarray:
     """The whole chain at pixels (q[s], p[s]), visibility-outermost; complex128 [n_samp]."""
     uvw, vis, wt, fr = _inputs(uvw, vis, wt, freq)

@@ -88,3 +88,24 @@ def test_predicted_visibilities_of_point_sources_equal_eq1(oracle, kernel, tol):
         ref += f * np.exp(-2j * np.pi * (u64[:, 0] * l + u64[:, 1] * m + wk * (math.sqrt(1 - l * l - m * m) - 1)))
     err = np.abs(pred - ref).max() / sum(f for _, _, f in src)
     assert err < tol, err
+
+
+def test_predict_samples_equal_the_chain(oracle):
+    """The sampled, re-ordered form used at full size against the plane-by-plane chain, both kernels, with drops."""
+    d = _small(seed=85, n_rows=300, n_chan=3, n_pix=128, n_w=6, wavelengths=False, fill=1.04, w_span=30.0, cell_rad=0.012)
+    rng = np.random.default_rng(2)
+    N = d.n_pix
+    sq, sp = rng.integers(0, N, 25), rng.integers(0, N, 25)
+    sq[:2], sp[:2] = [0, 64], [0, 64]                     # a corner outside the unit circle (ignored), the centre
+    val = rng.standard_normal(25) + 1j * rng.standard_normal(25)
+    M = np.zeros((N, N), np.complex128)
+    np.add.at(M, (sq, sp), val)
+    for kt, par in ((0, 1.0), (KB, _kb_beta(7))):
+        prm = _prm(oracle, d, kernel_type=kt)
+        prm.sigma = par
+        full = oracle.predict(prm, M, d.uvw.numpy(), d.n_chan, d.freqs_hz).ravel()
+        samp = rng.choice(full.size, 200, replace=False)
+        # duplicate source pixels add up in M: give predict_samples the same list
+        got = oracle.predict_samples(prm, d.uvw.numpy(), d.n_chan, d.freqs_hz, sq, sp, val, samp)
+        assert np.abs(got - full[samp]).max() <= 1e-11 * np.abs(full).max()
+        assert (0.012 * 64) ** 2 * 2 >= 1 and np.any(full[samp] == 0)      # the corner is outside; some samples are dropped
