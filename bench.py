@@ -179,13 +179,19 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
 
     d = make_dataset(cfg, device=f"cuda:{local_rank}")
+    # the paper's narrow-band mode (shared uvw): sum the channels of a row first, bin rows
+    presum = d.freqs_hz is None and d.n_chan > 1
+    flags = ws.WS_FLAG_PRESUM_CHANNELS if presum else 0
+    if presum:
+        args.no_degrid = True
     if KERNEL == "kb":
-        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, device=local_rank,
+        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, device=local_rank, flags=flags,
                        kernel_type=ws.WS_KERNEL_KAISER_BESSEL, kernel_param=kb_beta(d.support))
     else:
-        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank)
+        plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank,
+                       flags=flags)
     grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
-    wsp = plan.alloc_workspace(d.n_vis)
+    wsp = plan.alloc_workspace(d.n_rows if presum else d.n_vis)
 
     own = plan.fft_is_own
     OCC = ws.WS_FFT_USE_OCCUPANCY
@@ -348,6 +354,8 @@ def main():
            "library_path_ms": lib_ms, "degridding_ms": degrid_ms, "occupancy": occ,
            "mvis_per_s_gridding": d.n_vis / ((med[0] + med[1]) * 1e-3) / 1e6,
            "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
+           "ggpas_bin_and_grid": d.n_vis * d.support ** 2 / ((med[0] + med[1]) * 1e-3) / 1e9,
+           "presummed_channels": bool(presum),
            "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "kernels": per_kernel,
            "roofline_path": roof_path}
 

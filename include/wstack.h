@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 130
+#define WS_VERSION 140
 
 /* error codes */
 #define WS_OK 0
@@ -68,6 +68,13 @@ extern "C" {
 #define WS_FLAG_TRACK_SUMWT 4u  /* every gridding call also sums the weights of the visibilities it kept (one extra
                                    reduction kernel); needed by WS_NORM_SUMWT.  The sum restarts with ws_grid_zero and
                                    with an OVERWRITE / SPARSE call and grows with ACCUMULATE calls */
+
+#define WS_FLAG_PRESUM_CHANNELS 8u /* the paper's narrow-band mode at scale (one thread grids "all frequencies and
+                                     polarisations" of a measurement): with freq_hz == NULL the n_chan visibilities of a row
+                                     share one position, so sum_c weight * vis is formed per row first (one streaming pass)
+                                     and ROWS are binned and gridded: n_chan times fewer records.  The bins ws_get_bins
+                                     exports are then per row (n_vis = n_rows).  Ignored by ws_degrid_visibilities; a
+                                     gridding call with freq_hz != NULL on such a plan is WS_ERR_INVALID_ARG */
 
 /* kernel_type: the separable 1-D convolution function g(x), x in cells, unit integral (R2, R28) */
 #define WS_KERNEL_GAUSSIAN 0      /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)), kernel_param = sigma */
@@ -111,7 +118,7 @@ size_t ws_dirty_bytes(const ws_plan* plan);  /* 4 N^2     */
 /* Workspace that is always enough for ws_grid_visibilities with up to max_vis_per_call visibilities
  * (worst-case halo duplication) and for ws_fft_planes.  A smaller workspace may be passed: the record
  * capacity is then what fits, and exceeding it is reported by ws_async_status as WS_ERR_WORKSPACE. */
-size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis_per_call);
+size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis_per_call);   /* WS_FLAG_PRESUM_CHANNELS: count ROWS */
 /* The least workspace ws_grid_visibilities accepts for max_vis_per_call visibilities when at most
  * `dup_factor` records per visibility are stored (1.0 .. 4.0; typical data needs (1 + (S-1)/T)^2). */
 size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis_per_call, double dup_factor);

@@ -26,7 +26,7 @@ int cuda_fail(ws_plan* plan, cudaError_t e, const char* where) {
 }
 
 // Workspace layout for n_vis visibilities and a record capacity.  The two histograms at the head are cleared per call.
-WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) {
+WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity, int64_t presum_rows = 0) {
     WsLayout L;
     const size_t nb = plan->geom.n_bins;
     const size_t A = 256;
@@ -43,6 +43,7 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) 
     L.off_sorted_keys = take((size_t)n_vis * 4);
     L.rec_capacity = rec_capacity;
     L.item_capacity = (uint32_t)(2 * rec_capacity / WS_CHUNK + 2);   // sum of ceil(cnt/CHUNK) over bins with cnt > CHUNK
+    L.off_presum = take((size_t)presum_rows * sizeof(float2));
     L.off_items = take((size_t)L.item_capacity * sizeof(uint4));
     L.off_records = take((size_t)rec_capacity * sizeof(float4));
     L.total = off;
@@ -50,18 +51,18 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity) 
 }
 
 // Largest record capacity whose layout fits into `bytes` (0 if even the fixed part does not fit).
-bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out) {
-    WsLayout L0 = make_layout(plan, n_vis, 0);
+bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out, int64_t presum_rows = 0) {
+    WsLayout L0 = make_layout(plan, n_vis, 0, presum_rows);
     if (L0.total > bytes) return false;
     const uint64_t want = (uint64_t)n_vis * 4;                      // worst case: every footprint in 4 tiles
     const size_t spare = bytes - L0.total;
     // per record: 16 B + 32/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
     uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 32.0 / WS_CHUNK)) : 0;
     if (cap > want) cap = want;
-    WsLayout L = make_layout(plan, n_vis, cap);
+    WsLayout L = make_layout(plan, n_vis, cap, presum_rows);
     while (L.total > bytes && cap > 0) {
         cap = cap > 64 ? cap - 64 : 0;
-        L = make_layout(plan, n_vis, cap);
+        L = make_layout(plan, n_vis, cap, presum_rows);
     }
     if (L.total > bytes) return false;
     *out = L;
@@ -169,7 +170,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
     if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
-    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE | WS_FLAG_TRACK_SUMWT)) != 0 || p->device < 0)
+    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE | WS_FLAG_TRACK_SUMWT | WS_FLAG_PRESUM_CHANNELS)) != 0 ||
+        p->device < 0)
         return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->kernel_param)) return WS_ERR_INVALID_ARG;
     if (p->support > 2 * WS_HALO_MAX + 1) return WS_ERR_UNSUPPORTED;
@@ -203,6 +205,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->d_taper = nullptr;
     plan->last_weights = nullptr;
     plan->last_has_values = false;
+    plan->last_chan_per_key = 1;
     plan->launches = 0;
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
@@ -281,7 +284,8 @@ size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_f
     if (!(dup_factor >= 1.0)) dup_factor = 1.0;
     if (dup_factor > 4.0) dup_factor = 4.0;
     const uint64_t cap = (uint64_t)std::ceil((double)max_vis * dup_factor) + 64;
-    const size_t a = make_layout(plan, max_vis, cap).total + 4096;   // slack for fit_layout's alignment margin
+    const bool presum = (plan->prm.flags & WS_FLAG_PRESUM_CHANNELS) != 0;          // sized for n_chan = 1, the worst case
+    const size_t a = make_layout(plan, max_vis, cap, presum ? max_vis : 0).total + 4096;   // slack for fit_layout's alignment margin
     return a > plan->fft_work_bytes ? a : plan->fft_work_bytes;
 }
 
@@ -311,10 +315,26 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
         return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: null pointer");
     if (((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)workspace) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: pointers must be 16-byte aligned");
-    const int64_t n_vis = n_rows * n_chan;
+    // WS_FLAG_PRESUM_CHANNELS: the rows are what is binned, each carrying sum_c weight * vis
+    const bool presum = with_values && (plan->prm.flags & WS_FLAG_PRESUM_CHANNELS) != 0;
+    if (presum && freq_hz)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: WS_FLAG_PRESUM_CHANNELS needs freq_hz == NULL (shared uvw)");
+    const int64_t n_vis = presum ? n_rows : n_rows * n_chan;
+    const int32_t n_chan_in = n_chan;
     WsLayout L;
-    if (!fit_layout(plan, n_vis, workspace_bytes, &L) || (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
+    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0) || (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
         return fail(plan, WS_ERR_WORKSPACE, "ws_bin_visibilities: workspace too small (see ws_workspace_bytes_for)");
+    const void* vis_in = vis;
+    const float* wt_in = weights;
+    if (presum) {
+        float2* sums = (float2*)((char*)workspace + L.off_presum);
+        const int prc = ws_launch_presum(plan, (const float2*)vis, weights, n_rows, n_chan, sums, (cudaStream_t)stream);
+        if (prc < 0) return fail(plan, prc, "ws_bin_visibilities: launch failed");
+        plan->launches += prc;
+        vis_in = sums;
+        wt_in = nullptr;
+        n_chan = 1;
+    }
 
     // O1: per-channel constants, fp64, in exactly this operation order (the bit-exact bin contract)
     const ws_params& P = plan->prm;
@@ -337,7 +357,7 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
 
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
-    const int rc = ws_launch_bin(plan, L, (char*)workspace, cc, uvw, (const float2*)vis, weights, n_rows, n_chan,
+    const int rc = ws_launch_bin(plan, L, (char*)workspace, cc, uvw, (const float2*)vis_in, wt_in, n_rows, n_chan,
                                  (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_bin_visibilities: launch failed");
     plan->launches += rc;
@@ -345,6 +365,7 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
     plan->last_layout = L;
     plan->last_n_vis = n_vis;
     plan->last_weights = weights;
+    plan->last_chan_per_key = presum ? n_chan_in : 1;
     plan->last_has_values = with_values;
     plan->last_valid = true;
     return WS_OK;
@@ -389,8 +410,8 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
     if (plan->prm.flags & WS_FLAG_TRACK_SUMWT) {
         if (mode != WS_GRID_ACCUMULATE && cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), (cudaStream_t)stream) != cudaSuccess)
             return fail(plan, WS_ERR_CUDA, "ws_grid_binned: memset failed");
-        rc = ws_launch_sum_weights(plan, plan->last_layout, (char*)workspace, plan->last_weights, plan->last_n_vis,
-                                   (cudaStream_t)stream);
+        rc = ws_launch_sum_weights(plan, plan->last_layout, (char*)workspace, plan->last_weights,
+                                   plan->last_n_vis * plan->last_chan_per_key, plan->last_chan_per_key, (cudaStream_t)stream);
         if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
         plan->launches += rc;
     }

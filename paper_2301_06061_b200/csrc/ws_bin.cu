@@ -256,7 +256,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
     if (kept) {
         if (vis) {                                  // NULL: bins for the degridder, the records carry positions only
             v = __ldcs(vis + m);
-            w = __ldcs(wt + m);
+            w = wt ? __ldcs(wt + m) : 1.0f;         // NULL: pre-summed rows, the weights are already inside
         }
         tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
         lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
@@ -313,11 +313,12 @@ k_sorted_keys(const uint32_t* __restrict__ bin_start, uint32_t n_bins, uint32_t*
 
 // ---- WS_FLAG_TRACK_SUMWT: sum of the weights of the kept visibilities (keys[] != 0xFFFFFFFF), fp64 --------------
 __global__ void __launch_bounds__(256)
-k_sum_weights(const uint32_t* __restrict__ keys, const float* __restrict__ wt, uint32_t n_vis, double* __restrict__ sum) {
+k_sum_weights(const uint32_t* __restrict__ keys, const float* __restrict__ wt, uint32_t n_vis, uint32_t chan_per_key,
+              double* __restrict__ sum) {
     __shared__ double s_part[8];
     double acc = 0.0;
     for (uint32_t m = blockIdx.x * 256u + threadIdx.x; m < n_vis; m += gridDim.x * 256u)
-        if (__ldcs(keys + m) != 0xFFFFFFFFu) acc += (double)__ldcs(wt + m);
+        if (__ldg(keys + (chan_per_key == 1u ? m : m / chan_per_key)) != 0xFFFFFFFFu) acc += (double)__ldcs(wt + m);
 #pragma unroll
     for (int d = 16; d; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
     if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
@@ -330,12 +331,46 @@ k_sum_weights(const uint32_t* __restrict__ keys, const float* __restrict__ wt, u
     }
 }
 
+// ---- WS_FLAG_PRESUM_CHANNELS: out[row] = sum_c wt[row][c] * vis[row][c] (narrow-band mode) ----------
+__global__ void __launch_bounds__(256)
+k_presum_rows(const float2* __restrict__ vis, const float* __restrict__ wt, uint32_t n_rows, uint32_t n_chan,
+              float2* __restrict__ out) {
+    const uint32_t n_warps = gridDim.x * 8u, lane = threadIdx.x & 31u;
+    for (uint32_t row = blockIdx.x * 8u + (threadIdx.x >> 5); row < n_rows; row += n_warps) {
+        const size_t base = (size_t)row * n_chan;
+        float ar = 0.f, ai = 0.f;
+        for (uint32_t c = lane; c < n_chan; c += 32u) {
+            const float2 v = __ldcs(vis + base + c);
+            const float w = __ldcs(wt + base + c);
+            ar = fmaf(w, v.x, ar);
+            ai = fmaf(w, v.y, ai);
+        }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) {
+            ar += __shfl_xor_sync(0xffffffffu, ar, d);
+            ai += __shfl_xor_sync(0xffffffffu, ai, d);
+        }
+        if (lane == 0) out[row] = make_float2(ar, ai);
+    }
+}
+
 }  // namespace
 
-int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, cudaStream_t st) {
+int ws_launch_presum(ws_plan* plan, const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, float2* out,
+                     cudaStream_t st) {
+    if (n_rows <= 0) return 0;
+    const unsigned blocks = (unsigned)std::min<int64_t>((n_rows + 7) / 8, (int64_t)plan->sm_count * 32);
+    k_presum_rows<<<blocks, 256, 0, st>>>(vis, wt, (uint32_t)n_rows, (uint32_t)n_chan, out);
+    if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
+    return 1;
+}
+
+int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, int32_t chan_per_key,
+                          cudaStream_t st) {
     if (n_vis <= 0) return 0;
     const unsigned blocks = (unsigned)std::min<int64_t>((n_vis + 255) / 256, (int64_t)plan->sm_count * 8);
-    k_sum_weights<<<blocks, 256, 0, st>>>((const uint32_t*)(ws + L.off_keys), wt, (uint32_t)n_vis, plan->d_sumwt);
+    k_sum_weights<<<blocks, 256, 0, st>>>((const uint32_t*)(ws + L.off_keys), wt, (uint32_t)n_vis, (uint32_t)chan_per_key,
+                                          plan->d_sumwt);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;
 }

@@ -43,6 +43,7 @@ struct WsLayout {
     size_t off_cursor_home, off_cursor_halo;    // [n_bins] u32: running slot cursors of the scatter
     size_t off_block_sums;                      // scan scratch
     size_t off_keys, off_perm, off_sorted_keys; // [n_vis] u32 each
+    size_t off_presum;                          // [presum_rows] float2: per-row sums of weight * vis (WS_FLAG_PRESUM_CHANNELS)
     size_t off_items;                           // heavy-chunk work items (uint4)
     size_t off_records;                         // float4 records
     size_t total;                               // bytes used for capacity `rec_capacity`
@@ -85,6 +86,7 @@ struct ws_plan {
     double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)
     float* d_taper;                             // plan-owned [N]: 1 / ghat((p - N/2)/N), fp64-computed on the host
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
+    int32_t last_chan_per_key;                  // visibilities per binned entry: 1, or n_chan after a pre-summed call
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
     bool occ_sparse;                            // ... and it was written by WS_GRID_SPARSE (private layout, empty tiles unwritten)
@@ -104,7 +106,10 @@ int ws_launch_sorted_keys(ws_plan* plan, const WsLayout& L, char* ws, cudaStream
 int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
                        cudaStream_t st);
 int ws_launch_dirty(ws_plan* plan, const float2* image, float* dirty, uint32_t norm_flags, cudaStream_t st);
-int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, cudaStream_t st);
+int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const float* wt, int64_t n_vis, int32_t chan_per_key,
+                          cudaStream_t st);
+int ws_launch_presum(ws_plan* plan, const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, float2* out,
+                     cudaStream_t st);
 int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);
 bool ws_fft_own_supported(int n_pix, int n_wplanes);
 int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error

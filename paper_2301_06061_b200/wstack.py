@@ -17,6 +17,7 @@ WS_FLAG_NO_TRANSPOSE = 2
 WS_GRID_SPARSE = 2
 WS_FFT_USE_OCCUPANCY = 1
 WS_FLAG_TRACK_SUMWT = 4
+WS_FLAG_PRESUM_CHANNELS = 8
 WS_KERNEL_GAUSSIAN = 0
 WS_KERNEL_KAISER_BESSEL = 1
 WS_NORM_SUMWT, WS_NORM_N, WS_NORM_TAPER = 1, 2, 4

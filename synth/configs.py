@@ -27,6 +27,7 @@ class ObsConfig:
     # band: Hz. narrow_band=True -> uvw handed over in wavelengths, freq=None
     freqs_hz: Tuple[float, ...] = (150e6,)
     narrow_band: bool = True
+    n_shared_chan: int = 1      # narrow-band only: visibilities (channels x polarisations) per row sharing its uvw
     # sky model
     n_src: int = 5
     src_field: float = 0.1      # side of the square the sources fall in (rad); <0: fraction of FoV
@@ -54,7 +55,7 @@ class ObsConfig:
 
     @property
     def n_chan(self) -> int:
-        return len(self.freqs_hz)
+        return self.n_shared_chan if self.narrow_band else len(self.freqs_hz)
 
     @property
     def n_vis(self) -> int:
@@ -99,6 +100,13 @@ CONFIGS = {
         freqs_hz=_band(120, 180, 32), narrow_band=False, n_src=2000, src_field=-0.8, flux_law="powerlaw",
         noise_sigma=0.05, weights="uniform", diffuse_rms=0.1, n_pix=16384, n_wplanes=32, support=9,
         umax_lambda=8100.0, cell_rad=1.0 / 16384, n_chunks=8),
+    # the shape of the paper's own "Medium" test (Table 3: 0.54e9 visibilities, mesh
+    # 4096 x 4096 x 16) in its narrow-band mode (:207, one uvw per measurement shared by all frequencies and
+    # polarisations): 1891 baselines x 7200 samples = 13,615,200 rows x 40 (20 channels x 2 polarisations) = 544,608,000
+    "paper_medium": ObsConfig(
+        name="paper_medium", seed=1006, layout="lofar_like", n_ant=62, n_times=7200, hours=8.0, dec_deg=27.5,
+        freqs_hz=(150e6,), narrow_band=True, n_shared_chan=40, n_src=500, src_field=0.2, flux_law="powerlaw",
+        noise_sigma=0.05, weights="uniform", n_pix=4096, n_wplanes=16, support=7),
 }
 
 

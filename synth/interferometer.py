@@ -192,12 +192,14 @@ def make_dataset(cfg: ObsConfig, device="cpu", with_noise=True) -> Dataset:
     lattice = _diffuse_lattice(rng_src, cfg.diffuse_rms) if cfg.diffuse_rms > 0 else None
 
     n_rows, n_chan = uvw32.shape[0], len(ch_scale)
-    vis = torch.empty((n_rows, n_chan), dtype=torch.complex64, device=dev)
+    n_shared = cfg.n_shared_chan if cfg.narrow_band else 1
+    vis = torch.empty((n_rows, n_chan * n_shared), dtype=torch.complex64, device=dev)
     lmn = torch.tensor(np.stack([l, m, nm1], axis=0), dtype=torch.float64, device=dev)     # [3, n_src]
     flx = torch.tensor(flux, dtype=torch.complex128, device=dev)
     sc = torch.tensor(ch_scale, dtype=torch.float64, device=dev)
     lat_t = torch.tensor(lattice, device=dev) if lattice is not None else None
     rows_per_block = max(1, (1 << 25) // max(1, n_chan * cfg.n_src))
+    n_out = n_chan * n_shared
     uvw_t = torch.from_numpy(uvw32).to(dev)
     for lo in range(0, n_rows, rows_per_block):
         hi = min(n_rows, lo + rows_per_block)
@@ -211,21 +213,24 @@ def make_dataset(cfg: ObsConfig, device="cpu", with_noise=True) -> Dataset:
             iu = torch.clamp(torch.round((pl[:, 0] / umax * 0.5 + 0.5) * (nl - 1)).long(), 0, nl - 1)
             iv = torch.clamp(torch.round((pl[:, 1] / umax * 0.5 + 0.5) * (nl - 1)).long(), 0, nl - 1)
             v = v + lat_t[iv, iu]
-        vis[lo:hi] = v.reshape(hi - lo, n_chan).to(torch.complex64)
+        if n_shared > 1:      # narrow band: every channel / polarisation of the row sees the same model visibility
+            vis[lo:hi] = v.reshape(hi - lo, 1).to(torch.complex64).expand(hi - lo, n_shared)
+        else:
+            vis[lo:hi] = v.reshape(hi - lo, n_chan).to(torch.complex64)
     if with_noise and cfg.noise_sigma > 0:
         for lo in range(0, n_rows, _NOISE_BLOCK_ROWS):
             hi = min(n_rows, lo + _NOISE_BLOCK_ROWS)
-            z = rng_noise.standard_normal((hi - lo, n_chan, 2), dtype=np.float32) * np.float32(cfg.noise_sigma)
+            z = rng_noise.standard_normal((hi - lo, n_out, 2), dtype=np.float32) * np.float32(cfg.noise_sigma)
             vis[lo:hi] += torch.view_as_complex(torch.from_numpy(z)).to(dev)
 
     if cfg.weights == "unit":
-        wt = torch.ones((n_rows, n_chan), dtype=torch.float32, device=dev)
+        wt = torch.ones((n_rows, n_out), dtype=torch.float32, device=dev)
     else:
-        wt = torch.empty((n_rows, n_chan), dtype=torch.float32, device=dev)
+        wt = torch.empty((n_rows, n_out), dtype=torch.float32, device=dev)
         for lo in range(0, n_rows, _NOISE_BLOCK_ROWS):
             hi = min(n_rows, lo + _NOISE_BLOCK_ROWS)
             wt[lo:hi] = torch.from_numpy(
-                (0.5 + rng_wt.random((hi - lo, n_chan), dtype=np.float32)).astype(np.float32)).to(dev)
+                (0.5 + rng_wt.random((hi - lo, n_out), dtype=np.float32)).astype(np.float32)).to(dev)
 
     return Dataset(name=cfg.name, uvw=uvw_t, vis=vis, weights=wt, freqs_hz=freqs,
                    n_pix=cfg.n_pix, n_wplanes=cfg.n_wplanes, support=cfg.support,

@@ -161,3 +161,43 @@ def test_calibrated_image_equals_direct_dft_on_the_gpu(oracle):
     inner = slice(N // 4, 3 * N // 4)
     err = np.abs(dirty.cpu().numpy()[inner, inner] - ref[inner, inner]).max() / np.abs(ref).max()
     assert err < 1e-5, err
+
+
+@pytest.mark.parametrize("n_chan", [5, 40])
+def test_narrow_band_presummed_channels(oracle, n_chan):
+    """SURVEY 8(f) NEXT-4, the paper's narrow-band mode: freq_hz = NULL, the n_chan visibilities of a row
+    share its uvw.  A plan with WS_FLAG_PRESUM_CHANNELS sums weight * vis per row first and bins rows; mesh, image and
+    the sum of weights must equal the oracle's plain per-visibility gridding; the exported bins are per row."""
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(900 + n_chan, 3000, n_chan, 256, 4, 7, wavelengths=True, fill=1.03, w_span=30.0, cell_rad=2e-3)
+    assert d.freqs_hz is None
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells,
+                   flags=ws.WS_FLAG_PRESUM_CHANNELS | ws.WS_FLAG_TRACK_SUMWT)
+    prm = U.oracle_params(oracle, d, 32)
+    dev = d.to("cuda")
+    grid, image = plan.alloc_grid(), plan.alloc_image()
+    wsp = plan.alloc_workspace(d.n_rows)                     # rows, not visibilities
+    grid.fill_(float("nan"))
+    plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_OVERWRITE)
+    plan.async_status()
+    bins = plan.get_bins()
+    assert bins["n_vis"] == d.n_rows
+    key_rows = oracle.positions(prm, d.uvw.numpy(), 1)["key"]
+    assert np.array_equal(bins["keys"], key_rows) and bins["n_dropped"] == int((key_rows == 0xFFFFFFFF).sum()) > 0
+    D, G = oracle.dirty_image(prm, *_np(d), return_grid=True)
+    U.assert_close(U.logical(grid), G, "mesh (pre-summed channels)")
+    sw = oracle.sum_weights(prm, d.uvw.numpy(), d.weights.numpy())
+    assert abs(plan.sum_weights() - sw) <= 1e-12 * sw
+    grid.fill_(float("nan"))
+    plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, None, grid, wsp, mode=ws.WS_GRID_SPARSE)
+    plan.fft_wcorrect(grid, image, wsp, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    U.assert_close(image.cpu().numpy(), D, "image (pre-summed channels)")
+    # the same plan still degrids per visibility; a frequency axis is refused
+    pred = torch.empty_like(dev.vis)
+    wsp2 = plan.alloc_workspace(d.n_vis)
+    plan.predict_planes(torch.from_numpy(D.astype(np.complex64)).cuda(), grid, wsp2)
+    plan.degrid_visibilities(dev.uvw, None, d.n_chan, grid, pred, wsp2)
+    ref = oracle.predict(prm, D.astype(np.complex64), d.uvw.numpy(), d.n_chan, None)
+    U.assert_close(pred.cpu().numpy(), ref, "degridding on a pre-sum plan")
+    with pytest.raises(ws.WStackError):
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, [150e6] * n_chan, grid, wsp2, mode=ws.WS_GRID_OVERWRITE)
