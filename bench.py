@@ -131,6 +131,20 @@ def run_reference(args, d, cfg_name):
             "cpu_baseline": cb, "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
 
 
+def reduce_max_ms(ms, dist, device):
+    """The step time of the whole job: the MAX over ranks of the per-rank device time (replicas run side by side)."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_vis_per_rank, world, ms_step):
+    """Mvis/s of all ranks together (weak scaling: every rank images its own replica of the workload)."""
+    return world * n_vis_per_rank / (ms_step * 1e-3) / 1e6
+
+
 def workload_config(d, cfg_name):
     return {"workload": f"{cfg_name}: {d.n_vis} visibilities ({d.n_rows} rows x {d.n_chan} channels), "
                         f"{d.n_pix}x{d.n_pix} complex64 mesh, {d.n_wplanes} w-planes, "
@@ -243,15 +257,12 @@ def main():
     launches = plan.launch_count() - l0
     clk = clocks.stop()
     total_ms = t_start.elapsed_time(t_end)
-    if dist:
-        t = torch.tensor([total_ms], device=f"cuda:{local_rank}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = reduce_max_ms(total_ms, dist, f"cuda:{local_rank}")
     plan.async_status()
     ms_step = total_ms / args.steps
     st = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])     # bin, grid, fft, wcorrect
     med = np.median(st, axis=0)
-    value = world * d.n_vis / (ms_step * 1e-3) / 1e6
+    value = whole_job_value(d.n_vis, world, ms_step)
 
     # ---- the library path on the same inputs, for the separate FFT figure (north_star): OVERWRITE gridding,
     # cuFFT per plane, stand-alone w-correction.  Outside the timed region.
@@ -372,11 +383,8 @@ def main():
             plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
         torch.cuda.synchronize()
         e2e_ms = (time.perf_counter() - t0) / k_e2e * 1e3
-        if dist:
-            t = torch.tensor([e2e_ms], device=f"cuda:{local_rank}")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_ms = float(t.item())
-        out["e2e"] = {"value": world * d.n_vis / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": e2e_ms,
+        e2e_ms = reduce_max_ms(e2e_ms, dist, f"cuda:{local_rank}")
+        out["e2e"] = {"value": whole_job_value(d.n_vis, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                       "h2d_bytes_per_step": 12 * d.n_rows + 12 * d.n_vis, "d2h_bytes_per_step": 4 * d.n_pix ** 2,
                       "steps": k_e2e, "checksum": float(dirty_h[d.n_pix // 2, d.n_pix // 2])}
         del dev_in
