@@ -10,6 +10,7 @@ import torch
 
 from . import build as _build
 
+WS_VERSION = 140            # include/wstack.h
 WS_GRID_ACCUMULATE = 0
 WS_GRID_OVERWRITE = 1
 WS_FLAG_LIBRARY_FFT = 1
@@ -93,6 +94,9 @@ def lib():
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
         fn.restype, fn.argtypes = res, args
+    if L.ws_version() != WS_VERSION:
+        raise RuntimeError(f"libwstack.so is version {L.ws_version()}, the binding expects {WS_VERSION}: rebuild "
+                           "(python -m paper_2301_06061_b200.build --force)")
     _lib = L
     return L
 

@@ -27,7 +27,9 @@ def test_header_symbols_are_exported():
 def test_host_only_calls():
     import paper_2301_06061_b200 as ws
     L = ws.lib()
-    assert L.ws_version() == 140
+    assert L.ws_version() == ws.WS_VERSION
+    hdr = open(os.path.join(ROOT, "include", "wstack.h")).read()
+    assert int(re.search(r"#define WS_VERSION (\d+)", hdr).group(1)) == ws.WS_VERSION
     assert L.ws_strerror(-3) == b"workspace too small"
     assert L.ws_grid_bytes(None) == 0 and L.ws_launch_count(None) == 0
 

@@ -31,7 +31,7 @@ def _full_check(oracle, d, **kw):
 
 def test_library_loaded_is_the_cuda_one():
     import paper_2301_06061_b200 as ws
-    assert ws.lib().ws_version() == 140
+    assert ws.lib().ws_version() == ws.WS_VERSION
     assert torch.cuda.is_available()
 
 
