@@ -262,6 +262,9 @@ def main():
     ms_step = total_ms / args.steps
     st = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])     # bin, grid, fft, wcorrect
     med = np.median(st, axis=0)
+    per_step = st.sum(axis=1)      # device time of each timed step (median, mean +- std, min)
+    step_stats = {"median": float(np.median(per_step)), "mean": float(per_step.mean()), "std": float(per_step.std()),
+                  "min": float(per_step.min())}
     value = whole_job_value(d.n_vis, world, ms_step)
 
     # ---- the library path on the same inputs, for the separate FFT figure (north_star): OVERWRITE gridding,
@@ -360,7 +363,7 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
-           "stages_ms_median": {n: float(v) for n, v in zip(stage_names, med)},
+           "stages_ms_median": {n: float(v) for n, v in zip(stage_names, med)}, "step_ms_stats": step_stats,
            "fft": "own two-pass FFT with fused w-correction, occupancy-aware" if own else "cuFFT",
            "library_path_ms": lib_ms, "degridding_ms": degrid_ms, "occupancy": occ,
            "mvis_per_s_gridding": d.n_vis / ((med[0] + med[1]) * 1e-3) / 1e6,

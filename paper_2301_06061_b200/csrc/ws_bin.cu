@@ -90,7 +90,8 @@ __device__ __forceinline__ void row_chan(uint32_t m, uint32_t n_chan, int chan_s
 __global__ void __launch_bounds__(256)
 k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
             const float* __restrict__ uvw, uint32_t n_vis, uint32_t n_chan, int chan_shift,
-            uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_halo) {
+            uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_halo,
+            int home_only) {
     __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
     stage_consts(cc, n_chan, s_su, s_sw);
     const uint32_t m = blockIdx.x * 256u + threadIdx.x;
@@ -112,6 +113,7 @@ k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsG
         // tiles the footprint overlaps: own, and the neighbour on each side it sticks out of
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
+        if (home_only) dx = dy = 0;               // bins for the degridder: a gather needs no copies in neighbour tiles
     }
     if (m < n_vis) keys[m] = home;
     // two histograms: visibilities per home bin (-> bin_start) and halo copies received per bin; the record
@@ -235,7 +237,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
           const float* __restrict__ uvw, const float2* __restrict__ vis, const float* __restrict__ wt,
           uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home,
           uint32_t* __restrict__ cursor_halo, const uint32_t* __restrict__ halo_start, uint32_t* __restrict__ perm,
-          float4* __restrict__ records, const WsStatus* __restrict__ status) {
+          float4* __restrict__ records, const WsStatus* __restrict__ status, int home_only) {
     if (status->overflow) return;
     __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
     stage_consts(cc, n_chan, s_su, s_sw);
@@ -264,6 +266,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         hs = __ldg(halo_start + home);
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
+        if (home_only) dx = dy = 0;
     }
     // slots: every group leader issues its atomics back to back, the results are broadcast afterwards.  The home
     // copy needs no second atomic: its record slot is its perm slot shifted by the bin's halo_start.
@@ -378,6 +381,7 @@ int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const floa
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {
     const WsGeom& g = plan->geom;
+    const int home_only = vis == nullptr;          // positions only: the degridder's gather
     const uint32_t n_vis = (uint32_t)(n_rows * n_chan);
     uint32_t* counts_home = (uint32_t*)(ws + L.off_counts_home);   // -> bin_start
     uint32_t* counts_halo = (uint32_t*)(ws + L.off_counts_halo);   // -> halo_start
@@ -402,7 +406,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     const uint32_t n_blocks = (n_scan + SCAN_BLOCK - 1) / SCAN_BLOCK;
     if (n_vis) {
         k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, chan_shift, keys,
-                                                         counts_home, counts_halo);
+                                                         counts_home, counts_halo, home_only);
         ++launches;
     }
     k_scan_reduce<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
@@ -413,7 +417,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     launches += 4;
     if (n_vis) {
         k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift,
-                                                       cursor_home, cursor_halo, counts_halo, perm, records, status);
+                                                       cursor_home, cursor_halo, counts_halo, perm, records, status, home_only);
         ++launches;
     }
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
