@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-degrid", action="store_true")
+    ap.add_argument("--no-snapshot-hint", action="store_true")
     args = ap.parse_args()
     global KERNEL
     KERNEL = args.kernel
@@ -204,6 +205,8 @@ def main():
     else:
         plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank,
                        flags=flags)
+    if d.rows_per_snapshot and not args.no_snapshot_hint:   # the rows are time-major, every baseline per snapshot
+        plan.set_snapshot_rows(d.rows_per_snapshot)
     grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
     wsp = plan.alloc_workspace(d.n_rows if presum else d.n_vis)
 
@@ -370,6 +373,7 @@ def main():
            "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
            "ggpas_bin_and_grid": d.n_vis * d.support ** 2 / ((med[0] + med[1]) * 1e-3) / 1e9,
            "presummed_channels": bool(presum),
+           "snapshot_rows_hint": int(d.rows_per_snapshot) if (d.rows_per_snapshot and not args.no_snapshot_hint) else 0,
            "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "kernels": per_kernel,
            "roofline_path": roof_path}
 

@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 140
+#define WS_VERSION 150
 
 /* error codes */
 #define WS_OK 0
@@ -110,6 +110,14 @@ typedef struct ws_params {
  * caller's workspace).  *out is NULL on failure. */
 int ws_plan_create(const ws_params* p, ws_plan** out);
 int ws_plan_destroy(ws_plan* plan);
+
+/* Performance hint, never needed for correctness: the rows of every later gridding / degridding call are recorded
+ * snapshot after snapshot with `rows_per_snapshot` rows (all baselines) per snapshot, in the same baseline order each
+ * time (measurement sets are stored this way).  The binning kernels then walk the visibilities so that a
+ * warp holds a few memory-adjacent visibilities of consecutive snapshots, which fall into the same bins: binning is
+ * about twice as fast.  0 switches the hint off.  The results are the same sets either way (the order inside a bin
+ * is unspecified in both cases); a wrong hint only costs speed. */
+int ws_plan_set_snapshot_rows(ws_plan* plan, int64_t rows_per_snapshot);
 
 /* ---- sizes: all device memory is allocated by the caller ---------------------------------------------- */
 size_t ws_grid_bytes(const ws_plan* plan);   /* 8 N^2 N_w */

@@ -204,6 +204,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->d_sumwt = nullptr;
     plan->d_taper = nullptr;
     plan->last_weights = nullptr;
+    plan->snapshot_rows = 0;
     plan->last_has_values = false;
     plan->last_chan_per_key = 1;
     plan->launches = 0;
@@ -266,6 +267,14 @@ int ws_plan_destroy(ws_plan* plan) {
     if (plan->d_twiddles) cudaFree(plan->d_twiddles);
     if (plan->d_masks) cudaFree(plan->d_masks);
     delete plan;
+    return WS_OK;
+}
+
+int ws_plan_set_snapshot_rows(ws_plan* plan, int64_t rows_per_snapshot) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (rows_per_snapshot < 0 || rows_per_snapshot > MAX_VIS)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_plan_set_snapshot_rows: bad count");
+    plan->snapshot_rows = rows_per_snapshot;
     return WS_OK;
 }
 

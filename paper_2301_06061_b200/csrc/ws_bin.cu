@@ -5,6 +5,7 @@
 // the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
 // it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
 #include <algorithm>
+#include <cstdlib>
 
 #include "ws_internal.h"
 
@@ -76,6 +77,17 @@ __device__ __forceinline__ void stage_consts(const WsChanConsts& cc, uint32_t n_
     __syncthreads();
 }
 
+// thread index -> flat visibility index (WsRemap, ws_internal.h).  Warp w = (snapshot block tb, adjacent group f_hi);
+// lane = f_lo * ts + tt: the ts consecutive snapshots of one (baseline, channel) sit in consecutive lanes, so that
+// the slots they take in a bin are consecutive too.
+__device__ __forceinline__ uint32_t remap(const WsRemap& r, uint32_t mp) {
+    if (r.cw == 0u || mp >= r.n_main) return mp;
+    const uint32_t L = mp & 31u, wq = mp >> 5, ts_log2 = 5u - r.cw_log2;
+    const uint32_t tt = L & ((1u << ts_log2) - 1u), f_lo = L >> ts_log2;
+    const uint32_t f_hi = wq / r.n_t, tb = wq - f_hi * r.n_t;               // n_t: whole blocks of ts snapshots
+    return ((tb << ts_log2) + tt) * r.per_snap + (f_hi << r.cw_log2) + f_lo;
+}
+
 __device__ __forceinline__ void row_chan(uint32_t m, uint32_t n_chan, int chan_shift, uint32_t& row, uint32_t& c) {
     if (chan_shift >= 0) {
         row = m >> chan_shift;
@@ -91,10 +103,10 @@ __global__ void __launch_bounds__(256)
 k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
             const float* __restrict__ uvw, uint32_t n_vis, uint32_t n_chan, int chan_shift,
             uint32_t* __restrict__ keys, uint32_t* __restrict__ counts_home, uint32_t* __restrict__ counts_halo,
-            int home_only) {
+            int home_only, const __grid_constant__ WsRemap rm) {
     __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
     stage_consts(cc, n_chan, s_su, s_sw);
-    const uint32_t m = blockIdx.x * 256u + threadIdx.x;
+    const uint32_t m = remap(rm, blockIdx.x * 256u + threadIdx.x);
     const int lane = threadIdx.x & 31;
     Placed pl;
     bool kept = false;
@@ -237,11 +249,12 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
           const float* __restrict__ uvw, const float2* __restrict__ vis, const float* __restrict__ wt,
           uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home,
           uint32_t* __restrict__ cursor_halo, const uint32_t* __restrict__ halo_start, uint32_t* __restrict__ perm,
-          float4* __restrict__ records, const WsStatus* __restrict__ status, int home_only) {
+          float4* __restrict__ records, const WsStatus* __restrict__ status, int home_only,
+          const __grid_constant__ WsRemap rm) {
     if (status->overflow) return;
     __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
     stage_consts(cc, n_chan, s_su, s_sw);
-    const uint32_t m = blockIdx.x * 256u + threadIdx.x;
+    const uint32_t m = remap(rm, blockIdx.x * 256u + threadIdx.x);
     const int lane = threadIdx.x & 31;
     Placed pl;
     bool kept = false;
@@ -382,6 +395,19 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {
     const WsGeom& g = plan->geom;
     const int home_only = vis == nullptr;          // positions only: the degridder's gather
+    WsRemap rm = {0u, 0u, 0u, 0u, 0u};
+    if (plan->snapshot_rows > 0 && n_rows >= 2 * plan->snapshot_rows) {
+        const uint64_t F = (uint64_t)plan->snapshot_rows * (uint64_t)n_chan;
+        uint32_t lg = 2;                              // cw = 4 adjacent visibilities x 8 snapshots per warp
+        while (lg > 0 && (F & ((1u << lg) - 1u))) --lg;
+        if (const char* e = getenv("WS_DEBUG_REMAP_CW_LOG2")) lg = (uint32_t)atoi(e);   // tuning aid
+        rm.cw_log2 = lg;
+        rm.cw = 1u << lg;
+        rm.n_t = (uint32_t)((n_rows / plan->snapshot_rows) >> (5u - lg));    // blocks of ts = 32 / cw snapshots
+        rm.per_snap = (uint32_t)F;
+        rm.n_main = (uint32_t)(((uint64_t)rm.n_t << (5u - lg)) * F);
+        if (rm.n_t == 0) rm.cw = 0u;
+    }
     const uint32_t n_vis = (uint32_t)(n_rows * n_chan);
     uint32_t* counts_home = (uint32_t*)(ws + L.off_counts_home);   // -> bin_start
     uint32_t* counts_halo = (uint32_t*)(ws + L.off_counts_halo);   // -> halo_start
@@ -406,7 +432,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     const uint32_t n_blocks = (n_scan + SCAN_BLOCK - 1) / SCAN_BLOCK;
     if (n_vis) {
         k_keys_hist<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, n_vis, (uint32_t)n_chan, chan_shift, keys,
-                                                         counts_home, counts_halo, home_only);
+                                                         counts_home, counts_halo, home_only, rm);
         ++launches;
     }
     k_scan_reduce<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
@@ -417,7 +443,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     launches += 4;
     if (n_vis) {
         k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift,
-                                                       cursor_home, cursor_halo, counts_halo, perm, records, status, home_only);
+                                                       cursor_home, cursor_halo, counts_halo, perm, records, status, home_only, rm);
         ++launches;
     }
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;

@@ -36,6 +36,18 @@ struct WsGeom {
     float kb_c[WS_KB_MAX_TERMS];
 };
 
+// Order in which the binning kernels walk the visibilities (ws_plan_set_snapshot_rows).  The input is time-major: a
+// snapshot holds F = rows_per_snapshot * n_chan visibilities that lie next to each other in memory, and one (baseline,
+// channel) moves by about a cell from one snapshot to the next.  A warp takes `cw` memory-adjacent
+// visibilities of 32 / cw CONSECUTIVE SNAPSHOTS, so that most of its lanes fall into the same few bins: their slots
+// are adjacent, the record / perm stores coalesce and one atomic serves many lanes.  cw = 0: input order.
+struct WsRemap {
+    uint32_t cw_log2, cw;      // cw: power of two dividing F (4 where possible); ts = 32 / cw snapshots per warp
+    uint32_t n_t;              // whole blocks of ts snapshots in this call
+    uint32_t per_snap;         // F
+    uint32_t n_main;           // n_t * ts * F: visibilities beyond (ragged last block / snapshot) keep the input order
+};
+
 // Workspace carve-up for one ws_grid_visibilities call (all offsets 256-byte aligned).
 struct WsLayout {
     size_t off_counts_home, off_counts_halo;    // [n_bins + 1] u32 each: histograms -> exclusive scans (bin_start / halo_start)
@@ -85,6 +97,7 @@ struct ws_plan {
     size_t mask_words, mask_set_words;          // whole buffer; one set (class masks + band masks) of the two orientations
     double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)
     float* d_taper;                             // plan-owned [N]: 1 / ghat((p - N/2)/N), fp64-computed on the host
+    int64_t snapshot_rows;                      // ws_plan_set_snapshot_rows hint (0: none)
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
     int32_t last_chan_per_key;                  // visibilities per binned entry: 1, or n_chan after a pre-summed call
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)

@@ -48,6 +48,8 @@ class Dataset:
     src_l: Optional[np.ndarray] = None
     src_m: Optional[np.ndarray] = None
     src_flux: Optional[np.ndarray] = None
+    # rows per snapshot (= baselines) when the rows are time-major with every baseline per snapshot
+    rows_per_snapshot: Optional[int] = None
 
     @property
     def n_rows(self) -> int:
@@ -235,7 +237,7 @@ def make_dataset(cfg: ObsConfig, device="cpu", with_noise=True) -> Dataset:
     return Dataset(name=cfg.name, uvw=uvw_t, vis=vis, weights=wt, freqs_hz=freqs,
                    n_pix=cfg.n_pix, n_wplanes=cfg.n_wplanes, support=cfg.support,
                    sigma_cells=cfg.sigma_cells, cell_rad=float(cell), w_min=w_min, w_max=w_max,
-                   n_chunks=cfg.n_chunks, src_l=l, src_m=m, src_flux=flux)
+                   n_chunks=cfg.n_chunks, src_l=l, src_m=m, src_flux=flux, rows_per_snapshot=cfg.n_baselines)
 
 
 def make_random_dataset(seed: int, n_rows: int, n_chan: int, n_pix: int, n_wplanes: int, support: int,

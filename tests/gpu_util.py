@@ -13,7 +13,10 @@ def oracle_params(oracle, d, tile):
 
 def make_plan(d, device=0):
     import paper_2301_06061_b200 as ws
-    return ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=device)
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=device)
+    if getattr(d, "rows_per_snapshot", None):      # the configs are time-major: the launch configuration bench.py times
+        plan.set_snapshot_rows(d.rows_per_snapshot)
+    return plan
 
 
 def logical(grid_stored: torch.Tensor) -> np.ndarray:

@@ -129,6 +129,7 @@ def test_large_config_kaiser_bessel_and_degridding_sampled(oracle):
     beta = _kb_beta(d.support)
     plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, kernel_type=ws.WS_KERNEL_KAISER_BESSEL,
                    kernel_param=beta)
+    plan.set_snapshot_rows(d.rows_per_snapshot)
     prm = U.oracle_params(oracle, d, plan.tile)
     prm.kernel_type, prm.sigma = oracle.KERNEL_KAISER_BESSEL, beta
     grid, image = plan.alloc_grid(), plan.alloc_image()

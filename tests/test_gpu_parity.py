@@ -261,3 +261,26 @@ def test_small_config(oracle):
     d = make_dataset(get_config("small"))
     out, eg, ei = _full_check(oracle, d)
     print("small grid/image errors", eg, ei)
+
+
+@pytest.mark.parametrize("n_bl,n_chan,n_rows", [(100, 8, 4000), (100, 3, 4037), (97, 1, 4000), (64, 5, 130), (4000, 2, 4000)])
+def test_snapshot_order_hint_changes_nothing_but_speed(oracle, n_bl, n_chan, n_rows):
+    """ws_plan_set_snapshot_rows only changes the order in which the binning kernels walk the input: keys, bin
+    offsets, sorted keys bit-exact, perm the same per-bin sets, mesh and image within tolerance -- with a ragged last
+    snapshot, with F = n_bl * n_chan odd (cw falls back to 1), with fewer than two snapshots (hint ignored)."""
+    d = make_random_dataset(600 + n_bl + n_chan, n_rows, n_chan, 256, 4, 7, wavelengths=False, fill=1.03, w_span=30.0, cell_rad=2e-3)
+    plan = U.make_plan(d)
+    plan.set_snapshot_rows(n_bl)
+    out, _, _ = _full_check(oracle, d, plan=plan)
+    assert out["bins"]["n_dropped"] > 0
+    # degridding through the same walk
+    M = (np.random.default_rng(1).standard_normal((256, 256)) + 0j).astype(np.complex64)
+    dev = d.to("cuda")
+    planes, wsp = plan.alloc_grid(), plan.alloc_workspace(d.n_vis)
+    plan.predict_planes(torch.from_numpy(M).cuda(), planes, wsp)
+    vis = torch.empty_like(dev.vis)
+    plan.degrid_visibilities(dev.uvw, d.freqs_hz, d.n_chan, planes, vis, wsp)
+    prm = U.oracle_params(oracle, d, 32)
+    U.assert_close(vis.cpu().numpy(), oracle.predict(prm, M, d.uvw.numpy(), d.n_chan, d.freqs_hz), "degrid with the hint")
+    with pytest.raises(Exception):
+        plan.set_snapshot_rows(-1)
