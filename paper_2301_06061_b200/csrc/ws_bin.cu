@@ -5,7 +5,6 @@
 // the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
 // it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
 #include <algorithm>
-#include <cstdlib>
 
 #include "ws_internal.h"
 
@@ -400,7 +399,6 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
         const uint64_t F = (uint64_t)plan->snapshot_rows * (uint64_t)n_chan;
         uint32_t lg = 2;                              // cw = 4 adjacent visibilities x 8 snapshots per warp
         while (lg > 0 && (F & ((1u << lg) - 1u))) --lg;
-        if (const char* e = getenv("WS_DEBUG_REMAP_CW_LOG2")) lg = (uint32_t)atoi(e);   // tuning aid
         rm.cw_log2 = lg;
         rm.cw = 1u << lg;
         rm.n_t = (uint32_t)((n_rows / plan->snapshot_rows) >> (5u - lg));    // blocks of ts = 32 / cw snapshots

@@ -187,12 +187,8 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, f
              cudaStream_t st) {
     using C = DgCfg<S>;
     const size_t smem = C::WARP_BYTES * C::WARPS;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_degrid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return WS_ERR_CUDA;
-        attr_set = true;
-    }
+    // per device, and cheap: set on every launch rather than cached in a process-wide flag
+    if (cudaFuncSetAttribute(k_degrid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return WS_ERR_CUDA;
     const uint32_t* bin_start = (const uint32_t*)(ws + L.off_counts_home);
     const uint32_t* halo_start = (const uint32_t*)(ws + L.off_counts_halo);
     uint4* items = (uint4*)(ws + L.off_items);

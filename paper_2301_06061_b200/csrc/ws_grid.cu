@@ -269,12 +269,8 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     const uint32_t* orient = mode == WS_GRID_SPARSE ? ws_fft_orientation_flag(plan) : nullptr;
     using C = TileCfg<S>;
     const size_t smem = C::WARP_BYTES * C::WARPS;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_grid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return WS_ERR_CUDA;
-        attr_set = true;
-    }
+    // per device, and cheap: set on every launch rather than cached in a process-wide flag
+    if (cudaFuncSetAttribute(k_grid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return WS_ERR_CUDA;
     const uint32_t* rec_start = (const uint32_t*)(ws + L.off_rec_start);
     const float4* records = (const float4*)(ws + L.off_records);
     WsStatus* status = plan->d_status;
