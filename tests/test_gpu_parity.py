@@ -284,3 +284,22 @@ def test_snapshot_order_hint_changes_nothing_but_speed(oracle, n_bl, n_chan, n_r
     U.assert_close(vis.cpu().numpy(), oracle.predict(prm, M, d.uvw.numpy(), d.n_chan, d.freqs_hz), "degrid with the hint")
     with pytest.raises(Exception):
         plan.set_snapshot_rows(-1)
+
+
+def test_channel_count_limits_and_single_plane(oracle):
+    """Degenerate and maximal shapes: n_chan = 128 (the most a call accepts; 129 is refused), one w-plane, and a
+    non-power-of-two channel count with the row / channel split done by division."""
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(701, 300, 128, 256, 1, 7, wavelengths=False, fill=1.02, w_span=5.0, cell_rad=2e-3)
+    out, _, _ = _full_check(oracle, d)
+    assert out["plan"].n_wplanes == 1
+    dev = d.to("cuda")
+    plan = out["plan"]
+    grid, wsp = plan.alloc_grid(), plan.alloc_workspace(300 * 129)
+    vis129 = torch.zeros((300, 129), dtype=torch.complex64, device="cuda")
+    wt129 = torch.ones((300, 129), dtype=torch.float32, device="cuda")
+    with pytest.raises(ws.WStackError) as e:
+        plan.grid_visibilities(dev.uvw, vis129, wt129, [150e6] * 129, grid, wsp)
+    assert e.value.code == -2
+    d = make_random_dataset(702, 2000, 7, 256, 3, 5, wavelengths=False, fill=0.9, w_span=15.0, cell_rad=2e-3)
+    _full_check(oracle, d)
