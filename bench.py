@@ -166,6 +166,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-degrid", action="store_true")
     ap.add_argument("--no-snapshot-hint", action="store_true")
+    ap.add_argument("--chunked", action="store_true", help="configs with n_chunks > 1: grid the row chunks one call at a time")
     args = ap.parse_args()
     global KERNEL
     KERNEL = args.kernel
@@ -213,7 +214,32 @@ def main():
     own = plan.fft_is_own
     OCC = ws.WS_FFT_USE_OCCUPANCY
 
+    chunks = d.row_chunks() if (args.chunked and d.n_chunks > 1) else None
+    if chunks:      # Extreme's recipe: row chunks through repeated accumulate calls onto a cleared mesh
+        del wsp
+        wsp = plan.alloc_workspace(max(hi - lo for lo, hi in chunks) * d.n_chan)
+
+    def step_chunked(ev=None):
+        # stages: [zero] [bin + grid of all chunks] [FFT] [w-correct]; the library FFT path (no occupancy of a partial mesh)
+        if ev: ev[0].record()
+        plan.grid_zero(grid)
+        if ev: ev[1].record()
+        for lo, hi in chunks:
+            plan.grid_visibilities(d.uvw[lo:hi], d.vis[lo:hi], d.weights[lo:hi], d.freqs_hz, grid, wsp, mode=ws.WS_GRID_ACCUMULATE)
+        if ev: ev[2].record()
+        if own:
+            plan.fft_columns(grid, OCC)
+            if ev: ev[3].record()
+            plan.fft_rows_wcorrect(grid, image, accumulate=False, dirty=dirty, fft_flags=OCC)
+        else:
+            plan.fft_planes(grid, wsp)
+            if ev: ev[3].record()
+            plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
+        if ev: ev[4].record()
+
     def step(ev=None):
+        if chunks:
+            return step_chunked(ev)
         if ev: ev[0].record()
         plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
         if ev: ev[1].record()
@@ -235,12 +261,16 @@ def main():
         step()
     plan.async_status()
     bins_info = None
-    plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+    if chunks:      # statistics of the first chunk stand for all (same recipe per chunk)
+        lo0, hi0 = chunks[0]
+        plan.bin_visibilities(d.uvw[lo0:hi0], d.vis[lo0:hi0], d.weights[lo0:hi0], d.freqs_hz, wsp)
+    else:
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
     b = plan.get_bins(fields=("bin_start",))
     bins_info = {"n_dropped": b["n_dropped"], "n_records": b["n_records"],
                  "max_bin": int(np.diff(b["bin_start"].astype(np.int64)).max()),
                  "empty_bins_frac": float((np.diff(b["bin_start"].astype(np.int64)) == 0).mean())}
-    n_records = b["n_records"]
+    n_records = b["n_records"] * (len(chunks) if chunks else 1)
     del b
 
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
@@ -274,7 +304,7 @@ def main():
     # cuFFT per plane, stand-alone w-correction.  Outside the timed region.
     lib_ms = None
     occ = plan.occupancy() if own else None      # of the timed path's mesh (fractions the FFT passes touch; orientation)
-    if own:
+    if own and not chunks:
         e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         rows = []
         for _ in range(3):
@@ -294,7 +324,7 @@ def main():
     # ---- degridding on the same positions, outside the timed region: model image -> planes
     # (forward w-screen + cuFFT), then bins + footprint gather
     degrid_ms = None
-    if not args.no_degrid:
+    if not args.no_degrid and not chunks:
         model = torch.randn((d.n_pix, d.n_pix), dtype=torch.complex64, device=f"cuda:{local_rank}")
         pred = torch.empty_like(d.vis)
         e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
@@ -363,6 +393,8 @@ def main():
                  "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
 
     stage_names = ["bin", "grid", "fft_columns", "fft_rows_wcorrect"] if own else ["bin", "grid", "fft_cufft", "wcorrect"]
+    if chunks:
+        stage_names = ["zero", "bin_and_grid_%d_chunks" % len(chunks)] + stage_names[2:]
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
