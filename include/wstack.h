@@ -9,13 +9,19 @@
  *   ws_fft_wcorrect        a3 + a4 in one call: the library's own FFT with Eq. 2 fused into its last pass
  *   ws_wcorrect_accumulate a4: phase screen exp(2 pi i w_k (sqrt(1-l^2-m^2)-1)) times plane k, summed
  *                          over planes (PAPER.md:68 Eq. 2, :86)
- *   ws_dirty_image         a5: real part of the accumulated image
+ *   ws_dirty_image         a5: real part of the accumulated image, optionally normalised
+ *   ws_predict_planes,
+ *   ws_degrid_visibilities the opposite direction, image -> visibilities, the adjoint of the chain above
+ *
+ * Kernels: Gaussian or Kaiser-Bessel (:82, :459), both evaluated in registers.  Narrow-band data (one uvw
+ * per row shared by all channels, :207) can be pre-summed per row (WS_FLAG_PRESUM_CHANNELS).
  *
  * Conventions (DESIGN.md sections 2-3 give the readings R1-R16 of the paper behind them):
  *   - All data pointers are DEVICE pointers unless the argument is marked "host".  The caller owns every
  *     buffer and the stream; the library owns only the opaque plan.  Pointers must be 16-byte aligned.
  *   - Every call enqueues work on `stream` and returns; buffers must stay alive until the stream drains.
- *     Only ws_plan_create/destroy, ws_get_bins, ws_async_status and ws_image_from_host synchronise.
+ *     Only ws_plan_create/destroy, ws_get_bins, ws_get_occupancy, ws_get_sum_weights, ws_async_status and
+ *     ws_image_from_host synchronise.
  *   - Every call returns WS_OK (0) or a negative WS_ERR_* code; nothing throws, exits or prints.
  *     Arguments are validated before any launch.
  *   - Mesh ("grid") layout: complex64 [n_wplanes][n_pix][n_pix], u fastest, FFT-NATIVE storage order:
