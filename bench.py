@@ -342,6 +342,18 @@ def main():
         degrid_ms = {"predict_planes_wscreen_cufft": float(m[0]), "bin_and_gather": float(m[1]),
                      "mvis_per_s_degridding": d.n_vis / (m[1] * 1e-3) / 1e6,
                      "mvis_per_s_whole_prediction": d.n_vis / ((m[0] + m[1]) * 1e-3) / 1e6}
+        # the same prediction as ONE call: bins first, only the wanted column bands transformed (own column passes)
+        rows = []
+        for _ in range(4):
+            e[0].record()
+            plan.predict_visibilities(model, d.uvw, d.freqs_hz, d.n_chan, grid, pred, wsp)
+            e[1].record()
+            torch.cuda.synchronize()
+            rows.append(e[0].elapsed_time(e[1]))
+        plan.async_status()
+        one = float(np.median(rows[1:]))
+        degrid_ms["predict_visibilities_one_call"] = one
+        degrid_ms["mvis_per_s_one_call"] = d.n_vis / (one * 1e-3) / 1e6
         del model, pred
 
     # ---- roofline of the dominant own kernel -----------------------------------------

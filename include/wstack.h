@@ -41,7 +41,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 150
+#define WS_VERSION 160
 
 /* error codes */
 #define WS_OK 0
@@ -223,6 +223,13 @@ int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void
 int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_hz, int64_t n_rows, int32_t n_chan,
                            const void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
                            size_t workspace_bytes, void* stream);
+/* The two calls above as ONE, same result in vis_out (`planes` is scratch of ws_grid_bytes, its contents afterwards are
+ * private).  Where the library's own FFT exists (N = 2^8..2^13) the positions are binned FIRST, so that only the
+ * column bands of the planes that hold visibilities are transformed along v (the own column passes; along u: cuFFT),
+ * and the gather reads the column-transformed planes where those passes leave them.  Elsewhere it is the two calls. */
+int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float* uvw, const double* freq_hz, int64_t n_rows,
+                            int32_t n_chan, void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
+                            size_t workspace_bytes, void* stream);
 
 /* ---- the whole path from HOST buffers (end-to-end entry) ----------------------------------------------- */
 /* uvw_h, vis_h, weights_h, dirty_h are HOST pointers (pinned memory gives asynchronous copies); dev_inputs

@@ -244,7 +244,26 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->occ_sparse = false;
     int rc = make_fft_plan(plan);                       // ws_fft_planes is always the library's
     if (rc == WS_OK && plan->fft_own) rc = ws_fft_own_init(plan);
+    plan->fft_rows1d_ok = false;
+    plan->fft_rows1d_work = 0;
+    if (rc == WS_OK && plan->fft_own) {                 // degridding fast path: every row of the stack along u in one batch
+        long long n1[1] = {p->n_pix};
+        size_t work = 0;
+        cufftHandle h;
+        if (cufftCreate(&h) == CUFFT_SUCCESS) {
+            if (cufftSetAutoAllocation(h, 0) == CUFFT_SUCCESS &&
+                cufftMakePlanMany64(h, 1, n1, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C,
+                                    (long long)p->n_pix * (long long)p->n_wplanes, &work) == CUFFT_SUCCESS) {
+                plan->fft_rows1d = h;                   // (its work area, a few bytes per row, comes from the workspace's end)
+                plan->fft_rows1d_work = work;
+                plan->fft_rows1d_ok = true;
+            } else {
+                cufftDestroy(h);
+            }
+        }
+    }
     if (rc != WS_OK) {
+        if (plan->fft_rows1d_ok) cufftDestroy(plan->fft_rows1d);
         if (plan->fft_ok) cufftDestroy(plan->fft);
         if (plan->d_twiddles) cudaFree(plan->d_twiddles);
         if (plan->d_masks) cudaFree(plan->d_masks);
@@ -261,6 +280,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
 int ws_plan_destroy(ws_plan* plan) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (plan->fft_ok) cufftDestroy(plan->fft);
+    if (plan->fft_rows1d_ok) cufftDestroy(plan->fft_rows1d);
     if (plan->d_status) cudaFree(plan->d_status);
     if (plan->d_sumwt) cudaFree(plan->d_sumwt);
     if (plan->d_taper) cudaFree(plan->d_taper);
@@ -294,7 +314,8 @@ size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_f
     if (dup_factor > 4.0) dup_factor = 4.0;
     const uint64_t cap = (uint64_t)std::ceil((double)max_vis * dup_factor) + 64;
     const bool presum = (plan->prm.flags & WS_FLAG_PRESUM_CHANNELS) != 0;          // sized for n_chan = 1, the worst case
-    const size_t a = make_layout(plan, max_vis, cap, presum ? max_vis : 0).total + 4096;   // slack for fit_layout's alignment margin
+    const size_t a = make_layout(plan, max_vis, cap, presum ? max_vis : 0).total + 4096 +   // slack for fit_layout's alignment margin
+                     ws_align_up(plan->fft_rows1d_work, 256) + 256;                         // ws_predict_visibilities' row transforms
     return a > plan->fft_work_bytes ? a : plan->fft_work_bytes;
 }
 
@@ -474,7 +495,7 @@ int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void
     if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
         return fail(plan, WS_ERR_WORKSPACE, "ws_predict_planes: workspace smaller than ws_fft_workspace_bytes");
     if (plan->occ_grid == planes) plan->occ_grid = nullptr;      // no longer a mesh the gridder filled
-    const int rc = ws_launch_wscreen_fwd(plan, (const float2*)model_image, (float2*)planes, (cudaStream_t)stream);
+    const int rc = ws_launch_wscreen_fwd(plan, (const float2*)model_image, (float2*)planes, 0, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_predict_planes: launch failed");
     plan->launches += rc;
     return fft_planes_dir(plan, planes, workspace, workspace_bytes, stream, CUFFT_FORWARD);
@@ -495,8 +516,60 @@ int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_h
         cudaMemsetAsync(vis_out, 0, (size_t)n_rows * n_chan * 8, (cudaStream_t)stream) != cudaSuccess)   // dropped ones predict 0
         return fail(plan, WS_ERR_CUDA, "ws_degrid_visibilities: memset failed");
     rc = ws_launch_degrid(plan, plan->last_layout, (char*)workspace, (const float2*)planes, (float2*)vis_out, scale,
-                          accumulate, (cudaStream_t)stream);
+                          accumulate, -1, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_degrid_visibilities: launch failed");
+    plan->launches += rc;
+    return WS_OK;
+}
+
+int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float* uvw, const double* freq_hz, int64_t n_rows,
+                            int32_t n_chan, void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
+                            size_t workspace_bytes, void* stream) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (!plan->fft_own || !plan->fft_rows1d_ok) {      // the two library calls in sequence
+        const int rc = ws_predict_planes(plan, model_image, planes, workspace, workspace_bytes, stream);
+        if (rc != WS_OK) return rc;
+        return ws_degrid_visibilities(plan, uvw, freq_hz, n_rows, n_chan, planes, vis_out, scale, accumulate, workspace,
+                                      workspace_bytes, stream);
+    }
+    if (!model_image || !planes || (n_rows > 0 && !vis_out))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_visibilities: null pointer");
+    if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_visibilities: bad flag");
+    if (((uintptr_t)model_image | (uintptr_t)planes | (uintptr_t)vis_out) & 15)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_visibilities: pointers must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    // positions first: the bins say which column bands of the planes the gather will read
+    int rc = bin_impl(plan, uvw, nullptr, nullptr, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, false);
+    if (rc != WS_OK) return rc;
+    if (n_rows == 0) return WS_OK;
+    const WsLayout& L = plan->last_layout;
+    // the work area of the row transforms sits at the end of the workspace, behind the bins
+    const size_t w1 = ws_align_up(plan->fft_rows1d_work, 256);
+    if (L.total + w1 + 256 > workspace_bytes)
+        return fail(plan, WS_ERR_WORKSPACE, "ws_predict_visibilities: workspace too small (see ws_workspace_bytes)");
+    void* work1 = (char*)workspace + ((workspace_bytes - w1) & ~(size_t)255);
+    rc = ws_launch_fft_masks_degrid(plan, (const uint32_t*)((char*)workspace + L.off_counts_home), st);
+    if (rc < 0) return fail(plan, rc, "ws_predict_visibilities: launch failed");
+    plan->launches += rc;
+    plan->occ_grid = nullptr;                            // the masks no longer describe a gridded mesh
+    plan->occ_sparse = false;
+    // conj(M screen) -> inverse transforms (cuFFT along u, own column passes on the wanted bands) = conj(forward transform)
+    rc = ws_launch_wscreen_fwd(plan, (const float2*)model_image, (float2*)planes, 1, st);
+    if (rc < 0) return fail(plan, rc, "ws_predict_visibilities: launch failed");
+    plan->launches += rc;
+    if (cufftSetStream(plan->fft_rows1d, st) != CUFFT_SUCCESS ||
+        (plan->fft_rows1d_work > 0 && cufftSetWorkArea(plan->fft_rows1d, work1) != CUFFT_SUCCESS) ||
+        cufftExecC2C(plan->fft_rows1d, (cufftComplex*)planes, (cufftComplex*)planes, CUFFT_INVERSE) != CUFFT_SUCCESS)
+        return fail(plan, WS_ERR_CUFFT, "ws_predict_visibilities: cufftExecC2C");
+    rc = ws_launch_fft_cols(plan, (float2*)planes, true, st);
+    if (rc < 0) return fail(plan, rc, "ws_predict_visibilities: launch failed");
+    plan->launches += rc;
+    if (!accumulate && cudaMemsetAsync(vis_out, 0, (size_t)n_rows * n_chan * 8, st) != cudaSuccess)
+        return fail(plan, WS_ERR_CUDA, "ws_predict_visibilities: memset failed");
+    int lr0 = 0;
+    while ((256 << lr0) < plan->prm.n_pix) ++lr0;
+    rc = ws_launch_degrid(plan, L, (char*)workspace, (const float2*)planes, (float2*)vis_out, scale, accumulate, lr0, st);
+    if (rc < 0) return fail(plan, rc, "ws_predict_visibilities: launch failed");
     plan->launches += rc;
     return WS_OK;
 }

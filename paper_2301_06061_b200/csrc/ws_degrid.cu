@@ -22,18 +22,28 @@ constexpr int G = WS_WC_GROUP;
 // A thread owns two adjacent pixels; the phases over the planes are a geometric sequence, advanced by one complex
 // multiply per plane inside a block of G planes and restarted from an exactly reduced (fp64) phase per block.
 __global__ void __launch_bounds__(256)
-k_wscreen_fwd(const __grid_constant__ WcParams prm, const float4* __restrict__ image, float4* __restrict__ planes) {
+k_wscreen_fwd(const __grid_constant__ WcParams prm, const float2* __restrict__ image, float4* __restrict__ planes,
+              int conj_out, const uint32_t* __restrict__ orient) {
     const uint32_t N = (uint32_t)prm.n_pix, halfN = N >> 1, pairs = N >> 1;
     const uint64_t tid = (uint64_t)blockIdx.x * 256u + threadIdx.x;
     if (tid >= (uint64_t)N * pairs) return;
-    const uint32_t q = (uint32_t)(tid / pairs), p = (uint32_t)(tid - (uint64_t)q * pairs) * 2u;
-    const uint32_t sq = q >= halfN ? q - halfN : q + halfN;
-    const uint32_t sp = p >= halfN ? p - halfN : p + halfN;
+    // a: line of the stored plane, b, b + 1: the two adjacent cells of it.  [k][v][u]: a = q (m), b = p (l);
+    // transposed ([k][u][v], orient set): a = p, b = q -- the screen is symmetric in l and m, only the model is read across
+    const bool tr = orient && *orient;
+    const uint32_t a = (uint32_t)(tid / pairs), b = (uint32_t)(tid - (uint64_t)a * pairs) * 2u;
+    const uint32_t sa = a >= halfN ? a - halfN : a + halfN;
+    const uint32_t sb = b >= halfN ? b - halfN : b + halfN;
     const size_t plane_stride = (size_t)N * pairs;                 // in float4 units
-    float4* dst = planes + (size_t)sq * pairs + (sp >> 1);
-    float4 m = __ldcs(image + tid);
+    float4* dst = planes + (size_t)sa * pairs + (sb >> 1);
+    float4 m;
+    if (!tr) {
+        m = __ldcs((const float4*)image + tid);
+    } else {
+        const float2 m0 = __ldg(image + (size_t)b * N + a), m1 = __ldg(image + (size_t)(b + 1) * N + a);
+        m = make_float4(m0.x, m0.y, m1.x, m1.y);
+    }
     bool inA, inB;
-    const double tA = ws_n_minus_1(prm, (int)q, (int)p, &inA), tB = ws_n_minus_1(prm, (int)q, (int)p + 1, &inB);
+    const double tA = ws_n_minus_1(prm, (int)a, (int)b, &inA), tB = ws_n_minus_1(prm, (int)a, (int)b + 1, &inB);
     if (!inA) m.x = m.y = 0.f;                                      // R14
     if (!inB) m.z = m.w = 0.f;
     const float2 rA = ws_expi_turns(-prm.dw * tA), rB = ws_expi_turns(-prm.dw * tB);
@@ -45,7 +55,8 @@ k_wscreen_fwd(const __grid_constant__ WcParams prm, const float4* __restrict__ i
         for (int j = 0; j < G; ++j) {
             if (lo + j < nw) {
                 const float2 a = ws_cmul(make_float2(m.x, m.y), eA), b = ws_cmul(make_float2(m.z, m.w), eB);
-                __stcs(dst + (size_t)(lo + j) * plane_stride, make_float4(a.x, a.y, b.x, b.y));
+                __stcs(dst + (size_t)(lo + j) * plane_stride,
+                       conj_out ? make_float4(a.x, -a.y, b.x, -b.y) : make_float4(a.x, a.y, b.x, b.y));
                 eA = ws_cmul(eA, rA);
                 eB = ws_cmul(eB, rB);
             }
@@ -68,7 +79,7 @@ struct DgCfg {
 // visibility reads them, drop rule O3).
 template <int S>
 __device__ __forceinline__ void load_region(const WsGeom& g, const float2* __restrict__ planes, uint32_t bin, float2* region,
-                                            int lane) {
+                                            int lane, int xf_lr0, bool tr) {
     using C = DgCfg<S>;
     const uint32_t nt = (uint32_t)g.nt;
     const uint32_t tx = bin % nt, r = bin / nt;
@@ -78,12 +89,17 @@ __device__ __forceinline__ void load_region(const WsGeom& g, const float2* __res
     const float2* plane = planes + (size_t)k * (size_t)N * (size_t)N;
 #pragma unroll 8
     for (int idx = lane; idx < C::W * C::W; idx += 32) {     // independent loads: eight in flight per lane
-        const int ry = idx / C::W, rx = idx - ry * C::W;
+        const int i0 = idx / C::W, i1 = idx - i0 * C::W;     // consecutive lanes walk the stored line: x, or y if transposed
+        const int ry = tr ? i1 : i0, rx = tr ? i0 : i1;
         const int ly = y0 + ry, lx = x0 + rx;
         float2 v = make_float2(0.f, 0.f);
         if ((unsigned)ly < (unsigned)N && (unsigned)lx < (unsigned)N) {
             const int sy = ly >= half ? ly - half : ly + half, sx = lx >= half ? lx - half : lx + half;
-            v = __ldg(plane + (size_t)sy * N + sx);
+            int line = tr ? sx : sy;                         // the axis the column passes transformed
+            const int col = tr ? sy : sx;
+            if (xf_lr0 >= 0) line = ((line & ((1 << xf_lr0) - 1)) << 8) | (line >> xf_lr0);   // where ws_fft_columns left that frequency
+            v = __ldg(plane + (size_t)line * N + col);
+            if (xf_lr0 >= 0) v.y = -v.y;                     // ... of the conjugate transform
         }
         region[ry * C::P + rx] = v;
     }
@@ -147,12 +163,13 @@ __global__ void __launch_bounds__(DgCfg<S>::THREADS, 2)
 k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
          const uint4* __restrict__ items, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
          const float2* __restrict__ planes, float2* __restrict__ vis_out, float scale, int accumulate,
-         const WsStatus* __restrict__ status) {
+         const WsStatus* __restrict__ status, int xf_lr0, const uint32_t* __restrict__ orient) {
     using C = DgCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     float2* region = (float2*)(smem_raw + (size_t)wid * C::WARP_BYTES);
     if (status->overflow) return;
+    const bool tr = orient && *orient;           // planes stored [k][u][v] (ws_predict_visibilities may choose so)
     const uint32_t n_items = status->n_items;
     const uint32_t n_warps = gridDim.x * C::WARPS;
     const uint32_t gw = blockIdx.x * C::WARPS + wid;
@@ -164,7 +181,7 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
     auto do_item = [&]() {
         const uint4 w = items[it];
         it += n_warps;
-        load_region<S>(g, planes, w.x, region, lane);
+        load_region<S>(g, planes, w.x, region, lane, xf_lr0, tr);
         gather<S, KB>(g, records, perm, w.y, w.z, halo_start[w.x], region, vis_out, scale, accumulate, lane);
     };
 
@@ -176,7 +193,7 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
         ++since;
         const uint32_t s = bin_start[bin], e = bin_start[bin + 1];
         if (s == e || e - s > WS_CHUNK) continue;           // empty, or heavy: its chunks are items
-        load_region<S>(g, planes, bin, region, lane);
+        load_region<S>(g, planes, bin, region, lane, xf_lr0, tr);
         gather<S, KB>(g, records, perm, s, e, halo_start[bin], region, vis_out, scale, accumulate, lane);
     }
     while (it < n_items) do_item();
@@ -184,8 +201,9 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
 
 template <int S, bool KB>
 int launch_s(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale, int accumulate,
-             cudaStream_t st) {
+             int xf_lr0, cudaStream_t st) {
     using C = DgCfg<S>;
+    const uint32_t* orient = xf_lr0 >= 0 ? ws_fft_orientation_flag(plan) : nullptr;
     const size_t smem = C::WARP_BYTES * C::WARPS;
     // per device, and cheap: set on every launch rather than cached in a process-wide flag
     if (cudaFuncSetAttribute(k_degrid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return WS_ERR_CUDA;
@@ -197,14 +215,14 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, f
     k_degrid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(plan->geom, bin_start, halo_start, items,
                                                                   (const float4*)(ws + L.off_records),
                                                                   (const uint32_t*)(ws + L.off_perm), planes, vis_out, scale,
-                                                                  accumulate, plan->d_status);
+                                                                  accumulate, plan->d_status, xf_lr0, orient);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return rc + 1;
 }
 
 }  // namespace
 
-int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, cudaStream_t st) {
+int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, int conj_out, cudaStream_t st) {
     const ws_params& P = plan->prm;
     WcParams prm;
     prm.n_pix = P.n_pix;
@@ -213,18 +231,19 @@ int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, cu
     prm.dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
     prm.w0 = P.w_min + 0.5 * prm.dw;
     const uint64_t n_pairs = (uint64_t)P.n_pix * (uint64_t)(P.n_pix / 2);
-    k_wscreen_fwd<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(prm, (const float4*)image, (float4*)planes);
+    k_wscreen_fwd<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(prm, image, (float4*)planes, conj_out,
+                                                                     conj_out ? ws_fft_orientation_flag(plan) : nullptr);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;
 }
 
 int ws_launch_degrid(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale,
-                     int accumulate, cudaStream_t st) {
+                     int accumulate, int xf_lr0, cudaStream_t st) {
     const bool kb = plan->geom.kb_terms > 0;
 #define WS_DG_CASE(S_)                                                                                        \
     case S_:                                                                                                  \
-        return kb ? launch_s<S_, true>(plan, L, ws, planes, vis_out, scale, accumulate, st)                   \
-                  : launch_s<S_, false>(plan, L, ws, planes, vis_out, scale, accumulate, st);
+        return kb ? launch_s<S_, true>(plan, L, ws, planes, vis_out, scale, accumulate, xf_lr0, st)           \
+                  : launch_s<S_, false>(plan, L, ws, planes, vis_out, scale, accumulate, xf_lr0, st);
     switch (plan->geom.support) {
         WS_DG_CASE(1) WS_DG_CASE(3) WS_DG_CASE(5) WS_DG_CASE(7) WS_DG_CASE(9) WS_DG_CASE(11) WS_DG_CASE(13) WS_DG_CASE(15)
     }

@@ -204,6 +204,38 @@ k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_c
         if (!(atomicOr(band_mask + k * 8 + (bs >> 5), bit) & bit)) atomicAdd(masks + set, 1u);
     }
 }
+// Degridding (ws_degrid.cu): the planes are DENSE on the way in (rows of the model image times the w screen, transformed
+// along u) and only the column bands that hold visibilities -- or border on one that does: a footprint reaches S / 2
+// cells into the neighbour tile -- are wanted on the way out.  Such a band gets every class bit, all others none:
+// passes 1a / 1b then transform exactly those bands, whole.  bin_start: home counts per (plane, ty, tx), logical tiles.
+// As for a WS_GRID_SPARSE mesh the planes are private to the library and are laid out ([k][v][u] or [k][u][v]) so that
+// fewer bands are wanted.
+__global__ void __launch_bounds__(256)
+k_fft_masks_degrid(const uint32_t* __restrict__ bin_start, int nt, int r0, uint32_t n_kb, uint32_t set_words,
+                   uint32_t* __restrict__ masks) {
+    const uint32_t kb = blockIdx.x * 256u + threadIdx.x;      // k nt + band (storage order)
+    if (kb >= n_kb) return;
+    const int set = blockIdx.y;                               // 0: planes [k][v][u], a band is 32 adjacent u; 1: [k][u][v]
+    const int bs = kb % nt, k = kb / nt;
+    const int bl = (bs + nt / 2) & (nt - 1);                  // logical tile coordinate of the band
+    bool any = false;
+    for (int d = -1; d <= 1 && !any; ++d) {
+        const int x = bl + d;
+        if (x < 0 || x >= nt) continue;
+        for (int o = 0; o < nt && !any; ++o) {
+            const uint32_t bin = set == 0 ? ((uint32_t)k * nt + o) * nt + x : ((uint32_t)k * nt + x) * nt + o;
+            any = bin_start[bin + 1] > bin_start[bin];
+        }
+    }
+    if (!any) return;
+    uint32_t* class_mask = masks + MASK_CTRL + set * set_words;
+    uint32_t* band_mask = class_mask + n_kb * 8u;
+    const uint32_t full = r0 >= 32 ? 0xFFFFFFFFu : (1u << r0) - 1u;
+    for (int c = 0; c < 8; ++c) class_mask[kb * 8u + c] = full;
+    atomicOr(band_mask + k * 8 + (bs >> 5), 1u << (bs & 31));
+    atomicAdd(masks + set, 1u);
+}
+
 // the orientation of a WS_GRID_SPARSE mesh: transposed iff that leaves fewer bands (allow = 0: as the header says)
 __global__ void k_fft_orient(uint32_t* __restrict__ masks, int allow) { masks[2] = allow && masks[1] < masks[0] ? 1u : 0u; }
 
@@ -901,6 +933,18 @@ int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, int decide, cu
         ++launches;
     }
     return cudaGetLastError() == cudaSuccess ? launches : WS_ERR_CUDA;
+}
+
+// masks for the column passes of a degridding call (cleared first), for both orientations of the planes, and the choice
+int ws_launch_fft_masks_degrid(ws_plan* plan, const uint32_t* bin_start, cudaStream_t st) {
+    if (!plan->d_masks) return WS_ERR_UNSUPPORTED;
+    if (cudaMemsetAsync(plan->d_masks, 0, plan->mask_words * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
+    const int nt = plan->geom.nt, r0 = plan->prm.n_pix / 256;
+    const uint32_t n_kb = (uint32_t)plan->prm.n_wplanes * (uint32_t)nt;
+    k_fft_masks_degrid<<<dim3((n_kb + 255) / 256, 2), 256, 0, st>>>(bin_start, nt, r0, n_kb, (uint32_t)plan->mask_set_words,
+                                                                   (uint32_t*)plan->d_masks);
+    k_fft_orient<<<1, 1, 0, st>>>((uint32_t*)plan->d_masks, !(plan->prm.flags & WS_FLAG_NO_TRANSPOSE));   // fewer bands wins
+    return cudaGetLastError() == cudaSuccess ? 2 : WS_ERR_CUDA;
 }
 
 const uint32_t* ws_fft_orientation_flag(const ws_plan* plan) { return plan->d_masks ? (const uint32_t*)plan->d_masks + 2 : nullptr; }

@@ -77,6 +77,9 @@ struct ws_plan {
     int sm_count;
     cufftHandle fft;
     bool fft_ok;
+    cufftHandle fft_rows1d;                     // batched 1-D transforms along u of the whole stack (degridding fast path)
+    bool fft_rows1d_ok;
+    size_t fft_rows1d_work;                     // its work area (taken from the end of the caller's workspace)
     size_t fft_work_bytes;
     int fft_batch;                              // planes per cufftExec call
     int64_t launches;
@@ -112,9 +115,12 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);
 int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st);
-int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, cudaStream_t st);
+int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, int conj_out, cudaStream_t st);
+// xf_lr0 < 0: planes in natural (FFT-native) order; >= 0: log2(N / 256), the planes hold the CONJUGATE of the transform
+// with the rows where ws_fft_columns leaves them (frequency f at row ((f mod R0) << 8) | (f / R0))
 int ws_launch_degrid(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, float2* vis_out, float scale,
-                     int accumulate, cudaStream_t st);
+                     int accumulate, int xf_lr0, cudaStream_t st);
+int ws_launch_fft_masks_degrid(ws_plan* plan, const uint32_t* bin_start, cudaStream_t st);
 int ws_launch_sorted_keys(ws_plan* plan, const WsLayout& L, char* ws, cudaStream_t st);
 int ws_launch_wcorrect(ws_plan* plan, const float2* planes, float2* image, int accumulate, float* dirty,
                        cudaStream_t st);

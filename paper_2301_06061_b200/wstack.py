@@ -10,7 +10,7 @@ import torch
 
 from . import build as _build
 
-WS_VERSION = 150            # include/wstack.h
+WS_VERSION = 160            # include/wstack.h
 WS_GRID_ACCUMULATE = 0
 WS_GRID_OVERWRITE = 1
 WS_FLAG_LIBRARY_FFT = 1
@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count",
 ]
 
@@ -86,6 +86,7 @@ def lib():
         "ws_get_sum_weights": (C.c_int, [vp, C.POINTER(C.c_double), vp]),
         "ws_predict_planes": (C.c_int, [vp, vp, vp, vp, sz, vp]),
         "ws_degrid_visibilities": (C.c_int, [vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
+        "ws_predict_visibilities": (C.c_int, [vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
                                   C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
@@ -272,6 +273,17 @@ class Plan:
         self._check(lib().ws_degrid_visibilities(
             self._h, _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan, _dev(planes, torch.complex64, "planes"),
             _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+        self._ws = workspace
+
+    def predict_visibilities(self, model_image, uvw, freq_hz, n_chan: int, planes, vis_out, workspace, scale: float = 1.0,
+                             accumulate: bool = False, stream=None):
+        """Degridding in one call (`planes` is scratch): bins first, then only the wanted column bands are transformed."""
+        n_rows = int(uvw.shape[0])
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_predict_visibilities(
+            self._h, _dev(model_image, torch.complex64, "model_image"), _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan,
+            _dev(planes, torch.complex64, "planes"), _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
 

@@ -136,3 +136,53 @@ def test_predicted_point_sources_equal_eq1_on_the_gpu(oracle):
         ref += f * np.exp(-2j * np.pi * (uvw[:, 0] * l + uvw[:, 1] * m + wk * (math.sqrt(1 - l * l - m * m) - 1)))
     err = np.abs(vis.cpu().numpy()[:, 0] - ref).max() / 1.9
     assert err < 1e-5, err
+
+
+@pytest.mark.parametrize("support,kernel,n_pix", [(7, "gaussian", 256), (7, "kb", 512), (9, "kb", 256), (15, "kb", 256), (1, "gaussian", 256),
+                                                  (7, "kb", 128)])
+def test_predict_visibilities_one_call(oracle, support, kernel, n_pix):
+    """ws_predict_visibilities: bins first, only the wanted column bands transformed (own column passes), gather from
+    the column-transformed planes -- same visibilities as the oracle; the scratch stack is NaN-filled on entry.
+    n_pix = 128 has no own FFT: the call falls back to the two library calls.  A dataset squeezed into a corner of
+    the uv plane leaves most bands unwanted."""
+    d = make_random_dataset(800 + support, 5000, 3, n_pix, 5, support, wavelengths=False, fill=1.03, w_span=40.0,
+                            cell_rad=0.006 * 256 / n_pix)
+    d.uvw[:2500, :2] *= 0.15           # half of the rows in the centre: some planes / bands hold nothing else
+    plan, prm = _plan_and_prm(oracle, d, kernel)
+    M = _model(d, 4)
+    dev = d.to("cuda")
+    planes = plan.alloc_grid()
+    planes.fill_(float("nan"))
+    wsp = plan.alloc_workspace(max(d.n_vis, 1))
+    vis = torch.full((d.n_rows, d.n_chan), float("nan"), dtype=torch.complex64, device="cuda")
+    l0 = plan.launch_count()
+    plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, planes, vis, wsp)
+    plan.async_status()
+    # own FFT: binning (6) + masks + screen + two column passes + items + gather; library path: screen + binning + items + gather
+    assert plan.launch_count() - l0 >= (11 if plan.fft_is_own else 9) and (plan.fft_is_own or plan.launch_count() - l0 == 9)
+    ref = oracle.predict(prm, M, d.uvw.numpy(), d.n_chan, d.freqs_hz)
+    print("one-call degrid", support, kernel, n_pix, U.assert_close(vis.cpu().numpy(), ref, "predicted visibilities (one call)"))
+    # residual form
+    meas = dev.vis.clone()
+    plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, planes, meas, wsp, scale=-1.0, accumulate=True)
+    U.assert_close(d.vis.numpy().astype(np.complex128) - meas.cpu().numpy(), ref, "measured - residual (one call)")
+
+
+@pytest.mark.parametrize("axis,flags", [(0, 0), (1, 0), (1, 2)])
+def test_predict_visibilities_narrow_uv_coverage(oracle, axis, flags):
+    """All visibilities inside a narrow strip of u or of v: most column bands are unwanted and never transformed; the
+    library lays the planes out along whichever axis leaves fewer (strip in v: transposed, unless WS_FLAG_NO_TRANSPOSE)."""
+    d = make_random_dataset(850, 4000, 1, 512, 3, 7, fill=0.9, w_span=20.0, cell_rad=2e-3)
+    d.uvw[:, axis] *= 0.05
+    import paper_2301_06061_b200 as ws
+    _, prm = _plan_and_prm(oracle, d, "kb")
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, kernel_type=ws.WS_KERNEL_KAISER_BESSEL,
+                   kernel_param=prm.sigma, flags=flags)
+    M = _model(d, 5)
+    dev = d.to("cuda")
+    planes, wsp = plan.alloc_grid(), plan.alloc_workspace(d.n_vis)
+    planes.fill_(float("nan"))
+    vis = torch.empty_like(dev.vis)
+    plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, planes, vis, wsp)
+    U.assert_close(vis.cpu().numpy(), oracle.predict(prm, M, d.uvw.numpy(), 1, None), "narrow strip")
+    assert torch.isnan(torch.view_as_real(planes)).sum() == 0          # the screen kernel writes every cell
