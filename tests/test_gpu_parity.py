@@ -303,3 +303,29 @@ def test_channel_count_limits_and_single_plane(oracle):
     assert e.value.code == -2
     d = make_random_dataset(702, 2000, 7, 256, 3, 5, wavelengths=False, fill=0.9, w_span=15.0, cell_rad=2e-3)
     _full_check(oracle, d)
+
+
+@pytest.mark.parametrize("n_pix", [256, 128])
+def test_image_from_host_equals_oracle(oracle, n_pix):
+    """The end-to-end entry bench.py times (host buffers in, host dirty image out): own FFT (n_pix = 256) and the
+    library path (128).  Pinned and pageable host memory both work."""
+    d = make_random_dataset(900 + n_pix, 6000, 2, n_pix, 5, 7, wavelengths=False, fill=1.02, w_span=30.0, cell_rad=0.5 / n_pix)
+    plan = U.make_plan(d)
+    prm = U.oracle_params(oracle, d, 32)
+    D = oracle.dirty_image(prm, *_np(d))
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis)
+    dev_in = torch.empty(12 * d.n_rows + 12 * d.n_vis + 256, dtype=torch.uint8, device="cuda")
+    for pin in (True, False):
+        uvw_h, vis_h, wt_h = (t.pin_memory() if pin else t.clone() for t in (d.uvw, d.vis, d.weights))
+        dirty_h = torch.full((n_pix, n_pix), float("nan"), dtype=torch.float32)
+        if pin:
+            dirty_h = dirty_h.pin_memory()
+        grid.fill_(float("nan"))
+        plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+        plan.async_status()
+        ref = D.real
+        rel = np.linalg.norm(dirty_h.numpy() - ref) / np.linalg.norm(ref)
+        mx = np.abs(dirty_h.numpy() - ref).max() / np.abs(D).max()
+        assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL, (pin, rel, mx)
+        assert np.array_equal(dirty_h.numpy(), dirty.cpu().numpy())
