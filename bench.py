@@ -425,7 +425,7 @@ def main():
     if not args.no_e2e:
         uvw_h, vis_h, wt_h = (t.cpu().pin_memory() for t in (d.uvw, d.vis, d.weights))
         dirty_h = torch.empty((d.n_pix, d.n_pix), dtype=torch.float32).pin_memory()
-        dev_in = torch.empty(12 * d.n_rows + 12 * d.n_vis + 256, dtype=torch.uint8, device=f"cuda:{local_rank}")
+        dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device=f"cuda:{local_rank}")
         k_e2e = max(2, min(args.steps, 5))
         plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
         torch.cuda.synchronize()

@@ -41,7 +41,7 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 160
+#define WS_VERSION 200
 
 /* error codes */
 #define WS_OK 0
@@ -233,9 +233,13 @@ int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float*
 
 /* ---- the whole path from HOST buffers (end-to-end entry) ----------------------------------------------- */
 /* uvw_h, vis_h, weights_h, dirty_h are HOST pointers (pinned memory gives asynchronous copies); dev_inputs
- * is a device scratch of at least 12 n_rows + 12 n_rows n_chan + 64 bytes; grid, image, dirty_d, workspace
- * are device buffers as above.  Copies the inputs in, runs a1..a5 with WS_GRID_OVERWRITE, copies the dirty
- * image out and synchronises the stream. */
+ * is a 16-byte aligned device scratch of at least ws_dev_inputs_bytes(n_rows, n_chan) bytes (uvw | vis | weights,
+ * each padded to 16 bytes); grid, image, dirty_d, workspace are device buffers as above.  Copies the inputs in,
+ * runs a1..a5 (own FFT: WS_GRID_SPARSE + WS_FFT_USE_OCCUPANCY, so `grid` is private scratch whose empty tiles are
+ * never written; library FFT: WS_GRID_OVERWRITE), copies the dirty image out, synchronises the stream and returns
+ * the deferred status (WS_ERR_WORKSPACE if the record capacity of `workspace` was exceeded: dirty_h is then
+ * meaningless). */
+size_t ws_dev_inputs_bytes(int64_t n_rows, int32_t n_chan);
 int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, const float* weights_h,
                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
                        size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,

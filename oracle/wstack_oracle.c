@@ -105,10 +105,10 @@ static int orc_place(const orc_params *p, double u, double v, double w, double s
     double ck = floor(pw);                /* N_w equal bins over [w_min, w_max] (R6) */
     if (ck < 0.0) ck = 0.0;
     if (ck > (double)(p->n_wplanes - 1)) ck = (double)(p->n_wplanes - 1);
-    *k = (int32_t)ck;
-    /* drop rule O3 (R5): the whole S x S footprint must lie on the mesh */
+    *k = pw == pw ? (int32_t)ck : 0;
+    /* drop rule O3 (R5): the whole S x S footprint must lie on the mesh; a NaN coordinate drops too (R33) */
     if (!(ci >= (double)h && ci <= (double)(p->n_pix - 1 - h) &&
-          cj >= (double)h && cj <= (double)(p->n_pix - 1 - h))) {
+          cj >= (double)h && cj <= (double)(p->n_pix - 1 - h) && pw == pw)) {
         *i0 = *j0 = -1; *fu = *fv = 0.0;
         return 0;
     }

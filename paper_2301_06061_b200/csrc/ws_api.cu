@@ -51,10 +51,10 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity, 
 }
 
 // Largest record capacity whose layout fits into `bytes` (0 if even the fixed part does not fit).
-bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out, int64_t presum_rows = 0) {
+bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out, int64_t presum_rows = 0, int max_dup = 4) {
     WsLayout L0 = make_layout(plan, n_vis, 0, presum_rows);
     if (L0.total > bytes) return false;
-    const uint64_t want = (uint64_t)n_vis * 4;                      // worst case: every footprint in 4 tiles
+    const uint64_t want = (uint64_t)n_vis * (uint64_t)max_dup;      // worst case: every footprint in 4 tiles (home lists only: 1)
     const size_t spare = bytes - L0.total;
     // per record: 16 B + 32/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
     uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 32.0 / WS_CHUNK)) : 0;
@@ -352,7 +352,9 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
     const int64_t n_vis = presum ? n_rows : n_rows * n_chan;
     const int32_t n_chan_in = n_chan;
     WsLayout L;
-    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0) || (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
+    // positions only (degridding): home records alone, so that the rest of the workspace stays free for the caller's use
+    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0, with_values ? 4 : 1) ||
+        (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
         return fail(plan, WS_ERR_WORKSPACE, "ws_bin_visibilities: workspace too small (see ws_workspace_bytes_for)");
     const void* vis_in = vis;
     const float* wt_in = weights;
@@ -661,6 +663,12 @@ int ws_get_sum_weights(ws_plan* plan, double* sum_weights, void* stream) {
     return WS_OK;
 }
 
+size_t ws_dev_inputs_bytes(int64_t n_rows, int32_t n_chan) {
+    if (n_rows < 0 || n_chan <= 0) return 0;
+    const size_t n_vis = (size_t)n_rows * (size_t)n_chan;
+    return ws_align_up((size_t)n_rows * 12, 16) + ws_align_up(n_vis * 8, 16) + ws_align_up(n_vis * 4, 16);
+}
+
 int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, const float* weights_h,
                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
                        size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,
@@ -671,8 +679,10 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
     if (n_rows <= 0 || n_chan <= 0 || n_rows * n_chan > MAX_VIS)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: bad sizes");
     const size_t n_vis = (size_t)n_rows * n_chan;
-    const size_t b_uvw = ws_align_up((size_t)n_rows * 12, 16), b_vis = n_vis * 8, b_wt = n_vis * 4;
+    // every sub-buffer starts on a 16-byte boundary (bin_impl's alignment rule): uvw | vis | weights
+    const size_t b_uvw = ws_align_up((size_t)n_rows * 12, 16), b_vis = ws_align_up(n_vis * 8, 16), b_wt = n_vis * 4;
     if (dev_inputs_bytes < b_uvw + b_vis + b_wt) return fail(plan, WS_ERR_WORKSPACE, "ws_image_from_host: dev_inputs too small");
+    if ((uintptr_t)dev_inputs & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: dev_inputs must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
     char* d = (char*)dev_inputs;
     float* uvw_d = (float*)d;
@@ -680,7 +690,7 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
     float* wt_d = (float*)(d + b_uvw + b_vis);
     cudaError_t e;
     if ((e = cudaMemcpyAsync(uvw_d, uvw_h, (size_t)n_rows * 12, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(vis_d, vis_h, b_vis, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(vis_d, vis_h, n_vis * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(wt_d, weights_h, b_wt, cudaMemcpyHostToDevice, st)) != cudaSuccess)
         return cuda_fail(plan, e, "ws_image_from_host: H2D copy");
     // the mesh is never cleared nor completely written where the own FFT can skip what the gridder left empty
@@ -692,8 +702,8 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
         return rc;
     if ((e = cudaMemcpyAsync(dirty_h, dirty_d, ws_dirty_bytes(plan), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(plan, e, "ws_image_from_host: D2H copy");
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(plan, e, "ws_image_from_host: synchronize");
-    return WS_OK;
+    // synchronises and reads the deferred status: a record overflow means the gridder was skipped and dirty_h is garbage
+    return ws_async_status(plan, stream);
 }
 
 int ws_async_status(ws_plan* plan, void* stream) {

@@ -1,8 +1,8 @@
 // a1: binning of the visibilities by (w-plane, uv-tile)  --  PAPER.md:78 (sub-step 1, the per-region lists of
 // visibilities), :144-150 (bucketing then gather into contiguous arrays).  The paper builds linked lists on the
-// CPU; here it is a radix-2^b counting sort on the device: histogram over all bins (one digit = the whole
-// key), exclusive prefix scan (warp shuffles), and a scatter that writes, per bin, contiguous 16-byte records
-// the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
+// CPU; here it is a one-digit counting sort on the device (the whole key is the digit; the order INSIDE a bin is
+// unspecified, R19): histogram over all bins, exclusive prefix scan (warp shuffles), and a scatter that
+// writes, per bin, contiguous 16-byte records the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
 // it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
 #include <algorithm>
 
@@ -32,7 +32,7 @@ __device__ __forceinline__ bool place(const WsChanConsts& cc, const WsGeom& g, f
     const double ktop = (double)(g.n_wplanes - 1);
     ck = ck > ktop ? ktop : ck;
     const double lo = (double)g.halo, hi = (double)(g.n_pix - 1 - g.halo);
-    if (!(ci >= lo && ci <= hi && cj >= lo && cj <= hi)) return false;   // drop rule O3 (R5); NaN drops
+    if (!(ci >= lo && ci <= hi && cj >= lo && cj <= hi && pw == pw)) return false;   // drop rule O3 (R5); a NaN in u, v or w drops (R33)
     o.k = (int)ck;
     o.i0 = (int)ci;
     o.j0 = (int)cj;

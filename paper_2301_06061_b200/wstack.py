@@ -10,7 +10,7 @@ import torch
 
 from . import build as _build
 
-WS_VERSION = 160            # include/wstack.h
+WS_VERSION = 200            # include/wstack.h
 WS_GRID_ACCUMULATE = 0
 WS_GRID_OVERWRITE = 1
 WS_FLAG_LIBRARY_FFT = 1
@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count",
 ]
 
@@ -87,6 +87,7 @@ def lib():
         "ws_predict_planes": (C.c_int, [vp, vp, vp, vp, sz, vp]),
         "ws_degrid_visibilities": (C.c_int, [vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
         "ws_predict_visibilities": (C.c_int, [vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
+        "ws_dev_inputs_bytes": (sz, [i64, i32]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
                                   C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
@@ -291,6 +292,10 @@ class Plan:
         v = C.c_double()
         self._check(lib().ws_get_sum_weights(self._h, C.byref(v), _stream(stream)))
         return v.value
+
+    @staticmethod
+    def dev_inputs_bytes(n_rows: int, n_chan: int) -> int:
+        return int(lib().ws_dev_inputs_bytes(n_rows, n_chan))
 
     def image_from_host(self, uvw_h, vis_h, weights_h, freq_hz, dev_inputs, grid, image, dirty_d, dirty_h, workspace,
                         stream=None):

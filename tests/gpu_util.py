@@ -81,7 +81,9 @@ def assert_close(x, ref, what):
 
 
 def check_bins(oracle, prm, d, bins):
-    """Bit-exact: keys, sorted keys, bin_start, n_dropped; perm per bin as a set (order inside a bin is unspecified)."""
+    """Bit-exact: keys, bin_start, n_dropped; perm per bin as a set (order inside a bin is unspecified).  The device
+    expands `sorted_keys` from `bin_start` (k_sorted_keys), so its comparison repeats the bin_start one: the independent
+    statements are keys, bin_start and the per-bin sets of perm."""
     pos = oracle.positions(prm, d.uvw.numpy(), d.n_chan, d.freqs_hz)
     assert np.array_equal(bins["keys"], pos["key"]), "keys differ from the oracle"
     bin_start, perm, dropped = oracle.bins(prm, pos["key"])

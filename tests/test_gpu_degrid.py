@@ -186,3 +186,21 @@ def test_predict_visibilities_narrow_uv_coverage(oracle, axis, flags):
     plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, planes, vis, wsp)
     U.assert_close(vis.cpu().numpy(), oracle.predict(prm, M, d.uvw.numpy(), 1, None), "narrow strip")
     assert torch.isnan(torch.view_as_real(planes)).sum() == 0          # the screen kernel writes every cell
+
+
+def test_predict_visibilities_with_the_least_documented_workspace(oracle):
+    """ws_workspace_bytes_for(dup_factor = 1.0) is enough for the one-call prediction: its binning stores home records
+    only and leaves the tail of the workspace to the row transforms' work area."""
+    d = make_random_dataset(321, 5000, 2, 512, 4, 7, wavelengths=False, fill=0.9, w_span=40.0, cell_rad=1e-3)
+    plan = U.make_plan(d)
+    dev = d.to("cuda")
+    prm = U.oracle_params(oracle, d, plan.tile)
+    rng = np.random.default_rng(3)
+    M = (rng.standard_normal((512, 512)) + 1j * rng.standard_normal((512, 512))).astype(np.complex64)
+    ref = oracle.predict(prm, M.astype(np.complex128), d.uvw.numpy(), d.n_chan, d.freqs_hz)
+    planes = plan.alloc_grid()
+    pred = torch.full_like(dev.vis, float("nan"))
+    wsp = plan.alloc_workspace(d.n_vis, dup_factor=1.0)
+    plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, planes, pred, wsp)
+    plan.async_status()
+    U.assert_close(pred.cpu().numpy(), ref, "one-call prediction, dup_factor 1.0 workspace")

@@ -103,8 +103,7 @@ def _sampled_check(oracle, cfg_name, planes_to_check, n_pix_samples, chunks=1):
     assert np.isfinite(img).all()
 
 
-def test_large_config_sampled(oracle):
-    _sampled_check(oracle, "large", planes_to_check=(31, 5), n_pix_samples=24)
+# (Large as a whole -- all 64 planes of the mesh, the whole image, every bin -- is in test_gpu_wholearray.py.)
 
 
 @pytest.mark.skipif(os.environ.get("WS_SKIP_EXTREME") == "1", reason="WS_SKIP_EXTREME=1")

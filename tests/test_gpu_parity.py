@@ -305,17 +305,18 @@ def test_channel_count_limits_and_single_plane(oracle):
     _full_check(oracle, d)
 
 
-@pytest.mark.parametrize("n_pix", [256, 128])
-def test_image_from_host_equals_oracle(oracle, n_pix):
+@pytest.mark.parametrize("n_pix,n_rows,n_chan", [(256, 6000, 2), (128, 6000, 2), (256, 4037, 3), (256, 1, 1)])
+def test_image_from_host_equals_oracle(oracle, n_pix, n_rows, n_chan):
     """The end-to-end entry bench.py times (host buffers in, host dirty image out): own FFT (n_pix = 256) and the
-    library path (128).  Pinned and pageable host memory both work."""
-    d = make_random_dataset(900 + n_pix, 6000, 2, n_pix, 5, 7, wavelengths=False, fill=1.02, w_span=30.0, cell_rad=0.5 / n_pix)
+    library path (128).  Pinned and pageable host memory both work; an odd number of visibilities (4037 x 3) leaves the
+    weights 8 bytes off a 16-byte boundary unless every sub-buffer of dev_inputs is padded."""
+    d = make_random_dataset(900 + n_pix, n_rows, n_chan, n_pix, 5, 7, wavelengths=False, fill=1.02, w_span=30.0, cell_rad=0.5 / n_pix)
     plan = U.make_plan(d)
     prm = U.oracle_params(oracle, d, 32)
     D = oracle.dirty_image(prm, *_np(d))
     grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
     wsp = plan.alloc_workspace(d.n_vis)
-    dev_in = torch.empty(12 * d.n_rows + 12 * d.n_vis + 256, dtype=torch.uint8, device="cuda")
+    dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device="cuda")
     for pin in (True, False):
         uvw_h, vis_h, wt_h = (t.pin_memory() if pin else t.clone() for t in (d.uvw, d.vis, d.weights))
         dirty_h = torch.full((n_pix, n_pix), float("nan"), dtype=torch.float32)
@@ -329,3 +330,35 @@ def test_image_from_host_equals_oracle(oracle, n_pix):
         mx = np.abs(dirty_h.numpy() - ref).max() / np.abs(D).max()
         assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL, (pin, rel, mx)
         assert np.array_equal(dirty_h.numpy(), dirty.cpu().numpy())
+
+
+def test_image_from_host_reports_record_overflow(oracle):
+    """A workspace sized for fewer records than the data produce: the end-to-end entry must say so, not return an image."""
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(14, 2000, 1, 256, 1, 7, fill=0.9)
+    d.uvw[:, :2] = torch.round(d.uvw[:, :2] * (256 * d.cell_rad) / 32) * 32 / (256 * d.cell_rad)   # tile corners: 4 records each
+    plan = U.make_plan(d)
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis, dup_factor=1.0)
+    dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device="cuda")
+    dirty_h = torch.empty((256, 256), dtype=torch.float32)
+    with pytest.raises(ws.WStackError) as e:
+        plan.image_from_host(d.uvw, d.vis, d.weights, None, dev_in, grid, image, dirty, dirty_h, wsp)
+    assert e.value.code == -3
+
+
+def test_nan_coordinates_are_dropped_on_the_gpu(oracle):
+    """DESIGN.md R33: NaN in u, v or w drops the visibility (it used to land in plane 0); +-Inf in w clamps (R6)."""
+    d = make_random_dataset(77, 3000, 2, 256, 4, 7, wavelengths=False, fill=0.9, w_span=20.0, cell_rad=2e-3)
+    d.uvw[5, 0] = float("nan")
+    d.uvw[6, 1] = float("nan")
+    d.uvw[7, 2] = float("nan")
+    d.uvw[8, 2] = float("inf")
+    d.uvw[9, 2] = float("-inf")
+    out = U.run_chain(d)
+    prm = U.oracle_params(oracle, d, out["plan"].tile)
+    U.check_bins(oracle, prm, d, out["bins"])
+    assert out["bins"]["n_dropped"] >= 6
+    D, G = oracle.dirty_image(prm, *_np(d), return_grid=True)
+    U.assert_close(out["grid"], G, "grid with NaN rows")
+    U.assert_close(out["image"], D, "image with NaN rows")

@@ -97,6 +97,36 @@ def test_p9_positions_and_keys_exact_rational(oracle):
     assert n_checked == d.n_vis and 0 < n_dropped < d.n_vis // 4
 
 
+def test_nan_coordinates_are_dropped(oracle):
+    """DESIGN.md R33: a visibility with a NaN in u, v or w is dropped (key 0xFFFFFFFF, no contribution); +-Inf in w
+    clamps into the first / last plane like any w outside [w_min, w_max] (R6).  Pinned by construction: the mesh of the
+    data with such rows inserted equals the mesh of the data without them (+ the clamped ones added by hand)."""
+    d = _small(seed=15, n_rows=300, n_chan=2, n_pix=128, n_w=4, fill=0.8)
+    prm = _prm(oracle, d, tile=32)
+    uvw, vis, wt = d.uvw.numpy().copy(), d.vis.numpy(), d.weights.numpy()
+    clean = oracle.grid(prm, uvw, vis, wt, d.freqs_hz)
+    bad = uvw.copy()
+    bad[3, 0] = np.nan
+    bad[7, 1] = np.nan
+    bad[11, 2] = np.nan
+    bad[20, 2] = np.inf
+    bad[21, 2] = -np.inf
+    pos = oracle.positions(prm, bad, d.n_chan, d.freqs_hz)
+    key = pos["key"].reshape(d.n_rows, d.n_chan)
+    assert np.all(key[[3, 7, 11]] == 0xFFFFFFFF)
+    assert np.all(pos["k"].reshape(d.n_rows, d.n_chan)[20] == prm.n_wplanes - 1) and np.all(pos["k"].reshape(d.n_rows, d.n_chan)[21] == 0)
+    ok = np.ones(d.n_rows, bool)
+    ok[[3, 7, 11]] = False
+    ref_uvw = uvw[ok].copy()
+    sel = np.flatnonzero(ok)
+    ref_uvw[np.searchsorted(sel, 20), 2] = 1e30          # far beyond w_max: clamps into the last plane
+    ref_uvw[np.searchsorted(sel, 21), 2] = -1e30
+    want = oracle.grid(prm, ref_uvw, vis[ok], wt[ok], d.freqs_hz)
+    got = oracle.grid(prm, bad, vis, wt, d.freqs_hz)
+    assert np.array_equal(got, want) and not np.array_equal(got, clean)
+    assert oracle.sum_weights(prm, bad, wt, d.freqs_hz) == pytest.approx(float(wt[ok].astype(np.float64).sum()), rel=1e-12)
+
+
 def test_p9_bins_are_a_stable_counting_sort(oracle):
     d = _small(seed=12, n_rows=5000, n_chan=2, n_pix=128, n_w=3, fill=1.02)
     prm = _prm(oracle, d, tile=32)
