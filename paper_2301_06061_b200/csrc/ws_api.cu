@@ -761,14 +761,17 @@ int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* band
     const bool tr = all[2] != 0;
     const uint32_t* m = all.data() + 8 + (tr ? plan->mask_set_words : 0);      // the set of the orientation in use
     const size_t nw = (size_t)plan->prm.n_wplanes, nt = (size_t)plan->geom.nt, n_class = nw * nt * 8;
+    const size_t cw = (size_t)plan->mask_class_words, bw = (size_t)plan->mask_band_words;
     size_t t = 0, c = 0, b = 0, p = 0;
     for (size_t i = 0; i < n_class; ++i) {
-        t += (size_t)__builtin_popcount(m[i]);
-        c += m[i] != 0;
+        size_t bits = 0;
+        for (size_t j = 0; j < cw; ++j) bits += (size_t)__builtin_popcount(m[i * cw + j]);
+        t += bits;
+        c += bits != 0;
     }
     for (size_t k = 0; k < nw; ++k) {
         size_t nb = 0;
-        for (int i = 0; i < 8; ++i) nb += (size_t)__builtin_popcount(m[n_class + k * 8 + i]);
+        for (size_t i = 0; i < bw; ++i) nb += (size_t)__builtin_popcount(m[n_class * cw + k * bw + i]);
         b += nb;
         p += nb != 0;
     }

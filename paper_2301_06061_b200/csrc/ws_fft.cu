@@ -51,6 +51,7 @@ __host__ __device__ constexpr int log2r(int logn, int s) {
         case 11: return s < 2 ? 4 : 3;                      // 16 16 8
         case 12: return 4;                                  // 16 16 16
         case 13: return s == 0 ? 5 : 4;                     // 32 16 16 (the radix-32 butterflies are split over two threads)
+        case 14: return s == 0 ? 6 : 4;                     // 64 16 16 (radix 64 split over two threads of each of two CTAs)
     }
     return 0;
 }
@@ -67,6 +68,10 @@ __host__ __device__ constexpr int tw_offset(int logn, int s) {
     return o;
 }
 __host__ __device__ constexpr int tw_entries(int logn) { return tw_offset(logn, n_stages(logn) - 1); }   // last stage: Q = 1, none
+// what of it the row kernel keeps in shared memory: everything, except for N = 16384, whose first-stage twiddles are
+// thread constants held in registers (the 128 KB landing buffer leaves no room for a table): only stage 1 then
+__host__ __device__ constexpr int tw_smem_entries(int logn) { return logn == 14 ? tw_entries(logn) - tw_offset(logn, 1) : tw_entries(logn); }
+__host__ __device__ constexpr int tw_smem_off1(int logn) { return logn == 14 ? 0 : tw_offset(logn, 1); }
 
 __host__ __device__ constexpr int brev(int i, int bits) {
     int r = 0;
@@ -147,6 +152,77 @@ __device__ __forceinline__ E mul_w32(E a, int k) {
     }
 }
 
+// a * exp(+2 pi i k / 64), k = 0..63 a compile-time constant after unrolling (radix-64 first stage, N = 16384)
+__device__ __forceinline__ float2 mul_w64(float2 a, int k) {
+    switch (k & 63) {
+        case 0: return a;
+        case 1: return emul(a, 0.99518472667219693f, 0.098017140329560604f);
+        case 2: return emul(a, 0.98078528040323043f, 0.19509032201612825f);
+        case 3: return emul(a, 0.95694033573220882f, 0.29028467725446233f);
+        case 4: return emul(a, 0.92387953251128674f, 0.38268343236508978f);
+        case 5: return emul(a, 0.88192126434835505f, 0.47139673682599764f);
+        case 6: return emul(a, 0.83146961230254524f, 0.55557023301960218f);
+        case 7: return emul(a, 0.77301045336273699f, 0.63439328416364549f);
+        case 8: return escale(emul_1pi(a), 0.70710678118654752f);
+        case 9: return emul(a, 0.63439328416364549f, 0.77301045336273699f);
+        case 10: return emul(a, 0.55557023301960229f, 0.83146961230254524f);
+        case 11: return emul(a, 0.47139673682599781f, 0.88192126434835494f);
+        case 12: return emul(a, 0.38268343236508984f, 0.92387953251128674f);
+        case 13: return emul(a, 0.29028467725446233f, 0.95694033573220894f);
+        case 14: return emul(a, 0.19509032201612833f, 0.98078528040323043f);
+        case 15: return emul(a, 0.09801714032956077f, 0.99518472667219682f);
+        case 16: return emul_i(a);
+        case 17: return emul(a, -0.098017140329560645f, 0.99518472667219693f);
+        case 18: return emul(a, -0.19509032201612819f, 0.98078528040323043f);
+        case 19: return emul(a, -0.29028467725446216f, 0.95694033573220894f);
+        case 20: return emul(a, -0.38268343236508973f, 0.92387953251128674f);
+        case 21: return emul(a, -0.4713967368259977f, 0.88192126434835505f);
+        case 22: return emul(a, -0.55557023301960196f, 0.83146961230254546f);
+        case 23: return emul(a, -0.63439328416364538f, 0.7730104533627371f);
+        case 24: return escale(emul_m1pi(a), 0.70710678118654752f);
+        case 25: return emul(a, -0.77301045336273699f, 0.63439328416364549f);
+        case 26: return emul(a, -0.83146961230254535f, 0.55557023301960218f);
+        case 27: return emul(a, -0.88192126434835494f, 0.47139673682599786f);
+        case 28: return emul(a, -0.92387953251128674f, 0.38268343236508989f);
+        case 29: return emul(a, -0.95694033573220882f, 0.29028467725446239f);
+        case 30: return emul(a, -0.98078528040323043f, 0.19509032201612861f);
+        case 31: return emul(a, -0.99518472667219682f, 0.098017140329560826f);
+        case 32: return make_float2(-a.x, -a.y);
+        case 33: return emul(a, -0.99518472667219693f, -0.09801714032956059f);
+        case 34: return emul(a, -0.98078528040323043f, -0.19509032201612836f);
+        case 35: return emul(a, -0.95694033573220894f, -0.29028467725446211f);
+        case 36: return emul(a, -0.92387953251128685f, -0.38268343236508967f);
+        case 37: return emul(a, -0.88192126434835505f, -0.47139673682599764f);
+        case 38: return emul(a, -0.83146961230254546f, -0.55557023301960196f);
+        case 39: return emul(a, -0.7730104533627371f, -0.63439328416364527f);
+        case 40: return emul(a, -0.70710678118654768f, -0.70710678118654746f);
+        case 41: return emul(a, -0.63439328416364593f, -0.77301045336273666f);
+        case 42: return emul(a, -0.55557023301960218f, -0.83146961230254524f);
+        case 43: return emul(a, -0.47139673682599786f, -0.88192126434835494f);
+        case 44: return emul(a, -0.38268343236509034f, -0.92387953251128652f);
+        case 45: return emul(a, -0.29028467725446244f, -0.95694033573220882f);
+        case 46: return emul(a, -0.19509032201612866f, -0.98078528040323032f);
+        case 47: return emul(a, -0.098017140329560451f, -0.99518472667219693f);
+        case 48: return make_float2(a.y, -a.x);
+        case 49: return emul(a, 0.09801714032956009f, -0.99518472667219693f);
+        case 50: return emul(a, 0.1950903220161283f, -0.98078528040323043f);
+        case 51: return emul(a, 0.29028467725446205f, -0.95694033573220894f);
+        case 52: return emul(a, 0.38268343236509f, -0.92387953251128663f);
+        case 53: return emul(a, 0.47139673682599759f, -0.88192126434835505f);
+        case 54: return emul(a, 0.55557023301960184f, -0.83146961230254546f);
+        case 55: return emul(a, 0.6343932841636456f, -0.77301045336273688f);
+        case 56: return emul(a, 0.70710678118654735f, -0.70710678118654768f);
+        case 57: return emul(a, 0.77301045336273666f, -0.63439328416364593f);
+        case 58: return emul(a, 0.83146961230254524f, -0.55557023301960218f);
+        case 59: return emul(a, 0.88192126434835483f, -0.47139673682599792f);
+        case 60: return emul(a, 0.92387953251128652f, -0.38268343236509039f);
+        case 61: return emul(a, 0.95694033573220882f, -0.2902846772544625f);
+        case 62: return emul(a, 0.98078528040323032f, -0.19509032201612872f);
+        case 63: return emul(a, 0.99518472667219693f, -0.098017140329560506f);
+    }
+    return a;
+}
+
 // In-register inverse DFT of R = 2^LOGR points, decimation in frequency: on return x[i] = Y[brev(i)],
 // Y[m'] = sum_m x[m] exp(+2 pi i m m' / R).
 template <typename E, int LOGR, bool PACKED = true>
@@ -177,6 +253,10 @@ __device__ __forceinline__ void bfly(E* x) {
 // Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; set = class masks, band masks.
 // Masks are OR-ed into (chunked gridding accumulates); ws_fft_masks_clear zeroes them.
 constexpr int MASK_CTRL = 8;
+// Words per class mask (one bit per input of pass 1a's radix-R0 butterfly: R0 = 64 for N = 16384 needs two) and band
+// words per plane (one bit per 32-column band: 512 bands for N = 16384).
+__host__ __device__ constexpr int class_words(int r0) { return r0 > 32 ? 2 : 1; }
+__host__ __device__ constexpr int band_words(int nt) { return nt > 256 ? nt / 32 : 8; }
 __device__ __forceinline__ const uint32_t* mask_set(const uint32_t* __restrict__ masks, uint32_t set_words) {
     return masks + MASK_CTRL + (masks[2] ? set_words : 0u);
 }
@@ -185,23 +265,24 @@ k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_c
             uint32_t* __restrict__ masks) {
     const uint32_t id = blockIdx.x * 256u + threadIdx.x;      // (k nt + band) 8 + c
     if (id >= n_classes) return;
-    const int set = blockIdx.y;
+    const int set = blockIdx.y, cw = class_words(r0), bw = band_words(nt);
     uint32_t* class_mask = masks + MASK_CTRL + set * set_words;
-    uint32_t* band_mask = class_mask + n_classes;
+    uint32_t* band_mask = class_mask + (size_t)n_classes * cw;
     const int c = id & 7;
     const uint32_t kb = id >> 3;
     const int bs = kb % nt, k = kb / nt;
     const int bl = (bs + nt / 2) & (nt - 1);                  // logical tile coordinate of the band
-    uint32_t mask = 0;
+    uint32_t mask[2] = {0u, 0u};
     for (int m = 0; m < r0; ++m) {
         const int ol = (c + 8 * m + nt / 2) & (nt - 1);       // the other coordinate: ty (set 0) or tx (set 1)
         const uint32_t bin = set == 0 ? ((uint32_t)k * nt + ol) * nt + bl : ((uint32_t)k * nt + bl) * nt + ol;
-        if (rec_start[bin + 1] > rec_start[bin]) mask |= 1u << m;
+        if (rec_start[bin + 1] > rec_start[bin]) mask[m >> 5] |= 1u << (m & 31);
     }
-    if (mask) {
-        atomicOr(class_mask + id, mask);
+    if (mask[0] | mask[1]) {
+        for (int i = 0; i < cw; ++i)
+            if (mask[i]) atomicOr(class_mask + (size_t)id * cw + i, mask[i]);
         const uint32_t bit = 1u << (bs & 31);
-        if (!(atomicOr(band_mask + k * 8 + (bs >> 5), bit) & bit)) atomicAdd(masks + set, 1u);
+        if (!(atomicOr(band_mask + k * bw + (bs >> 5), bit) & bit)) atomicAdd(masks + set, 1u);
     }
 }
 // Degridding (ws_degrid.cu): the planes are DENSE on the way in (rows of the model image times the w screen, transformed
@@ -215,7 +296,7 @@ k_fft_masks_degrid(const uint32_t* __restrict__ bin_start, int nt, int r0, uint3
                    uint32_t* __restrict__ masks) {
     const uint32_t kb = blockIdx.x * 256u + threadIdx.x;      // k nt + band (storage order)
     if (kb >= n_kb) return;
-    const int set = blockIdx.y;                               // 0: planes [k][v][u], a band is 32 adjacent u; 1: [k][u][v]
+    const int set = blockIdx.y, cw = class_words(r0), bw = band_words(nt);   // set 0: planes [k][v][u], a band is 32 adjacent u; 1: [k][u][v]
     const int bs = kb % nt, k = kb / nt;
     const int bl = (bs + nt / 2) & (nt - 1);                  // logical tile coordinate of the band
     bool any = false;
@@ -229,10 +310,13 @@ k_fft_masks_degrid(const uint32_t* __restrict__ bin_start, int nt, int r0, uint3
     }
     if (!any) return;
     uint32_t* class_mask = masks + MASK_CTRL + set * set_words;
-    uint32_t* band_mask = class_mask + n_kb * 8u;
-    const uint32_t full = r0 >= 32 ? 0xFFFFFFFFu : (1u << r0) - 1u;
-    for (int c = 0; c < 8; ++c) class_mask[kb * 8u + c] = full;
-    atomicOr(band_mask + k * 8 + (bs >> 5), 1u << (bs & 31));
+    uint32_t* band_mask = class_mask + (size_t)n_kb * 8u * cw;
+    for (int c = 0; c < 8; ++c)
+        for (int i = 0; i < cw; ++i) {
+            const int left = r0 - 32 * i;
+            class_mask[((size_t)kb * 8u + c) * cw + i] = left >= 32 ? 0xFFFFFFFFu : (1u << left) - 1u;
+        }
+    atomicOr(band_mask + k * bw + (bs >> 5), 1u << (bs & 31));
     atomicAdd(masks + set, 1u);
 }
 
@@ -243,31 +327,69 @@ __global__ void k_fft_orient(uint32_t* __restrict__ masks, int allow) { masks[2]
 // Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
 // row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
 template <int LOGN>
-__global__ void __launch_bounds__(CT, 2)
+__global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
-    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32;
+    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32, CW = class_words(R0);
     const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
         const uint32_t jb = item & 31, ktx = item >> 5;            // 32 groups of 8 rows per (plane, band)
         const uint32_t tx = ktx % NT, k = ktx / NT;
-        const uint32_t mask = class_mask ? class_mask[ktx * 8 + (jb >> 2)] : 0xFFFFFFFFu;
-        if (mask == 0) continue;
         const int j = (int)jb * 8 + w;
         float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
-        float2 x[R0];
+        if constexpr (LOGN == 14) {
+            // radix 64 = one radix-2 step over the two halves of the column, then radix 32 on the sum and on the
+            // (twiddled) difference: a[r] = Y[2 brev5(r)], b[r] = Y[2 brev5(r) + 1]
+            const uint32_t m_lo = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW] : 0xFFFFFFFFu;
+            const uint32_t m_hi = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW + 1] : 0xFFFFFFFFu;
+            if ((m_lo | m_hi) == 0) continue;
+            float2 a[32], b[32];
 #pragma unroll
-        for (int m = 0; m < R0; ++m)
-            x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-        bfly<float2, LR0, false>(x);
+            for (int m = 0; m < 32; ++m) {
+                a[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+                b[m] = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
+            }
 #pragma unroll
-        for (int r = 1; r < R0; ++r) {
-            const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
-            x[r] = emul(x[r], tv.x, tv.y);
+            for (int m = 0; m < 32; ++m) {
+                const float2 d = ssub(a[m], b[m]);
+                a[m] = sadd(a[m], b[m]);
+                b[m] = mul_w64(d, m);
+            }
+            bfly<float2, 5, false>(a);
+            bfly<float2, 5, false>(b);
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {
+                const int f0 = 2 * brev(r, 5);
+                if (f0) {
+                    const float2 tv = __ldg(tw + (f0 - 1) * 256 + j);
+                    a[r] = emul(a[r], tv.x, tv.y);
+                }
+                const float2 tu = __ldg(tw + f0 * 256 + j);
+                b[r] = emul(b[r], tu.x, tu.y);
+            }
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {
+                const int f0 = 2 * brev(r, 5);
+                p[(size_t)f0 * 256 * N] = a[r];
+                p[(size_t)(f0 + 1) * 256 * N] = b[r];
+            }
+        } else {
+            const uint32_t mask = class_mask ? class_mask[ktx * 8 + (jb >> 2)] : 0xFFFFFFFFu;
+            if (mask == 0) continue;
+            float2 x[R0];
+#pragma unroll
+            for (int m = 0; m < R0; ++m)
+                x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+            bfly<float2, LR0, false>(x);
+#pragma unroll
+            for (int r = 1; r < R0; ++r) {
+                const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
+                x[r] = emul(x[r], tv.x, tv.y);
+            }
+#pragma unroll
+            for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
         }
-#pragma unroll
-        for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
     }
 }
 
@@ -278,7 +400,7 @@ template <int LOGN>
 __global__ void __launch_bounds__(CT, 2)
 k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
-    constexpr int N = 1 << LOGN, R0 = 1 << (LOGN - 8), NT = N / 32;
+    constexpr int N = 1 << LOGN, R0 = 1 << (LOGN - 8), NT = N / 32, CW = class_words(R0);
     const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
@@ -290,7 +412,11 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
         if (class_mask) {
             cmask = 0;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) cmask |= (class_mask[ktx * 8 + c] != 0 ? 1u : 0u) << c;
+            for (int c = 0; c < 8; ++c) {
+                uint32_t any = class_mask[(ktx * 8 + c) * CW];
+                if (CW > 1) any |= class_mask[(ktx * 8 + c) * CW + 1];
+                cmask |= (any != 0 ? 1u : 0u) << c;
+            }
         }
         if (cmask == 0) continue;
         float2* p = grid + ((size_t)k * N + m0 * 256) * N + tx * 32 + lane;
@@ -370,38 +496,35 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // odd first digit are separate problems.
 // band_mask (or NULL = dense): only the non-empty 32-column bands of a plane are copied in, as maximal runs; a
 // band that is empty now but was filled by the previous copy is cleared first; a plane without any is skipped.
-struct BandMask {
-    uint32_t w[8];
-};
-__device__ __forceinline__ BandMask load_bands(const uint32_t* __restrict__ band_mask, int k, int nt) {
-    BandMask b;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int lo = 32 * i;
-        const uint32_t full = nt >= lo + 32 ? 0xFFFFFFFFu : (nt > lo ? (1u << (nt - lo)) - 1u : 0u);
-        b.w[i] = band_mask ? (band_mask[k * 8 + i] & full) : full;
-    }
-    return b;
-}
-__device__ __forceinline__ bool any_band(const BandMask& b) {
+template <int BW>
+__device__ __forceinline__ bool any_band_of(const uint32_t* __restrict__ band_mask, int k, int nt) {
     uint32_t o = 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) o |= b.w[i];
+    for (int i = 0; i < BW; ++i) {
+        const int lo = 32 * i;
+        const uint32_t full = nt >= lo + 32 ? 0xFFFFFFFFu : (nt > lo ? (1u << (nt - lo)) - 1u : 0u);
+        o |= band_mask ? (band_mask[k * BW + i] & full) : full;
+    }
     return o != 0;
 }
 template <int LOGN>
 struct RowCfg {
-    static constexpr int N = 1 << LOGN, ROWS = PTS / N, NT = N / 32, R0 = 1 << (LOGN - 8);
+    static constexpr int N = 1 << LOGN, NT = N / 32, R0 = 1 << (LOGN - 8);
+    static constexpr int LAND = N > PTS ? N : PTS;    // points the landing buffer holds: whole rows, at least 8192 points
+    static constexpr int ROWS = LAND / N;
     static constexpr int S = n_stages(LOGN);
     static constexpr bool GROUPED = LOGN >= 12;       // two independent 8-warp groups
     static constexpr bool SPLIT32 = LOGN == 13;       // first stage: radix 32 split over the groups
+    static constexpr bool SPLIT64 = LOGN == 14;       // first stage: radix 64 split over the groups of TWO CTAs (by output parity)
+    static constexpr int ITEMS_PER_ROW = SPLIT64 ? 2 : 1;
+    static constexpr int BW = band_words(NT);
     static constexpr int LRL = log2r(LOGN, S - 1);    // last stage
 };
 
 // butterfly i of thread u in stage s (s >= 1, or any stage when not SPLIT32)
 template <int LOGN>
 __device__ __forceinline__ int bfly_id(int u, int i) {
-    if constexpr (RowCfg<LOGN>::SPLIT32) return (((u & 255) >> 4) << 5) | ((u >> 8) << 4) | (u & 15);   // first digit parity = group
+    if constexpr (RowCfg<LOGN>::SPLIT32 || RowCfg<LOGN>::SPLIT64) return (((u & 255) >> 4) << 5) | ((u >> 8) << 4) | (u & 15);   // first digit parity = group
     return u + FT * i;
 }
 template <int LOGL, int LOGR>
@@ -470,14 +593,16 @@ template <int LOGN>
 __device__ __forceinline__ int final_pos(int slot, int u);
 template <int LOGN>
 __device__ __forceinline__ int slot_row(int slot, int u) {
-    if constexpr (LOGN == 13) return 0;
+    if constexpr (LOGN >= 13) return 0;
     else if constexpr (LOGN == 12) return u >> 8;
     else return final_pos<LOGN>(slot, u) >> LOGN;
 }
+// (par: N = 16384 only, the parity of the output frequencies this CTA computes)
 template <int LOGN>
-__device__ __forceinline__ int slot_freq(int slot, int u) {
+__device__ __forceinline__ int slot_freq(int slot, int u, int par) {
     const int ug = u & 255, g = u >> 8;
-    if constexpr (LOGN == 13) return (2 * (ug >> 4) + g) + 32 * (ug & 15) + 512 * brev(slot, 4);
+    if constexpr (LOGN == 14) return (2 * (2 * (ug >> 4) + g) + par) + 64 * (ug & 15) + 1024 * brev(slot, 4);
+    else if constexpr (LOGN == 13) return (2 * (ug >> 4) + g) + 32 * (ug & 15) + 512 * brev(slot, 4);
     else if constexpr (LOGN == 12) return (ug >> 4) + 16 * (ug & 15) + 256 * brev(slot, 4);
     else return freq_of<LOGN>(final_pos<LOGN>(slot, u) & ((1 << LOGN) - 1));
 }
@@ -497,14 +622,35 @@ __device__ __forceinline__ int final_pos(int slot, int u) {
 //                 exchange between the last two stages needs a warp barrier only.
 template <int LOGN>
 struct Grouped {
-    static constexpr bool SPLIT32 = LOGN == 13;
-    __device__ static __forceinline__ int blk(int ug, int g) { return SPLIT32 ? 2 * (ug >> 4) + g : 16 * g + (ug >> 4); }
-    // frequency of register r after the third stage
-    __device__ static __forceinline__ int freq(int ug, int g, int r) {
-        return SPLIT32 ? (2 * (ug >> 4) + g) + 32 * (ug & 15) + 512 * brev(r, 4) : (ug >> 4) + 16 * (ug & 15) + 256 * brev(r, 4);
+    static constexpr bool SPLIT32 = LOGN == 13, SPLIT64 = LOGN == 14, SPLIT = SPLIT32 || SPLIT64;
+    __device__ static __forceinline__ int blk(int ug, int g) { return SPLIT ? 2 * (ug >> 4) + g : 16 * g + (ug >> 4); }
+    // N = 16384, first stage radix 64, m' = m + 16 t: output digit d = 4 d' + q gets
+    //   Y[d] = sum_m [ (sum_t x[m + 16 t] i^(t q)) W_64^(m q) ] W_16^(m d'),
+    // so a thread that wants the outputs of ONE q (= 2 g + parity of the CTA) forms z[m] from four inputs and runs
+    // the 16-point butterfly over m.
+    template <int Q>
+    __device__ static __forceinline__ void load_first64(float2* x, const float2* __restrict__ in) {
+#pragma unroll
+        for (int m = 0; m < 16; ++m) {
+            const float2 x0 = in[256 * m], x1 = in[256 * m + 4096], x2 = in[256 * m + 8192], x3 = in[256 * m + 12288];
+            float2 z;
+            if (Q == 0) z = eadd(eadd(x0, x2), eadd(x1, x3));
+            else if (Q == 1) z = eadd(esub(x0, x2), emul_i(esub(x1, x3)));
+            else if (Q == 2) z = esub(eadd(x0, x2), eadd(x1, x3));
+            else z = esub(esub(x0, x2), emul_i(esub(x1, x3)));
+            x[m] = mul_w64(z, Q * m);
+        }
     }
-    __device__ static __forceinline__ void load_first(float2* x, const float2* __restrict__ landing, int ug, int g) {
-        if constexpr (SPLIT32) {
+    __device__ static __forceinline__ void load_first(float2* x, const float2* __restrict__ landing, int ug, int g, int par) {
+        if constexpr (SPLIT64) {
+            const float2* in = landing + ug;
+            switch (2 * g + par) {                 // warp-uniform
+                case 0: load_first64<0>(x, in); break;
+                case 1: load_first64<1>(x, in); break;
+                case 2: load_first64<2>(x, in); break;
+                default: load_first64<3>(x, in); break;
+            }
+        } else if constexpr (SPLIT32) {
             const float2* in = landing + ug;
             if (g == 0) {
 #pragma unroll
@@ -519,10 +665,21 @@ struct Grouped {
             for (int m = 0; m < 16; ++m) x[m] = in[256 * m];
         }
     }
+    // tc (N = 16384 only): the thread's first-stage twiddles as 7 register constants, tc[b] = W_N^(ug (4 b + q)), b < 4,
+    // tc[3 + a] = W_N^(16 a ug), a = 1..3: output d = 16 a + 4 b + q is multiplied by tc[b] tc[3 + a].
     __device__ static __forceinline__ void finish_first(float2* x, float2* __restrict__ work, const float2* __restrict__ tw,
-                                                        int ug, int g) {
+                                                        int ug, int g, const float2* tc) {
         bfly<float2, 4>(x);
-        if constexpr (SPLIT32) {
+        if constexpr (SPLIT64) {
+            float2* out = work + g * 272 + ug + (ug >> 4);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const int pq = brev(r, 4), b = pq & 3, a = pq >> 2;
+                float2 v = emul(x[r], tc[b].x, tc[b].y);
+                if (a) v = emul(v, tc[3 + a].x, tc[3 + a].y);
+                out[pq * 544] = v;
+            }
+        } else if constexpr (SPLIT32) {
             float2* out = work + g * 272 + ug + (ug >> 4);
             const float2* t = tw + ug + (g - 1) * 256;              // tw[(d - 1) 256 + j], d = 2 brev(r) + g
 #pragma unroll
@@ -555,7 +712,7 @@ struct Grouped {
                                                         int ug, int g) {
         const int jj = ug & 15;
         float2* b1 = work + blk(ug, g) * 272 + jj;
-        const float2* t = tw + tw_offset(LOGN, 1) + jj - 16;        // tw1[(m' - 1) 16 + jj]
+        const float2* t = tw + tw_smem_off1(LOGN) + jj - 16;        // tw1[(m' - 1) 16 + jj]
 #pragma unroll
         for (int m = 0; m < 16; ++m) x[m] = b1[17 * m];
         bfly<float2, 4>(x);
@@ -579,9 +736,12 @@ struct Grouped {
 // Work item -> super-row.  For N = 8192 (one row position per super-row) items are taken in the order of the
 // FREQUENCY the row position holds, pos = (F mod R0) 256 + F / R0, so that the CTAs running side by side own adjacent
 // lines of the image: when the mesh is transposed their 8-byte pixels share 32-byte sectors and meet in L2.
+// N = 16384: two items per row (even / odd output frequencies), taken by neighbouring CTAs at the same time, so that the
+// second reader of the row finds it in L2.
 template <int LOGN>
 __device__ __forceinline__ uint32_t super_row_of(uint32_t item) {
     constexpr int LR0 = LOGN - 8;
+    if constexpr (RowCfg<LOGN>::SPLIT64) item >>= 1;
     if constexpr (RowCfg<LOGN>::ROWS == 1) return ((item & ((1u << LR0) - 1u)) << 8) | (item >> LR0);
     else return item;
 }
@@ -589,30 +749,31 @@ __device__ __forceinline__ uint32_t super_row_of(uint32_t item) {
 template <int LOGN>
 __global__ void __launch_bounds__(FT + PT, 1)
 k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ planes, float2* __restrict__ image,
-           float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g,
+           float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g, const float2* __restrict__ tc_g,
            const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_super) {
     using C = RowCfg<LOGN>;
-    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0;
+    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0, LAND = C::LAND, BW = C::BW;
     // occupancy: the band masks of the orientation the mesh is stored in; transposed: the mesh is [k][u][v], i.e. a
     // row position is a u-frequency and the image comes out transposed (the phase screen is symmetric in l and m)
-    const uint32_t* band_mask = masks ? mask_set(masks, set_words) + (set_words - 8u * (uint32_t)prm.n_wplanes) : nullptr;
+    const uint32_t* band_mask = masks ? mask_set(masks, set_words) + (set_words - (uint32_t)BW * (uint32_t)prm.n_wplanes) : nullptr;
     const bool transposed = masks && masks[2];
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* landing = (float2*)smem_raw;
-    float2* work = landing + PTS;
+    float2* work = landing + LAND;
     float2* tw = work + PAD_PTS;
-    uint64_t* full = (uint64_t*)(tw + ((tw_entries(LOGN) + 1) & ~1));   // the copy of a plane has landed
+    uint64_t* full = (uint64_t*)(tw + ((tw_smem_entries(LOGN) + 1) & ~1));   // the copy of a plane has landed
     uint64_t* empty = full + 1;                                         // every group has consumed it
     uint32_t* s_any = (uint32_t*)(empty + 1);                           // bit k: plane k has a non-empty band
     const int u = threadIdx.x, g = u >> 8;
+    const int par = C::SPLIT64 ? (int)(blockIdx.x & 1u) : 0;           // (the grid is even: every item of a CTA has its parity)
     const int nw = prm.n_wplanes;
     const size_t plane_elems = (size_t)N * N;
-    for (int i = u; i < tw_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
-    for (int i = u; i < PTS; i += FT + PT) landing[i] = make_float2(0.f, 0.f);
+    for (int i = u; i < tw_smem_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
+    for (int i = u; i < LAND; i += FT + PT) landing[i] = make_float2(0.f, 0.f);
     for (int k0 = 0; k0 < nw; k0 += FT + PT) {       // (FT + PT is a multiple of 32: one ballot per mask word)
         const int k = k0 + u;
         bool any = false;
-        if (k < nw) any = any_band(load_bands(band_mask, k, NT));
+        if (k < nw) any = any_band_of<BW>(band_mask, k, NT);
         const uint32_t bits = __ballot_sync(0xffffffffu, any);
         if ((u & 31) == 0 && k < nw) s_any[k >> 5] = bits;
     }
@@ -628,7 +789,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
         if (u >= FT + 32) return;
         // ---- producer warp: clears the bands of `landing` that the last copy filled and the next one will not, then
-        // brings the non-empty bands of the next plane in.  Lane wi < 8 owns mask word wi (32 bands = 8 KB per row)
+        // brings the non-empty bands of the next plane in.  Lane wi < BW owns mask word wi (32 bands = 8 KB per row)
         // and issues one bulk copy per maximal run of set bits.
         const int lane = u & 31;
         uint32_t was = 0, e_parity = 0;
@@ -638,10 +799,10 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
             for (int k = nw - 1; k >= 0; --k) {
                 if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
                 uint32_t now = 0;
-                if (lane < 8) {
+                if (lane < BW) {
                     const int lo = 32 * lane;
                     const uint32_t fullw = NT >= lo + 32 ? 0xFFFFFFFFu : (NT > lo ? (1u << (NT - lo)) - 1u : 0u);
-                    now = band_mask ? (__ldg(band_mask + k * 8 + lane) & fullw) : fullw;
+                    now = band_mask ? (__ldg(band_mask + k * BW + lane) & fullw) : fullw;
                 }
                 // what needs neither `landing` nor the barrier happens before the wait for the consumers
                 uint32_t n_bands = __popc(now);
@@ -654,10 +815,11 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                     e_parity ^= 1u;
                 }
                 first = false;
-                if (lane == 0) mbar_expect_tx(full, n_bands * 256u * ROWS);     // (the previous phase is complete now)
+                // stale bands are cleared BEFORE the arrive: its release then orders the zeroing stores ahead of the
+                // consumers' reads (they acquire `full`), whatever the bulk copies' timing
                 if (any_stale) {
 #pragma unroll
-                    for (int wi = 0; wi < 8; ++wi) {
+                    for (int wi = 0; wi < BW; ++wi) {
                         uint32_t z = __shfl_sync(0xffffffffu, stale, wi);
                         while (z) {
                             const int b = wi * 32 + __ffs(z) - 1;
@@ -666,9 +828,11 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                         }
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    __syncwarp();
                 }
-                const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * PTS);
+                __syncwarp();
+                if (lane == 0) mbar_expect_tx(full, n_bands * 256u * ROWS);     // (the previous phase is complete now)
+                __syncwarp();
+                const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * LAND);
                 uint32_t m = now;
                 while (m) {
                     const int b0 = __ffs(m) - 1;
@@ -694,6 +858,13 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     };
     uint32_t parity = 0;
     const int top_span_lo = ((nw - 1) / WC_SPAN) * WC_SPAN;
+    float2 tc[7];      // N = 16384: first-stage twiddles of this thread (Grouped::finish_first), constant for the whole kernel
+    if constexpr (C::SPLIT64) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) tc[i] = __ldg(tc_g + ((2 * g + par) * 4 + i) * 256 + (u & 255));
+#pragma unroll
+        for (int i = 0; i < 3; ++i) tc[4 + i] = __ldg(tc_g + (16 + i) * 256 + (u & 255));
+    }
 
     for (uint32_t it = blockIdx.x; it < n_super; it += gridDim.x) {
         const uint32_t sr = super_row_of<LOGN>(it);
@@ -702,7 +873,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         for (int s = 0; s < EPT; ++s) {
             const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
             const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-            const int p = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
+            const int p = (slot_freq<LOGN>(s, u, par) + N / 2) & (N - 1);
             bool inside;
             const double tt = ws_n_minus_1(prm, q, p, &inside);
             rot[s] = ws_expi_turns(prm.dw * tt);
@@ -714,14 +885,14 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                 while (!mbar_try_wait(full, parity)) {}
                 parity ^= 1u;
                 // ---- first stage: inputs from the landing buffer
-                if constexpr (C::GROUPED) Grouped<LOGN>::load_first(x, landing, u & 255, g);
+                if constexpr (C::GROUPED) Grouped<LOGN>::load_first(x, landing, u & 255, g, par);
                 else row_stage<LOGN, 0, true, false>(x, landing, work, tw, u);
                 group_sync();          // this group is done with `landing` (and with last plane's reads of `work`)
                 if ((u & 255) == 0 && (C::GROUPED || g == 0))
                     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty)) : "memory");
                 // ---- arithmetic, twiddles, exchanges
                 if constexpr (C::GROUPED) {
-                    Grouped<LOGN>::finish_first(x, work, tw, u & 255, g);
+                    Grouped<LOGN>::finish_first(x, work, tw, u & 255, g, tc);
                     group_sync();
                     Grouped<LOGN>::second_third(x, work, tw, u & 255, g);
                 } else {
@@ -745,7 +916,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
             for (int s = 0; s < EPT; ++s) {
                 const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
                 const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-                const int p = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
+                const int p = (slot_freq<LOGN>(s, u, par) + N / 2) & (N - 1);
                 bool inside;
                 const double tt = ws_n_minus_1(prm, q, p, &inside);
                 x[s] = ws_cmul(h[s], ws_expi_turns((prm.w0 + (double)k * prm.dw) * tt));
@@ -757,7 +928,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                 for (int s = 0; s < EPT; ++s) {
                     const int pos = (int)sr * ROWS + slot_row<LOGN>(s, u);
                     const int a = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-                    const int b = (slot_freq<LOGN>(s, u) + N / 2) & (N - 1);
+                    const int b = (slot_freq<LOGN>(s, u, par) + N / 2) & (N - 1);
                     const size_t o = (size_t)b * N + a;
                     float2 v = x[s];
                     if (accumulate || k != top_span_lo) {
@@ -771,24 +942,45 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
             }
             // un-permute through `work`: natural order along the rows of the centred image (both groups)
             cta_sync();
+            if constexpr (C::SPLIT64) {
+                // this CTA holds every second pixel of the line (those of its parity): work[i] = pixel 2 i + par
 #pragma unroll
-            for (int s = 0; s < EPT; ++s)
-                work[pad(slot_row<LOGN>(s, u) * N + ((slot_freq<LOGN>(s, u) + N / 2) & (N - 1)))] = x[s];
-            cta_sync();
-#pragma unroll
-            for (int i = 0; i < EPT / 2; ++i) {
-                const int e = (u + FT * i) * 2;
-                const float2 a = work[pad(e)], b = work[pad(e) + 1];
-                float4 v = make_float4(a.x, a.y, b.x, b.y);
-                const int pos = (int)sr * ROWS + (e >> LOGN);
+                for (int s = 0; s < EPT; ++s) work[pad(((slot_freq<LOGN>(s, u, par) + N / 2) & (N - 1)) >> 1)] = x[s];
+                cta_sync();
+                const int pos = (int)sr;
                 const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
-                const size_t o = (size_t)q * N + (e & (N - 1));
-                if (accumulate || k != top_span_lo) {
-                    const float4 old = *(const float4*)(image + o);
-                    v.x += old.x; v.y += old.y; v.z += old.z; v.w += old.w;
+#pragma unroll
+                for (int i = 0; i < EPT; ++i) {
+                    const int e = u + FT * i;
+                    float2 v = work[pad(e)];
+                    const size_t o = (size_t)q * N + 2 * e + par;
+                    if (accumulate || k != top_span_lo) {
+                        const float2 old = image[o];
+                        v.x += old.x; v.y += old.y;
+                    }
+                    image[o] = v;
+                    if (dirty && k == 0) dirty[o] = v.x;
                 }
-                *(float4*)(image + o) = v;
-                if (dirty && k == 0) *(float2*)(dirty + o) = make_float2(v.x, v.z);
+            } else {
+#pragma unroll
+                for (int s = 0; s < EPT; ++s)
+                    work[pad(slot_row<LOGN>(s, u) * N + ((slot_freq<LOGN>(s, u, par) + N / 2) & (N - 1)))] = x[s];
+                cta_sync();
+#pragma unroll
+                for (int i = 0; i < EPT / 2; ++i) {
+                    const int e = (u + FT * i) * 2;
+                    const float2 a = work[pad(e)], b = work[pad(e) + 1];
+                    float4 v = make_float4(a.x, a.y, b.x, b.y);
+                    const int pos = (int)sr * ROWS + (e >> LOGN);
+                    const int q = ((pos >> 8) + R0 * (pos & 255) + N / 2) & (N - 1);
+                    const size_t o = (size_t)q * N + (e & (N - 1));
+                    if (accumulate || k != top_span_lo) {
+                        const float4 old = *(const float4*)(image + o);
+                        v.x += old.x; v.y += old.y; v.z += old.z; v.w += old.w;
+                    }
+                    *(float4*)(image + o) = v;
+                    if (dirty && k == 0) *(float2*)(dirty + o) = make_float2(v.x, v.z);
+                }
             }
             cta_sync();            // `work` is free again before the next plane's first stage stores into it
         }
@@ -799,8 +991,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
 // ---- host side ---------------------------------------------------------------------------------------------
 template <int LOGN>
 size_t rows_smem() {
-    return (size_t)PTS * sizeof(float2) + (size_t)PAD_PTS * sizeof(float2) +
-           (size_t)((tw_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16 + MAX_PLANES / 8;
+    return (size_t)RowCfg<LOGN>::LAND * sizeof(float2) + (size_t)PAD_PTS * sizeof(float2) +
+           (size_t)((tw_smem_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16 + MAX_PLANES / 8;
 }
 
 float2 unit(long long e, long long L) {      // exp(+2 pi i e / L), fp64 -> fp32
@@ -808,13 +1000,14 @@ float2 unit(long long e, long long L) {      // exp(+2 pi i e / L), fp64 -> fp32
     return make_float2((float)cos(a), (float)sin(a));
 }
 
-// Table = [pass 2: every stage but the last, (R-1) Q entries W_L^(j m') each | pass 1a: (R0-1) x 256 entries
-// W_N^(j m') | pass 1b: 15 x 16 entries W_256^(j m')]
+// Table = [pass 2: every stage but the last, (R-1) Q entries W_L^(j m') each (N = 16384: stage 1 only) | pass 1a:
+// (R0-1) x 256 entries W_N^(j m') | pass 1b: 15 x 16 entries W_256^(j m') | N = 16384: the first-stage register constants
+// of the row kernel, [q][b][ug] = W_N^(ug (4 b + q)) (4 x 4 x 256) then [a][ug] = W_N^(16 a ug), a = 1..3]
 template <int LOGN>
 int init_n(ws_plan* plan) {
     constexpr int N = 1 << LOGN, R0 = N / 256;
     std::vector<float2> tw;
-    for (int s = 0; s + 1 < n_stages(LOGN); ++s) {
+    for (int s = LOGN == 14 ? 1 : 0; s + 1 < n_stages(LOGN); ++s) {
         const int L = 1 << log2l(LOGN, s), R = 1 << log2r(LOGN, s), Q = L / R;
         for (int m = 1; m < R; ++m)
             for (int j = 0; j < Q; ++j) tw.push_back(unit((long long)j * m, L));
@@ -825,8 +1018,19 @@ int init_n(ws_plan* plan) {
     plan->tw_off_b = tw.size();
     for (int m = 1; m < 16; ++m)
         for (int j = 0; j < 16; ++j) tw.push_back(unit((long long)j * m, 256));
-    const size_t n_class = (size_t)plan->prm.n_wplanes * (N / 32) * 8, n_band = (size_t)plan->prm.n_wplanes * 8;
+    plan->tw_off_c = tw.size();
+    if (LOGN == 14) {
+        for (int q = 0; q < 4; ++q)
+            for (int b = 0; b < 4; ++b)
+                for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * (4 * b + q), N));
+        for (int a = 1; a < 4; ++a)
+            for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * 16 * a, N));
+    }
+    const size_t n_class = (size_t)plan->prm.n_wplanes * (N / 32) * 8 * class_words(R0),
+                 n_band = (size_t)plan->prm.n_wplanes * band_words(N / 32);
     plan->mask_set_words = n_class + n_band;
+    plan->mask_class_words = class_words(R0);
+    plan->mask_band_words = band_words(N / 32);
     plan->mask_words = MASK_CTRL + 2 * plan->mask_set_words;
     if (cudaMalloc((void**)&plan->d_twiddles, tw.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&plan->d_masks, plan->mask_words * sizeof(uint32_t)) != cudaSuccess)
@@ -873,17 +1077,19 @@ int launch_rows_n(ws_plan* plan, const float2* grid, float2* image, float* dirty
     prm.cell = P.cell_rad;
     prm.dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
     prm.w0 = P.w_min + 0.5 * prm.dw;
-    const uint32_t n_super = (uint32_t)(((size_t)N * N) / PTS);
-    const uint32_t ctas = n_super < (uint32_t)plan->sm_count ? n_super : (uint32_t)plan->sm_count;
+    const uint32_t n_super = (uint32_t)(((size_t)N * N) / RowCfg<LOGN>::LAND) * RowCfg<LOGN>::ITEMS_PER_ROW;
+    uint32_t ctas = n_super < (uint32_t)plan->sm_count ? n_super : (uint32_t)plan->sm_count;
+    if (RowCfg<LOGN>::ITEMS_PER_ROW == 2) ctas &= ~1u;      // even grid: a CTA keeps the parity of its first item
     const uint32_t* bm = sparse ? (const uint32_t*)plan->d_masks : nullptr;
     k_fft_rows<LOGN><<<ctas, FT + PT, rows_smem<LOGN>(), st>>>(prm, grid, image, dirty, accumulate,
-                                                          (const float2*)plan->d_twiddles, bm,
-                                                                    (uint32_t)plan->mask_set_words, n_super);
+                                                          (const float2*)plan->d_twiddles,
+                                                          (const float2*)plan->d_twiddles + plan->tw_off_c, bm,
+                                                          (uint32_t)plan->mask_set_words, n_super);
     return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
 }
 
 int logn_of(int n_pix) {
-    for (int l = 8; l <= 13; ++l)
+    for (int l = 8; l <= 14; ++l)
         if (n_pix == (1 << l)) return l;
     return 0;
 }
@@ -898,6 +1104,7 @@ int logn_of(int n_pix) {
         case 11: return fn<11>(__VA_ARGS__);         \
         case 12: return fn<12>(__VA_ARGS__);         \
         case 13: return fn<13>(__VA_ARGS__);         \
+        case 14: return fn<14>(__VA_ARGS__);         \
     }                                                \
     return WS_ERR_UNSUPPORTED;
 
@@ -924,7 +1131,7 @@ int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st) {
 int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, int decide, cudaStream_t st) {
     if (!plan->d_masks) return 0;
     const int nt = plan->geom.nt, r0 = plan->prm.n_pix / 256;
-    const uint32_t n_classes = (uint32_t)plan->prm.n_wplanes * (uint32_t)nt * 8u;
+    const uint32_t n_classes = (uint32_t)plan->prm.n_wplanes * (uint32_t)nt * 8u;     // (class masks: class_words(r0) words each)
     uint32_t* m = (uint32_t*)plan->d_masks;
     k_fft_masks<<<dim3((n_classes + 255) / 256, 2), 256, 0, st>>>(rec_start, nt, r0, n_classes, (uint32_t)plan->mask_set_words, m);
     int launches = 1;

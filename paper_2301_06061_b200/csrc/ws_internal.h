@@ -95,7 +95,8 @@ struct ws_plan {
     // own FFT (ws_fft.cu): available for N = 2^8 .. 2^13 unless WS_FLAG_LIBRARY_FFT is set
     bool fft_own;
     void* d_twiddles;                           // plan-owned inter-stage twiddle tables (fp64-computed, < 140 KB)
-    size_t tw_off_a, tw_off_b;                  // entry offsets of the pass 1a / 1b tables
+    size_t tw_off_a, tw_off_b, tw_off_c;        // entry offsets of the pass 1a / 1b tables and of the row kernel's register constants
+    int mask_class_words, mask_band_words;      // words per class mask (2 for N = 16384) and band words per plane (16 for N = 16384)
     void* d_masks;                              // plan-owned tile-occupancy masks of the mesh (class masks, band masks)
     size_t mask_words, mask_set_words;          // whole buffer; one set (class masks + band masks) of the two orientations
     double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)

@@ -185,9 +185,10 @@ def test_paper_medium_whole_mesh_image_and_sum_of_weights(oracle):
     _whole_config(oracle, "paper_medium", presum=True)
 
 
-@pytest.mark.parametrize("n_pix,n_wplanes", [(4096, 3), (8192, 2)])
+@pytest.mark.parametrize("n_pix,n_wplanes", [(4096, 3), (8192, 2), (16384, 2)])
 def test_own_fft_dense_random_planes_full_width(oracle, n_pix, n_wplanes):
-    """The row-pass stage plans of N = 4096 (a row per group) and N = 8192 (split radix-32) on arbitrary dense planes."""
+    """The row-pass stage plans of N = 4096 (a row per group), N = 8192 (split radix-32) and N = 16384 (radix 64 split over
+    two CTAs; radix-64 column pass) on arbitrary dense planes."""
     d = make_random_dataset(50 + n_wplanes, 10, 1, n_pix, n_wplanes, 7, w_span=250.0, cell_rad=0.6 / n_pix)
     plan = U.make_plan(d)
     assert plan.fft_is_own
@@ -207,10 +208,10 @@ def test_own_fft_dense_random_planes_full_width(oracle, n_pix, n_wplanes):
     assert torch.equal(dirty, image.real)
 
 
-@pytest.mark.parametrize("n_pix", [4096, 8192])
+@pytest.mark.parametrize("n_pix", [4096, 8192, 16384])
 @pytest.mark.parametrize("squeeze_axis", [0, 1])
 def test_own_fft_sparse_both_orientations_full_width(oracle, n_pix, squeeze_axis):
-    """Sparse mesh + occupancy-aware passes at N = 4096 / 8192 in both storage orientations (uv coverage squeezed along
+    """Sparse mesh + occupancy-aware passes at N = 4096 / 8192 / 16384 in both storage orientations (uv coverage squeezed along
     u or along v), whole image against the oracle."""
     import paper_2301_06061_b200 as ws
     d = make_random_dataset(60 + squeeze_axis, 200000, 1, n_pix, 3, 7, fill=0.9, w_span=80.0, cell_rad=0.5 / n_pix)
