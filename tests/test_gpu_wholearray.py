@@ -61,10 +61,11 @@ def _sparse_plane_logical(grid_k: torch.Tensor, transposed: bool) -> torch.Tenso
     return g.T if transposed else g
 
 
-def _whole_config(oracle, cfg_name, planes=None, presum=False, one_mesh=False, dup_factor=None):
-    """Mesh (OVERWRITE: every cell; SPARSE: every written cell, unwritten ones must be exact zeros of the oracle) on the
-    planes `planes` (None: all) and, when all planes are covered, the whole image of the timed path.  one_mesh: the two
-    meshes do not fit the device side by side (Extreme): one buffer, gridded twice, the oracle's planes kept on the host."""
+def _whole_config(oracle, cfg_name, presum=False, one_mesh=False, dup_factor=None, overwrite_planes=(0, 11, 20, 31)):
+    """Every plane of the mesh (OVERWRITE: every cell; SPARSE: every written cell, unwritten ones must be exact zeros of
+    the oracle) and the whole image of the timed path, then of the dense own FFT on the OVERWRITE mesh.  one_mesh: the
+    two meshes do not fit the device side by side (Extreme): one buffer, SPARSE first; the OVERWRITE mesh is gridded
+    into it after the image and compared on `overwrite_planes` (the oracle's planes are kept on the host for that)."""
     import paper_2301_06061_b200 as ws
     cfg = get_config(cfg_name)
     dg = make_dataset(cfg, device="cuda")
@@ -75,9 +76,6 @@ def _whole_config(oracle, cfg_name, planes=None, presum=False, one_mesh=False, d
     assert plan.fft_is_own
     prm = U.oracle_params(oracle, d, plan.tile)
     N, NW = d.n_pix, d.n_wplanes
-    all_planes = planes is None
-    planes = list(range(NW)) if all_planes else list(planes)
-    assert not (one_mesh and all_planes)
     grid_s = plan.alloc_grid()
     grid_o = grid_s if one_mesh else plan.alloc_grid()
     image, dirty = plan.alloc_image(), plan.alloc_dirty()
@@ -105,50 +103,35 @@ def _whole_config(oracle, cfg_name, planes=None, presum=False, one_mesh=False, d
         assert not bool(torch.any(ref[unwritten] != 0)), f"plane {k}: a tile the sparse gridder skipped is not empty"
         e_sparse.add(torch.where(unwritten, torch.zeros_like(got), got), ref)
 
-    transposed = None
     if not one_mesh:
         grid_overwrite()
-        transposed = grid_sparse()
+    transposed = grid_sparse()
     if presum:
         sw = oracle.sum_weights(prm, d.uvw.numpy(), d.weights.numpy(), d.freqs_hz)
         assert abs(plan.sum_weights() - sw) <= 1e-9 * sw
     torch.cuda.synchronize()
 
-    D = np.zeros((N, N), np.complex128) if all_planes else None
+    D = np.zeros((N, N), np.complex128)
     B = _plane_batch(oracle, N)
     kept = {}
     t0 = time.time()
-    for lo in range(0, len(planes), B):
-        ks = planes[lo:lo + B]
-        if ks == list(range(ks[0], ks[0] + len(ks))):
-            G = oracle.grid(prm, *_np(d), plane_lo=ks[0], plane_hi=ks[0] + len(ks))
-        else:
-            G = np.concatenate([oracle.grid(prm, *_np(d), plane_lo=k, plane_hi=k + 1) for k in ks])
-        for i, k in enumerate(ks):
+    for lo in range(0, NW, B):
+        hi = min(lo + B, NW)
+        G = oracle.grid(prm, *_np(d), plane_lo=lo, plane_hi=hi)
+        for k in range(lo, hi):
+            ref = torch.from_numpy(G[k - lo]).cuda()
             if one_mesh:
-                kept[k] = G[i].copy()
-                continue
-            ref = torch.from_numpy(G[i]).cuda()
-            cmp_overwrite(k, ref)
+                if k in overwrite_planes:
+                    kept[k] = G[k - lo].copy()
+            else:
+                cmp_overwrite(k, ref)
             cmp_sparse(k, ref, transposed)
             del ref
-            if all_planes:
-                oracle.wcorrect(prm, oracle.fft2(G[i], inplace=True)[None], k, D)
+            oracle.wcorrect(prm, oracle.fft2(G[k - lo], inplace=True)[None], k, D)
         del G
-    print(f"{cfg_name}: oracle streamed over {len(planes)} planes in {time.time() - t0:.0f} s (batches of {B})")
-    if one_mesh:
-        grid_overwrite()
-        for k, g in kept.items():
-            cmp_overwrite(k, torch.from_numpy(g).cuda())
-        transposed = grid_sparse()
-        for k, g in kept.items():
-            cmp_sparse(k, torch.from_numpy(g).cuda(), transposed)
-        kept.clear()
-    e_over.check()
+    print(f"{cfg_name}: oracle streamed over {NW} planes in {time.time() - t0:.0f} s (batches of {B})")
     e_sparse.check()
-    if not all_planes:
-        return plan, d, dg, prm, grid_s, image, dirty
-    # the image of the timed path, whole; then the dense own FFT on the OVERWRITE mesh
+    # the image of the timed path, whole
     plan.fft_columns(grid_s, ws.WS_FFT_USE_OCCUPANCY)
     plan.fft_rows_wcorrect(grid_s, image, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
     plan.async_status()
@@ -157,16 +140,23 @@ def _whole_config(oracle, cfg_name, planes=None, presum=False, one_mesh=False, d
     e.add(image, Dd)
     e.check()
     assert torch.equal(dirty, image.real)
+    if one_mesh:
+        grid_overwrite()
+        for k, g in kept.items():
+            cmp_overwrite(k, torch.from_numpy(g).cuda())
+        kept.clear()
+    e_over.check()
+    # the dense own FFT on the OVERWRITE mesh
     plan.fft_wcorrect(grid_o, image, wsp, accumulate=False, dirty=None, fft_flags=0)
     e = Running(f"{cfg_name} image (dense own FFT)")
     e.add(image, Dd)
     e.check()
-    return plan, d, dg, prm, grid_s, image, dirty
+    return plan, d, dg, prm
 
 
 def test_large_whole_mesh_and_image(oracle):
     """All 64 planes of Large's mesh and its whole 8192^2 image; bins bit-exact over all 10^8 visibilities."""
-    plan, d, dg, prm, *_ = _whole_config(oracle, "large")
+    plan, d, dg, prm = _whole_config(oracle, "large")
     key = oracle.positions(prm, d.uvw.numpy(), d.n_chan, d.freqs_hz)["key"]
     bins = plan.get_bins()
     assert np.array_equal(bins["keys"], key)
@@ -233,29 +223,7 @@ def test_own_fft_sparse_both_orientations_full_width(oracle, n_pix, squeeze_axis
 
 
 @pytest.mark.skipif(os.environ.get("WS_SKIP_EXTREME") == "1", reason="WS_SKIP_EXTREME=1")
-def test_extreme_planes_and_pixels(oracle):
-    """Extreme (4 x 10^8 visibilities, 16384^2 x 32, S = 9) in ONE call: four whole planes of the mesh (first, last and
-    two inner ones; OVERWRITE and SPARSE) and 64 pixels of the image of the timed path against the oracle's chain
-    evaluated pixel by pixel (the whole image would need all 32 fp64 planes of 4.3 GB transformed on the host)."""
-    import paper_2301_06061_b200 as ws
-    plan, d, dg, prm, grid_s, image, dirty = _whole_config(oracle, "extreme", planes=(0, 11, 20, 31), one_mesh=True,
-                                                           dup_factor=2.0)
-    plan.fft_columns(grid_s, ws.WS_FFT_USE_OCCUPANCY)
-    plan.fft_rows_wcorrect(grid_s, image, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
-    plan.async_status()
-    assert torch.equal(dirty, image.real)
-    assert bool(torch.isfinite(image.real).all()) and bool(torch.isfinite(image.imag).all())
-    N, c = d.n_pix, d.n_pix // 2
-    rng = np.random.default_rng(77)
-    top = np.argsort(d.src_flux)[-8:]
-    q = [c, 0, N - 1, 0, N - 1] + [int(round(d.src_m[i] / d.cell_rad)) + c for i in top]
-    p = [c, 0, N - 1, N - 1, 0] + [int(round(d.src_l[i] / d.cell_rad)) + c for i in top]
-    q += list(rng.integers(0, N, 64 - len(q)))
-    p += list(rng.integers(0, N, 64 - len(p)))
-    q, p = np.clip(q, 0, N - 1), np.clip(p, 0, N - 1)
-    ref = oracle.image_samples(prm, *_np(d), q, p)
-    got = image[torch.from_numpy(q).cuda(), torch.from_numpy(p).cuda()].cpu().numpy().astype(np.complex128)
-    peak = max(np.abs(ref).max(), float(torch.abs(image).max()))
-    rel, mx = np.linalg.norm(got - ref) / np.linalg.norm(ref), np.abs(got - ref).max() / peak
-    print("extreme image, 64 pixels: rel-L2 %.3e, max-abs/peak %.3e" % (rel, mx))
-    assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL
+def test_extreme_whole_mesh_and_image(oracle):
+    """Extreme (4 x 10^8 visibilities, 16384^2 x 32, S = 9) in ONE call: all 32 planes of the sparse mesh, the whole
+    16384^2 image of the timed path (own FFT for N = 16384) and of the dense own FFT, four planes of the OVERWRITE mesh."""
+    _whole_config(oracle, "extreme", one_mesh=True, dup_factor=2.0)
