@@ -94,39 +94,69 @@ def oracle_params(orc, d, tile=32):
                             kernel_type=1 if kb else 0)
 
 
-def cpu_baseline(d, n_sample_planes=2):
-    """The fp64 oracle as it stands, plane-streamed like oracle.dirty_image, timed on the host cores on a bounded
-    sample: `n_sample_planes` of the N_w planes (each plane pass = place + grid all visibilities onto that plane,
-    transform it, w-correct it); the whole-workload time is the sample time x N_w / n_sample_planes."""
-    from oracle import wstack_oracle as orc
-    prm = oracle_params(orc, d)
-    uvw, vis, wt = d.uvw.cpu().numpy(), d.vis.cpu().numpy(), d.weights.cpu().numpy()
-    n_s = min(n_sample_planes, d.n_wplanes)
-    planes = sorted(set(int(round((i + 0.5) * d.n_wplanes / n_s - 0.5)) for i in range(n_s)))
+def _omp_threads(n):
+    """Sets the OpenMP thread count of the process (the oracle's runtime is libgomp); False if that is not possible."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def _oracle_planes(orc, prm, d, lo, n):
+    """The oracle's chain on planes [lo, lo + n): one gridding call (a plane per host thread: every core works), then
+    its transform and w-correction plane by plane.  Returns the seconds it took."""
+    uvw, vis, wt = d.uvw.numpy(), d.vis.numpy(), d.weights.numpy()
     D = np.zeros((d.n_pix, d.n_pix), np.complex128)
     t0 = time.perf_counter()
-    for k in planes:
-        G = orc.grid(prm, uvw, vis, wt, d.freqs_hz, k, k + 1)
-        orc.wcorrect(prm, orc.transform(G[0])[None], k, D)
-    dt = time.perf_counter() - t0
-    full = dt * d.n_wplanes / len(planes)
-    return {"value": d.n_vis / full / 1e6, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": f"planes {planes} of {d.n_wplanes} (all {d.n_vis} visibilities placed per plane pass, fp64 grid + "
-                      f"radix-2 FFT + w-correction of those planes): {dt:.1f} s, whole workload extrapolated x"
-                      f"{d.n_wplanes / len(planes):.0f} = {full:.0f} s",
-            "sample_seconds": dt}
+    G = orc.grid(prm, uvw, vis, wt, d.freqs_hz, lo, lo + n)
+    for i in range(n):
+        orc.wcorrect(prm, orc.transform(G[i])[None], lo + i, D)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(d, single_thread=True):
+    """The fp64 oracle as it stands, plane-streamed like oracle.dirty_image, timed on the host cores on a bounded
+    sample: ONE batch of `cores` adjacent planes from the middle of the stack (each plane pass places all visibilities,
+    grids those of its plane, transforms and w-corrects it); the whole-workload time is the sample time x N_w / planes.
+    Also the same on ONE thread and one plane (comparison with the paper's per-core rows)."""
+    import psutil
+    from oracle import wstack_oracle as orc
+    prm = oracle_params(orc, d)
+    d = d.to("cpu")
+    cores = orc.num_threads()
+    fit = int(psutil.virtual_memory().available * 0.4 // (16 * d.n_pix ** 2))
+    n_s = max(1, min(cores, d.n_wplanes, fit))
+    lo = (d.n_wplanes - n_s) // 2
+    dt = _oracle_planes(orc, prm, d, lo, n_s)
+    full = dt * d.n_wplanes / n_s
+    out = {"value": d.n_vis / full / 1e6, "unit": UNIT, "cores": min(cores, n_s), "kind": "oracle",
+           "planes_timed": n_s, "planes_total": d.n_wplanes, "extrapolated": n_s < d.n_wplanes, "sample_seconds": dt,
+           "sample": f"planes {lo}..{lo + n_s - 1} of {d.n_wplanes}, one per thread (all {d.n_vis} visibilities placed per plane "
+                     f"pass, fp64 grid + radix-2 FFT + w-correction of those planes): {dt:.1f} s"
+                     + (f", whole workload extrapolated x{d.n_wplanes / n_s:.1f} = {full:.0f} s" if n_s < d.n_wplanes else "")}
+    if single_thread and _omp_threads(1):
+        try:
+            k1 = d.n_wplanes // 2
+            dt1 = _oracle_planes(orc, prm, d, k1, 1)
+        finally:
+            _omp_threads(cores)
+        out["single_thread"] = {"value": d.n_vis / (dt1 * d.n_wplanes) / 1e6, "unit": UNIT, "cores": 1, "planes_timed": 1,
+                                "extrapolated": d.n_wplanes > 1, "sample_seconds": dt1}
+    return out
 
 
 def run_reference(args, d, cfg_name):
-    n_planes = 2 if args.steps + args.warmup <= 6 else 1
     for _ in range(args.warmup):
-        cpu_baseline(d, n_planes)
-    vals = [cpu_baseline(d, n_planes) for _ in range(args.steps)]
+        cpu_baseline(d, single_thread=False)
+    vals = [cpu_baseline(d, single_thread=False) for _ in range(args.steps)]
     v = float(np.mean([x["value"] for x in vals]))
     cb = dict(vals[-1]); cb["value"] = v
     ms = d.n_vis / (v * 1e6) * 1e3
     return {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_is_extrapolated": bool(cb["extrapolated"]),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(d, cfg_name),
             "cpu_baseline": cb, "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
 
@@ -220,12 +250,16 @@ def main():
         wsp = plan.alloc_workspace(max(hi - lo for lo, hi in chunks) * d.n_chan)
 
     def step_chunked(ev=None):
-        # stages: [zero] [bin + grid of all chunks] [FFT] [w-correct]; the library FFT path (no occupancy of a partial mesh)
+        # stages: [-] [bin + grid of all chunks] [FFT] [w-correct].  The mesh is never cleared: the first chunk is gridded
+        # WS_GRID_SPARSE (library FFT: OVERWRITE), the later ones WS_GRID_SPARSE_ADD (ACCUMULATE)
         if ev: ev[0].record()
-        plan.grid_zero(grid)
         if ev: ev[1].record()
-        for lo, hi in chunks:
-            plan.grid_visibilities(d.uvw[lo:hi], d.vis[lo:hi], d.weights[lo:hi], d.freqs_hz, grid, wsp, mode=ws.WS_GRID_ACCUMULATE)
+        for i, (lo, hi) in enumerate(chunks):
+            if own:
+                mode = ws.WS_GRID_SPARSE if i == 0 else ws.WS_GRID_SPARSE_ADD
+            else:
+                mode = ws.WS_GRID_OVERWRITE if i == 0 else ws.WS_GRID_ACCUMULATE
+            plan.grid_visibilities(d.uvw[lo:hi], d.vis[lo:hi], d.weights[lo:hi], d.freqs_hz, grid, wsp, mode=mode)
         if ev: ev[2].record()
         if own:
             plan.fft_columns(grid, OCC)
@@ -360,53 +394,90 @@ def main():
     peak, peak_src = peaks()
     mesh_b = 8.0 * d.n_pix ** 2 * d.n_wplanes
     N, NW = d.n_pix, d.n_wplanes
+    n_keys = d.n_rows if presum else d.n_vis
+    # a1: inputs read once (12 B/row + 12 B/visibility), keys + perm written (4 + 4 B per binned entry), records written
+    alg_bin = 12.0 * d.n_rows + 12.0 * d.n_vis + 8.0 * n_keys + 16.0 * n_records
     if own:
         # k_grid: records read + non-empty tiles written; pass 1: non-empty tiles read, classes written, then the
         # non-empty bands read and written; pass 2: non-empty bands read once, image + dirty written
-        alg = {"k_grid_tiles": 16.0 * n_records + mesh_b * occ["tiles"],
+        alg = {"bin": alg_bin, "k_grid_tiles": 16.0 * n_records + mesh_b * occ["tiles"],
                "k_fft_columns": mesh_b * (occ["tiles"] + occ["classes"] + 2 * occ["bands"]),
                "k_fft_rows_wcorrect": mesh_b * occ["bands"] + 12.0 * N * N}
-        times = {"k_grid_tiles": med[1], "k_fft_columns": med[2], "k_fft_rows_wcorrect": med[3]}
+        times = {"bin": med[0], "k_grid_tiles": med[1], "k_fft_columns": med[2], "k_fft_rows_wcorrect": med[3]}
         # nominal FFT flops (5 n log2 n per transform) of the transforms that are not skipped, + 8 per point-plane of Horner
         flops = {"k_fft_columns": 5.0 * N * np.log2(N) * N * NW * occ["bands"],
                  "k_fft_rows_wcorrect": (5.0 * N * np.log2(N) + 8.0 * N) * N * NW * occ["planes"]}
     else:
         occ = None
-        alg = {"k_grid_tiles": mesh_b + 16.0 * n_records, "k_wcorrect": mesh_b + 12.0 * N * N}
-        times = {"k_grid_tiles": med[1], "k_wcorrect": med[3]}
+        alg = {"bin": alg_bin, "k_grid_tiles": mesh_b + 16.0 * n_records, "k_wcorrect": mesh_b + 12.0 * N * N}
+        times = {"bin": med[0], "k_grid_tiles": med[1], "k_wcorrect": med[3]}
         flops = {}
-    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures of this command
-    # (profiles/r1m_large_ncu.md) -- Large, Gaussian only
-    ncu_traffic = {"k_fft_rows_wcorrect": 13.967e9 + 1.113e9, "k_fft_columns": (1.437e9 + 11.106e9) + (10.838e9 + 13.589e9)} if (cfg.name == "large" and KERNEL == "gaussian" and own) else {}
-    dom = max(times, key=times.get)
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch: from the committed ncu --set full capture of this command
+    # and configuration, if there is one (profiles/traffic.json names the capture each figure comes from), else null
+    ncu_traffic, traffic_src = {}, None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tj = json.load(f)
+        ent = tj.get(f"{cfg.name}/{KERNEL}")
+        if ent and own and not chunks:
+            ncu_traffic, traffic_src = {k: float(v) for k, v in ent["dram_bytes_per_launch"].items()}, ent["capture"]
+    except Exception:
+        pass
+    kernel_times = {k: v for k, v in times.items() if k != "bin"}
+    dom = max(kernel_times, key=kernel_times.get)
     ach = alg[dom] / (times[dom] * 1e-3) / 1e9
     hbm_frac = ach / peak
     roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": hbm_frac,
-            "traffic": ncu_traffic.get(dom), "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
-            "launch_ms": float(times[dom])}
+            "traffic": ncu_traffic.get(dom), "traffic_source": traffic_src if dom in ncu_traffic else None,
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom], "launch_ms": float(times[dom])}
     if dom in flops:
-        # fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x max SM clock (B200_PROFILING.md unit counts and clocks)
+        # fp32 peak: DERIVED, 148 SMs x 128 lanes x 2 flop x max SM clock (B200_PROFILING.md unit counts and clocks);
+        # `fp32_fma_measured_tflops` beside it is what a register-only FFMA loop of this library reaches on this GPU
         alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
         tf = flops[dom] / (times[dom] * 1e-3) / 1e12
         if tf / alu_peak > hbm_frac:
             roof = {"bound": "alu", "kernel": dom, "achieved": tf, "peak": alu_peak, "unit": "TFLOP/s", "frac": tf / alu_peak,
-                    "traffic": ncu_traffic.get(dom), "peak_source": "148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (guide's unit counts and clocks)",
+                    "traffic": ncu_traffic.get(dom), "traffic_source": traffic_src if dom in ncu_traffic else None,
+                    "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz (guide's unit counts and clocks)",
+                    "fp32_fma_measured_tflops": plan.measure_fp32_tflops(),
                     "nominal_flops_per_launch": flops[dom], "launch_ms": float(times[dom]),
                     "hbm_view": {"achieved": ach, "peak": peak, "frac": hbm_frac, "algorithmic_bytes_per_launch": alg[dom]}}
     per_kernel = {k: {"ms": float(times[k]), "alg_GB": alg[k] / 1e9, "GBps": alg[k] / (times[k] * 1e-3) / 1e9,
                       "frac_of_hbm_peak": alg[k] / (times[k] * 1e-3) / 1e9 / peak,
                       "ncu_dram_GB": ncu_traffic[k] / 1e9 if k in ncu_traffic else None} for k in times}
-    # B_alg(path) counts every plane cell written once and read once; the sparse path moves less
+    # the whole timed step against HBM: sum of the algorithmic bytes of its stages / its device time
+    b_step = float(sum(alg.values()))
+    roof_step = {"what": "sum of the stages' algorithmic bytes / ms_per_step (the timed step as a whole)", "bytes": b_step,
+                 "ms": float(ms_step), "achieved": b_step / (ms_step * 1e-3) / 1e9,
+                 "frac_of_measured_peak": b_step / (ms_step * 1e-3) / 1e9 / peak}
+    # B_alg(path) counts every plane cell written once and read once (a DENSE mesh), so its time is that of
+    # the gridder that writes every cell (WS_GRID_OVERWRITE) + the stand-alone w-correction that reads every cell
     b_path = 12.0 * d.n_rows + 12.0 * d.n_vis + 2 * mesh_b + 8.0 * N * N
-    t_path = med[0] + med[1] + (lib_ms["wcorrect_standalone"] if lib_ms else med[3])
-    roof_path = {"what": "a1+a2+a4 without any FFT (bin + grid + stand-alone w-correction), SURVEY 8(d) B_alg(path)",
-                 "bytes": b_path, "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
-                 "frac_of_measured_peak": b_path / (t_path * 1e-3) / 1e9 / peak,
-                 "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
+    roof_path = None
+    if lib_ms:
+        t_path = med[0] + lib_ms["grid_overwrite"] + lib_ms["wcorrect_standalone"]
+        roof_path = {"what": "a1 + a2 (WS_GRID_OVERWRITE: every cell written) + stand-alone a4, no FFT: SURVEY 8(d) B_alg(path), dense accounting",
+                     "bytes": b_path, "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
+                     "frac_of_measured_peak": b_path / (t_path * 1e-3) / 1e9 / peak,
+                     "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
+    elif not own:
+        t_path = med[0] + med[1] + med[3]
+        roof_path = {"what": "a1 + a2 (every cell written) + stand-alone a4 of the timed step, no FFT: SURVEY 8(d) B_alg(path)",
+                     "bytes": b_path, "ms": float(t_path), "achieved": b_path / (t_path * 1e-3) / 1e9,
+                     "frac_of_measured_peak": b_path / (t_path * 1e-3) / 1e9 / peak,
+                     "frac_of_nominal_8TBs": b_path / (t_path * 1e-3) / 1e9 / 8000.0}
+    # the sparse path's gridding with ITS OWN bytes (inputs, keys, records, only the tiles that hold visibilities)
+    roof_sparse = None
+    if own:
+        b_sp = alg["bin"] + alg["k_grid_tiles"]
+        t_sp = med[0] + med[1]
+        roof_sparse = {"what": "a1 + a2 of the timed step (WS_GRID_SPARSE) with the bytes that path moves", "bytes": b_sp,
+                       "ms": float(t_sp), "achieved": b_sp / (t_sp * 1e-3) / 1e9,
+                       "frac_of_measured_peak": b_sp / (t_sp * 1e-3) / 1e9 / peak}
 
     stage_names = ["bin", "grid", "fft_columns", "fft_rows_wcorrect"] if own else ["bin", "grid", "fft_cufft", "wcorrect"]
     if chunks:
-        stage_names = ["zero", "bin_and_grid_%d_chunks" % len(chunks)] + stage_names[2:]
+        stage_names = ["-", "bin_and_grid_%d_chunks" % len(chunks)] + stage_names[2:]
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
            "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk, "gpu_launches": int(launches),
@@ -419,7 +490,7 @@ def main():
            "presummed_channels": bool(presum),
            "snapshot_rows_hint": int(d.rows_per_snapshot) if (d.rows_per_snapshot and not args.no_snapshot_hint) else 0,
            "image_wall_ms": ms_step, "bins": bins_info, "roofline": roof, "kernels": per_kernel,
-           "roofline_path": roof_path}
+           "roofline_step": roof_step, "roofline_path": roof_path, "roofline_sparse_gridding": roof_sparse}
 
     # ---- end to end through the C ABI with HOST buffers --------------------------------------------------
     if not args.no_e2e:

@@ -52,13 +52,19 @@ extern "C" {
 #define WS_ERR_CUFFT (-5)
 
 /* ws_grid_visibilities mode */
-#define WS_GRID_ACCUMULATE 0 /* add onto the existing mesh (call ws_grid_zero first); tiles without visibilities untouched */
+#define WS_GRID_ACCUMULATE 0 /* add onto the existing mesh (call ws_grid_zero first, or start with an OVERWRITE call); tiles
+                                without visibilities untouched */
 #define WS_GRID_OVERWRITE 1  /* the mesh is taken as zero on entry and EVERY cell is written: no ws_grid_zero needed */
 #define WS_GRID_SPARSE 2     /* as OVERWRITE, but only the 32 x 32 tiles that receive visibilities are written; every
                                 other cell keeps whatever it held, and the layout is PRIVATE: the library stores the
                                 planes transposed ([k][u][v]) when that leaves fewer 32-line bands to transform.  Only
                                 ws_fft_* with WS_FFT_USE_OCCUPANCY can consume such a mesh (own FFT: N = 2^8..2^13
                                 and no WS_FLAG_LIBRARY_FFT), and nothing can be accumulated onto it */
+
+#define WS_GRID_SPARSE_ADD 3 /* a further chunk of visibilities onto a WS_GRID_SPARSE mesh (same plan, same `grid`, nothing else
+                                having written it since): tiles the earlier calls filled are added to, tiles that are new are
+                                stored, the recorded occupancy grows.  The orientation the first call chose is kept.  This is
+                                how chunks are streamed through the gridder without ever clearing the mesh (Extreme) */
 
 /* fft_flags of ws_fft_wcorrect / ws_fft_columns / ws_fft_rows_wcorrect */
 #define WS_FFT_USE_OCCUPANCY 1u /* skip the tiles / column bands the gridding calls on this plan left empty.  The plan
@@ -240,6 +246,11 @@ int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float*
  * the deferred status (WS_ERR_WORKSPACE if the record capacity of `workspace` was exceeded: dirty_h is then
  * meaningless). */
 size_t ws_dev_inputs_bytes(int64_t n_rows, int32_t n_chan);
+/* The rows are fed through the gridder in chunks of about `bytes` input bytes (0: the default, 160 MiB; at most 32
+ * chunks): the copy of chunk c + 1 runs on a second stream beside the binning and gridding of chunk c (first chunk
+ * WS_GRID_SPARSE, later ones WS_GRID_SPARSE_ADD), so that only the last chunk's gridding, the FFT and the copy out
+ * are exposed behind the PCIe time (the paper's GPU timings include the copies). */
+int ws_plan_set_e2e_chunk_bytes(ws_plan* plan, size_t bytes);
 int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, const float* weights_h,
                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
                        size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,
@@ -263,6 +274,10 @@ int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* band
 /* Synchronises `stream` and returns the deferred status of the work enqueued so far (record capacity
  * exceeded -> WS_ERR_WORKSPACE, CUDA fault -> WS_ERR_CUDA). */
 int ws_async_status(ws_plan* plan, void* stream);
+
+/* Diagnostic (not part of the path): the fp32 FMA rate, in TFLOP/s, that a register-only FFMA loop reaches on the plan's
+ * device (best of four short launches; synchronises `stream`).  bench.py prints it beside the derived fp32 peak. */
+int ws_measure_fp32_tflops(ws_plan* plan, double* tflops, void* stream);
 
 /* Number of kernels this library has launched through `plan` since it was created. */
 int64_t ws_launch_count(const ws_plan* plan);

@@ -237,6 +237,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     }
     // a3: the FFT of ws_fft.cu where it exists (N = 2^8 .. 2^13), else (or on request) the library's
     plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix, p->n_wplanes);
+    plan->e2e_ready = false;
+    plan->e2e_chunk_bytes = 0;
     plan->d_twiddles = nullptr;
     plan->d_masks = nullptr;
     plan->mask_words = 0;
@@ -279,6 +281,11 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
 
 int ws_plan_destroy(ws_plan* plan) {
     if (!plan) return WS_ERR_INVALID_ARG;
+    if (plan->e2e_ready) {
+        cudaStreamDestroy(plan->copy_stream);
+        cudaEventDestroy(plan->ev_start);
+        for (int i = 0; i < WS_E2E_MAX_CHUNKS; ++i) cudaEventDestroy(plan->ev_chunk[i]);
+    }
     if (plan->fft_ok) cufftDestroy(plan->fft);
     if (plan->fft_rows1d_ok) cufftDestroy(plan->fft_rows1d);
     if (plan->d_status) cudaFree(plan->d_status);
@@ -295,6 +302,12 @@ int ws_plan_set_snapshot_rows(ws_plan* plan, int64_t rows_per_snapshot) {
     if (rows_per_snapshot < 0 || rows_per_snapshot > MAX_VIS)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_plan_set_snapshot_rows: bad count");
     plan->snapshot_rows = rows_per_snapshot;
+    return WS_OK;
+}
+
+int ws_plan_set_e2e_chunk_bytes(ws_plan* plan, size_t bytes) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    plan->e2e_chunk_bytes = bytes;
     return WS_OK;
 }
 
@@ -412,44 +425,54 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid || !workspace) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: null pointer");
-    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE)
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: bad mode");
-    if (mode == WS_GRID_SPARSE && !plan->fft_own)
-        return fail(plan, WS_ERR_UNSUPPORTED, "ws_grid_binned: WS_GRID_SPARSE needs the own FFT (N = 2^8..2^13, no WS_FLAG_LIBRARY_FFT)");
+    const bool sparse_mode = mode == WS_GRID_SPARSE || mode == WS_GRID_SPARSE_ADD;
+    if (sparse_mode && !plan->fft_own)
+        return fail(plan, WS_ERR_UNSUPPORTED, "ws_grid_binned: WS_GRID_SPARSE needs the own FFT (N = 2^8..2^14, no WS_FLAG_LIBRARY_FFT)");
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: grid must be 16-byte aligned");
     if (!plan->last_valid || !plan->last_has_values || plan->last_ws != workspace || plan->last_layout.total > workspace_bytes)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: workspace does not hold the bins of ws_bin_visibilities");
     if (mode == WS_GRID_ACCUMULATE && plan->occ_sparse && plan->occ_grid == grid)
-        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written)");
-    // Tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE.  It
-    // comes BEFORE the gridding kernel: a SPARSE mesh is stored in the orientation the masks favour.
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written): use WS_GRID_SPARSE_ADD");
+    if (mode == WS_GRID_SPARSE_ADD && !(plan->occ_sparse && plan->occ_grid == grid))
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: WS_GRID_SPARSE_ADD needs a mesh this plan wrote with WS_GRID_SPARSE");
+    cudaStream_t st = (cudaStream_t)stream;
+    // Tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE /
+    // SPARSE_ADD.  It comes BEFORE the gridding kernel -- a SPARSE mesh is stored in the orientation the masks favour --
+    // except for SPARSE_ADD, whose kernel must see the occupancy of the EARLIER chunks to know which tiles to add to.
     int rc;
-    if (plan->d_masks) {
-        if (mode != WS_GRID_ACCUMULATE) {
-            if (ws_launch_fft_masks_clear(plan, (cudaStream_t)stream) < 0) return fail(plan, WS_ERR_CUDA, "ws_grid_binned: mask clear failed");
+    auto update_masks = [&]() -> int {
+        if (!plan->d_masks) return WS_OK;
+        if (mode == WS_GRID_OVERWRITE || mode == WS_GRID_SPARSE) {
+            if (ws_launch_fft_masks_clear(plan, st) < 0) return fail(plan, WS_ERR_CUDA, "ws_grid_binned: mask clear failed");
             plan->occ_grid = grid;
             plan->occ_sparse = mode == WS_GRID_SPARSE;
         }
         if (plan->occ_grid == grid) {
-            rc = ws_launch_fft_masks(plan, (const uint32_t*)((char*)workspace + plan->last_layout.off_rec_start),
-                                     mode == WS_GRID_SPARSE ? 1 : (mode == WS_GRID_OVERWRITE ? 0 : -1), (cudaStream_t)stream);
-            if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
-            plan->launches += rc;
+            const int r = ws_launch_fft_masks(plan, (const uint32_t*)((char*)workspace + plan->last_layout.off_rec_start),
+                                              mode == WS_GRID_SPARSE ? 1 : (mode == WS_GRID_OVERWRITE ? 0 : -1), st);
+            if (r < 0) return fail(plan, r, "ws_grid_binned: launch failed");
+            plan->launches += r;
         } else {
             plan->occ_grid = nullptr;                    // accumulation onto a mesh this plan has no record of
         }
-    }
+        return WS_OK;
+    };
+    if (mode != WS_GRID_SPARSE_ADD && (rc = update_masks()) != WS_OK) return rc;
     if (plan->prm.flags & WS_FLAG_TRACK_SUMWT) {
-        if (mode != WS_GRID_ACCUMULATE && cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), (cudaStream_t)stream) != cudaSuccess)
+        if ((mode == WS_GRID_OVERWRITE || mode == WS_GRID_SPARSE) &&
+            cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), st) != cudaSuccess)
             return fail(plan, WS_ERR_CUDA, "ws_grid_binned: memset failed");
         rc = ws_launch_sum_weights(plan, plan->last_layout, (char*)workspace, plan->last_weights,
-                                   plan->last_n_vis * plan->last_chan_per_key, plan->last_chan_per_key, (cudaStream_t)stream);
+                                   plan->last_n_vis * plan->last_chan_per_key, plan->last_chan_per_key, st);
         if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
         plan->launches += rc;
     }
-    rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, (cudaStream_t)stream);
+    rc = ws_launch_grid(plan, plan->last_layout, (char*)workspace, (float2*)grid, mode, st);
     if (rc < 0) return fail(plan, rc, "ws_grid_binned: launch failed");
     plan->launches += rc;
+    if (mode == WS_GRID_SPARSE_ADD && (rc = update_masks()) != WS_OK) return rc;
     return WS_OK;
 }
 
@@ -458,7 +481,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
                          void* workspace, size_t workspace_bytes, void* stream) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
-    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE)
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: bad mode");
     const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
@@ -684,19 +707,56 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
     if (dev_inputs_bytes < b_uvw + b_vis + b_wt) return fail(plan, WS_ERR_WORKSPACE, "ws_image_from_host: dev_inputs too small");
     if ((uintptr_t)dev_inputs & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: dev_inputs must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if (!plan->e2e_ready) {
+        if ((e = cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
+            return cuda_fail(plan, e, "ws_image_from_host: stream");
+        bool ok = cudaEventCreateWithFlags(&plan->ev_start, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; i < WS_E2E_MAX_CHUNKS; ++i)
+            ok = ok && cudaEventCreateWithFlags(&plan->ev_chunk[i], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) return fail(plan, WS_ERR_CUDA, "ws_image_from_host: events");
+        plan->e2e_ready = true;
+    }
+    // Row chunks: the copy of chunk c + 1 (copy stream) runs beside the binning + gridding of chunk c (caller's stream),
+    // which therefore hide under the PCIe time; what remains exposed is the last chunk's gridding, the FFT and the
+    // copy out.  Chunk starts are multiples of 4 rows (16-byte alignment of every array) and of eight snapshots (the
+    // snapshot-ordered walk of the binning, if the hint is set).
+    const size_t total_in = (size_t)n_rows * 12 + n_vis * 12;
+    const size_t chunk_bytes = plan->e2e_chunk_bytes ? plan->e2e_chunk_bytes : ((size_t)160 << 20);
+    int64_t n_chunks = (int64_t)((total_in + chunk_bytes - 1) / chunk_bytes);
+    n_chunks = n_chunks < 1 ? 1 : (n_chunks > WS_E2E_MAX_CHUNKS ? WS_E2E_MAX_CHUNKS : n_chunks);
+    int64_t quantum = 4;
+    if (plan->snapshot_rows > 0) quantum = plan->snapshot_rows * 8 % 4 == 0 ? plan->snapshot_rows * 8 : plan->snapshot_rows * 32;
+    int64_t chunk_rows = (n_rows + n_chunks - 1) / n_chunks;
+    chunk_rows = (chunk_rows + quantum - 1) / quantum * quantum;
+    n_chunks = (n_rows + chunk_rows - 1) / chunk_rows;
     char* d = (char*)dev_inputs;
     float* uvw_d = (float*)d;
-    void* vis_d = d + b_uvw;
+    char* vis_d = d + b_uvw;
     float* wt_d = (float*)(d + b_uvw + b_vis);
-    cudaError_t e;
-    if ((e = cudaMemcpyAsync(uvw_d, uvw_h, (size_t)n_rows * 12, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(vis_d, vis_h, n_vis * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(wt_d, weights_h, b_wt, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-        return cuda_fail(plan, e, "ws_image_from_host: H2D copy");
+    if ((e = cudaEventRecord(plan->ev_start, st)) != cudaSuccess ||               // dev_inputs may still be read by earlier work
+        (e = cudaStreamWaitEvent(plan->copy_stream, plan->ev_start, 0)) != cudaSuccess)
+        return cuda_fail(plan, e, "ws_image_from_host: event");
+    for (int64_t c = 0; c < n_chunks; ++c) {
+        const int64_t r0 = c * chunk_rows, nr = (r0 + chunk_rows <= n_rows ? chunk_rows : n_rows - r0);
+        const size_t v0 = (size_t)r0 * n_chan, nv = (size_t)nr * n_chan;
+        if ((e = cudaMemcpyAsync(uvw_d + 3 * r0, uvw_h + 3 * r0, (size_t)nr * 12, cudaMemcpyHostToDevice, plan->copy_stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(vis_d + v0 * 8, (const char*)vis_h + v0 * 8, nv * 8, cudaMemcpyHostToDevice, plan->copy_stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(wt_d + v0, weights_h + v0, nv * 4, cudaMemcpyHostToDevice, plan->copy_stream)) != cudaSuccess ||
+            (e = cudaEventRecord(plan->ev_chunk[c], plan->copy_stream)) != cudaSuccess)
+            return cuda_fail(plan, e, "ws_image_from_host: H2D copy");
+    }
     // the mesh is never cleared nor completely written where the own FFT can skip what the gridder left empty
-    int rc = ws_grid_visibilities(plan, uvw_d, vis_d, wt_d, freq_hz, n_rows, n_chan, grid,
-                                  plan->fft_own ? WS_GRID_SPARSE : WS_GRID_OVERWRITE, workspace, workspace_bytes, stream);
-    if (rc != WS_OK) return rc;
+    for (int64_t c = 0; c < n_chunks; ++c) {
+        const int64_t r0 = c * chunk_rows, nr = (r0 + chunk_rows <= n_rows ? chunk_rows : n_rows - r0);
+        const size_t v0 = (size_t)r0 * n_chan;
+        if ((e = cudaStreamWaitEvent(st, plan->ev_chunk[c], 0)) != cudaSuccess) return cuda_fail(plan, e, "ws_image_from_host: event");
+        const int mode = plan->fft_own ? (c == 0 ? WS_GRID_SPARSE : WS_GRID_SPARSE_ADD) : (c == 0 ? WS_GRID_OVERWRITE : WS_GRID_ACCUMULATE);
+        const int rc = ws_grid_visibilities(plan, uvw_d + 3 * r0, vis_d + v0 * 8, wt_d + v0, freq_hz, nr, n_chan, grid, mode,
+                                            workspace, workspace_bytes, stream);
+        if (rc != WS_OK) return rc;
+    }
+    int rc;
     if ((rc = ws_fft_wcorrect(plan, grid, image, 0, dirty_d, plan->fft_own ? WS_FFT_USE_OCCUPANCY : 0u, workspace,
                               workspace_bytes, stream)) != WS_OK)
         return rc;
@@ -713,8 +773,10 @@ int ws_async_status(ws_plan* plan, void* stream) {
     WsStatus s;
     e = cudaMemcpy(&s, plan->d_status, sizeof(s), cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(plan, e, "ws_async_status: status read");
-    if (s.overflow)
+    if (s.overflow || s.sticky_overflow) {
+        cudaMemset(&plan->d_status->sticky_overflow, 0, sizeof(uint32_t));
         return fail(plan, WS_ERR_WORKSPACE, "record capacity of the workspace exceeded: gridding was skipped");
+    }
     return WS_OK;
 }
 

@@ -4,6 +4,8 @@
 // unspecified, R19): histogram over all bins, exclusive prefix scan (warp shuffles), and a scatter that
 // writes, per bin, contiguous 16-byte records the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
 // it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
+#include <stddef.h>
+
 #include <algorithm>
 
 #include "ws_internal.h"
@@ -235,7 +237,7 @@ k_finish_offsets(const uint32_t* __restrict__ bin_start, const uint32_t* __restr
     } else {
         status->n_kept = bs;
         status->n_records = bs + hs;
-        if ((uint64_t)bs + (uint64_t)hs > rec_capacity) status->overflow = 1u;
+        if ((uint64_t)bs + (uint64_t)hs > rec_capacity) status->overflow = status->sticky_overflow = 1u;
     }
 }
 
@@ -424,7 +426,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
 
     // the two histograms are contiguous at the head of the workspace: one clear, plus the plan's status block
     if (cudaMemsetAsync(ws, 0, L.off_rec_start, st) != cudaSuccess) return WS_ERR_CUDA;
-    if (cudaMemsetAsync(status, 0, sizeof(WsStatus), st) != cudaSuccess) return WS_ERR_CUDA;
+    if (cudaMemsetAsync(status, 0, offsetof(WsStatus, sticky_overflow), st) != cudaSuccess) return WS_ERR_CUDA;
 
     const uint32_t n_scan = g.n_bins + 1;
     const uint32_t n_blocks = (n_scan + SCAN_BLOCK - 1) / SCAN_BLOCK;

@@ -252,7 +252,7 @@ __device__ __forceinline__ void bfly(E* x) {
 // squeezed in v by sin(dec), and a band costs 2 N x 256 B of traffic in pass 1b and pass 2.
 // Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; set = class masks, band masks.
 // Masks are OR-ed into (chunked gridding accumulates); ws_fft_masks_clear zeroes them.
-constexpr int MASK_CTRL = 8;
+constexpr int MASK_CTRL = WS_MASK_CTRL;
 // Words per class mask (one bit per input of pass 1a's radix-R0 butterfly: R0 = 64 for N = 16384 needs two) and band
 // words per plane (one bit per 32-column band: 512 bands for N = 16384).
 __host__ __device__ constexpr int class_words(int r0) { return r0 > 32 ? 2 : 1; }
@@ -1152,6 +1152,10 @@ int ws_launch_fft_masks_degrid(ws_plan* plan, const uint32_t* bin_start, cudaStr
                                                                    (uint32_t*)plan->d_masks);
     k_fft_orient<<<1, 1, 0, st>>>((uint32_t*)plan->d_masks, !(plan->prm.flags & WS_FLAG_NO_TRANSPOSE));   // fewer bands wins
     return cudaGetLastError() == cudaSuccess ? 2 : WS_ERR_CUDA;
+}
+
+WsMaskView ws_fft_mask_view(const ws_plan* plan) {
+    return WsMaskView{(const uint32_t*)plan->d_masks, (uint32_t)plan->mask_set_words, plan->d_masks ? plan->mask_class_words : 1};
 }
 
 const uint32_t* ws_fft_orientation_flag(const ws_plan* plan) { return plan->d_masks ? (const uint32_t*)plan->d_masks + 2 : nullptr; }

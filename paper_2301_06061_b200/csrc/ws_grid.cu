@@ -155,7 +155,7 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
 __global__ void __launch_bounds__(256)
 k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, uint4* __restrict__ items,
                 uint32_t item_capacity, WsStatus* __restrict__ status, float2* __restrict__ grid, int mode,
-                const uint32_t* __restrict__ orient) {
+                const uint32_t* __restrict__ orient, const WsMaskView mv) {
     if (status->overflow) return;
     const bool tr = orient && *orient;
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
@@ -180,7 +180,7 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
     if (lane == 0) base = atomicAdd(&status->n_items, total);
     base = __shfl_sync(0xffffffffu, base, 0);
     if (base + total > item_capacity) {
-        if (lane == 0) status->overflow = 1u;
+        if (lane == 0) status->overflow = status->sticky_overflow = 1u;
         return;
     }
     if (heavy) {
@@ -190,6 +190,10 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
     if (mode != WS_GRID_ACCUMULATE) {
         for (unsigned m = hm; m; m &= m - 1) {
             const uint32_t hb = (b - lane) + (__ffs(m) - 1);
+            if (mode == WS_GRID_SPARSE_ADD) {                   // a tile earlier chunks filled is added to, not cleared
+                const uint32_t nt = (uint32_t)g.nt, tx = hb % nt, r = hb / nt;
+                if (ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx)) continue;
+            }
             store_zero_tile(tile_origin(g, grid, hb, tr), (size_t)g.n_pix, lane);
         }
     }
@@ -200,7 +204,7 @@ template <int S, bool KB>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 2)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint4* __restrict__ items,
        const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
-       const uint32_t* __restrict__ orient) {
+       const uint32_t* __restrict__ orient, const WsMaskView mv) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -245,18 +249,19 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         }
         zero_tile<S>(sm.tile, lane);
         accumulate<S, KB>(g, records, s, e, sm, lane);
-        if (mode != WS_GRID_ACCUMULATE) {
+        bool add = mode == WS_GRID_ACCUMULATE;
+        if (mode == WS_GRID_SPARSE_ADD) {                       // warp-uniform: did an earlier chunk fill this tile?
+            const uint32_t nt = (uint32_t)g.nt, tx = bin % nt, r = bin / nt;
+            add = ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx);
+        }
+        if (!add) {
 #pragma unroll 4
             for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane]);
-        } else {
+        } else {        // no other warp writes this tile in this launch except through red: fire-and-forget vector adds
 #pragma unroll 4
             for (int y = 0; y < T; ++y) {
-                float2 v = sm.tile[y * C::P + lane];
-                float2* p = out + (size_t)y * N + lane;
-                const float2 old = *p;
-                v.x += old.x;
-                v.y += old.y;
-                *p = v;
+                const float2 v = tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane];
+                if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
             }
         }
         __syncwarp();
@@ -266,7 +271,9 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
 
 template <int S, bool KB>
 int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st) {
-    const uint32_t* orient = mode == WS_GRID_SPARSE ? ws_fft_orientation_flag(plan) : nullptr;
+    const uint32_t* orient = (mode == WS_GRID_SPARSE || mode == WS_GRID_SPARSE_ADD) ? ws_fft_orientation_flag(plan) : nullptr;
+    const WsMaskView mv = ws_fft_mask_view(plan);
+    if (mode == WS_GRID_SPARSE_ADD && !mv.masks) return WS_ERR_UNSUPPORTED;
     using C = TileCfg<S>;
     const size_t smem = C::WARP_BYTES * C::WARPS;
     // per device, and cheap: set on every launch rather than cached in a process-wide flag
@@ -277,8 +284,8 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient);
-    k_grid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient);
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient, mv);
+    k_grid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient, mv);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }
@@ -290,7 +297,7 @@ int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&plan->d_status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
     k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, items, item_capacity, plan->d_status, nullptr,
-                                                          WS_GRID_ACCUMULATE, nullptr);
+                                                          WS_GRID_ACCUMULATE, nullptr, WsMaskView{nullptr, 0u, 1});
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;
 }

@@ -13,6 +13,7 @@
 #define WS_CHUNK 1024         // records a warp accumulates in shared memory before it flushes
 #define WS_HALO_MAX 7         // (S-1)/2 for S <= 15
 #define WS_KB_MAX_TERMS 48    // terms of the I0 power series kept for the Kaiser-Bessel taps (beta <= 24)
+#define WS_E2E_MAX_CHUNKS 32   // row chunks ws_image_from_host pipelines (copy of chunk c + 1 beside the gridding of chunk c)
 #define WS_WC_GROUP 8          // planes per Horner block in the w-correction (exact restart between blocks)
 
 // Per-channel position constants (O1): fp64, computed on the host exactly as the header states.
@@ -67,8 +68,9 @@ struct WsStatus {                               // device-side, 64 bytes
     uint32_t n_kept;                            // kept visibilities (home histogram total)
     uint32_t n_records;                         // records incl. halo copies
     uint32_t n_items;                           // heavy chunks queued
-    uint32_t overflow;                          // 1: record or item capacity exceeded, gridding skipped
-    uint32_t pad[12];
+    uint32_t overflow;                          // 1: record or item capacity exceeded, gridding skipped (cleared by every binning call)
+    uint32_t sticky_overflow;                   // ... of ANY call since the last ws_async_status (which clears it)
+    uint32_t pad[11];
 };
 
 struct ws_plan {
@@ -105,16 +107,43 @@ struct ws_plan {
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
     int32_t last_chan_per_key;                  // visibilities per binned entry: 1, or n_chan after a pre-summed call
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
+    cudaStream_t copy_stream;                   // ws_image_from_host: the H2D copies of the next chunk run beside the gridding
+    cudaEvent_t ev_start, ev_chunk[WS_E2E_MAX_CHUNKS];    // of this one (created on first use)
+    bool e2e_ready;
+    size_t e2e_chunk_bytes;                     // input bytes per chunk (0: 160 MiB)
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
     bool occ_sparse;                            // ... and it was written by WS_GRID_SPARSE (private layout, empty tiles unwritten)
 };
 
 static inline size_t ws_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Tile-occupancy masks of the mesh (built by ws_fft.cu, also read by the gridder in WS_GRID_SPARSE_ADD mode).
+// Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; a set = class masks, band masks.
+// class mask ((k nt + band) 8 + c) x cw words: bit m <=> the tile at (other coordinate = c + 8 m, band) of plane k holds
+// visibilities, in STORAGE (FFT-native) tile coordinates; set 0: band = tx, other = ty; set 1 (transposed mesh): swapped.
+#define WS_MASK_CTRL 8
+struct WsMaskView {
+    const uint32_t* masks;     // NULL: no occupancy available
+    uint32_t set_words;
+    int32_t class_words;
+};
+#ifdef __CUDACC__
+// was the logical tile (k, ty, tx) marked occupied?  (the set of the orientation the mesh is stored in)
+__device__ __forceinline__ bool ws_tile_occupied(const WsMaskView& mv, int nt, uint32_t k, uint32_t ty, uint32_t tx) {
+    const uint32_t tr = mv.masks[2];
+    const uint32_t* cm = mv.masks + WS_MASK_CTRL + (tr ? mv.set_words : 0u);
+    const uint32_t sx = (tx + (uint32_t)nt / 2) & ((uint32_t)nt - 1), sy = (ty + (uint32_t)nt / 2) & ((uint32_t)nt - 1);
+    const uint32_t band = tr ? sy : sx, other = tr ? sx : sy;
+    const uint32_t m = other >> 3;
+    return (cm[(((size_t)k * nt + band) * 8 + (other & 7)) * mv.class_words + (m >> 5)] >> (m & 31)) & 1u;
+}
+#endif
+
 // ---- launchers (each returns the number of kernels it launched, or a negative WS_ERR_*) ----------------
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);
+WsMaskView ws_fft_mask_view(const ws_plan* plan);
 int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st);
 int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, int conj_out, cudaStream_t st);
 // xf_lr0 < 0: planes in natural (FFT-native) order; >= 0: log2(N / 256), the planes hold the CONJUGATE of the transform

@@ -16,6 +16,7 @@ WS_GRID_OVERWRITE = 1
 WS_FLAG_LIBRARY_FFT = 1
 WS_FLAG_NO_TRANSPOSE = 2
 WS_GRID_SPARSE = 2
+WS_GRID_SPARSE_ADD = 3
 WS_FFT_USE_OCCUPANCY = 1
 WS_FLAG_TRACK_SUMWT = 4
 WS_FLAG_PRESUM_CHANNELS = 8
@@ -27,8 +28,8 @@ EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
-    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
-    "ws_launch_count",
+    "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_plan_set_e2e_chunk_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
+    "ws_launch_count", "ws_measure_fp32_tflops",
 ]
 
 
@@ -88,11 +89,13 @@ def lib():
         "ws_degrid_visibilities": (C.c_int, [vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
         "ws_predict_visibilities": (C.c_int, [vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, vp, C.c_float, i32, vp, sz, vp]),
         "ws_dev_inputs_bytes": (sz, [i64, i32]),
+        "ws_plan_set_e2e_chunk_bytes": (C.c_int, [vp, sz]),
         "ws_image_from_host": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp, vp, vp, vp, vp, sz, vp]),
         "ws_get_bins": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
                                   C.POINTER(i64), C.POINTER(i64), C.POINTER(i64), vp]),
         "ws_async_status": (C.c_int, [vp, vp]),
         "ws_launch_count": (i64, [vp]),
+        "ws_measure_fp32_tflops": (C.c_int, [vp, C.POINTER(C.c_double), vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -293,6 +296,10 @@ class Plan:
         self._check(lib().ws_get_sum_weights(self._h, C.byref(v), _stream(stream)))
         return v.value
 
+    def set_e2e_chunk_bytes(self, nbytes: int):
+        """Input bytes per pipelined chunk of image_from_host (0: default)."""
+        self._check(lib().ws_plan_set_e2e_chunk_bytes(self._h, int(nbytes)))
+
     @staticmethod
     def dev_inputs_bytes(n_rows: int, n_chan: int) -> int:
         return int(lib().ws_dev_inputs_bytes(n_rows, n_chan))
@@ -311,6 +318,12 @@ class Plan:
             _dev(dev_inputs, torch.uint8, "dev_inputs"), dev_inputs.numel(), _dev(grid, torch.complex64, "grid"),
             _dev(image, torch.complex64, "image"), _dev(dirty_d, torch.float32, "dirty_d"), dirty_h.data_ptr(),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
+
+    def measure_fp32_tflops(self, stream=None) -> float:
+        """Diagnostic: the fp32 FMA rate (TFLOP/s) of a register-only loop on this device."""
+        v = C.c_double()
+        self._check(lib().ws_measure_fp32_tflops(self._h, C.byref(v), _stream(stream)))
+        return v.value
 
     def occupancy(self, stream=None) -> dict:
         """Fractions of the mesh marked non-empty by the gridding calls: tiles, classes, bands, planes."""

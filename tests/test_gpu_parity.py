@@ -362,3 +362,54 @@ def test_nan_coordinates_are_dropped_on_the_gpu(oracle):
     D, G = oracle.dirty_image(prm, *_np(d), return_grid=True)
     U.assert_close(out["grid"], G, "grid with NaN rows")
     U.assert_close(out["image"], D, "image with NaN rows")
+
+
+@pytest.mark.parametrize("squeeze_axis", [0, 1])
+def test_sparse_add_chunks_equal_one_shot(oracle, squeeze_axis):
+    """WS_GRID_SPARSE then WS_GRID_SPARSE_ADD chunks (never a cleared mesh: NaN-filled) = the oracle's image of all the
+    data; chunks overlap in tiles (added to) and bring new tiles (stored), heavy bins included; both orientations."""
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(41 + squeeze_axis, 30000, 2, 512, 5, 7, wavelengths=False, fill=0.9, w_span=50.0, cell_rad=1e-3)
+    d.uvw[:, squeeze_axis] *= 0.3
+    d.uvw[20000:, :2] *= 0.02          # the last chunk piles onto a few tiles: heavy bins that earlier chunks touched
+    plan = U.make_plan(d)
+    dev = d.to("cuda")
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis)
+    grid.fill_(float("nan"))
+    for i, (lo, hi) in enumerate(((0, 7000), (7000, 7100), (7100, 20000), (20000, 30000))):
+        plan.grid_visibilities(dev.uvw[lo:hi].contiguous(), dev.vis[lo:hi].contiguous(), dev.weights[lo:hi].contiguous(),
+                               d.freqs_hz, grid, wsp, mode=ws.WS_GRID_SPARSE if i == 0 else ws.WS_GRID_SPARSE_ADD)
+    plan.fft_wcorrect(grid, image, wsp, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    plan.async_status()
+    assert bool(plan.occupancy()["transposed"]) == (squeeze_axis == 1)
+    prm = U.oracle_params(oracle, d, plan.tile)
+    U.assert_close(image.cpu().numpy(), oracle.dirty_image(prm, *_np(d)), "image from SPARSE + SPARSE_ADD chunks")
+    assert np.array_equal(dirty.cpu().numpy(), image.cpu().numpy().real)
+    other = plan.alloc_grid()
+    with pytest.raises(ws.WStackError):        # only onto the mesh this plan wrote sparsely
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, d.freqs_hz, other, wsp, mode=ws.WS_GRID_SPARSE_ADD)
+
+
+@pytest.mark.parametrize("n_pix,hint", [(256, 0), (256, 50), (128, 0)])
+def test_image_from_host_pipelined_chunks(oracle, n_pix, hint):
+    """ws_image_from_host with many small chunks (copy of chunk c + 1 beside the gridding of chunk c): own FFT
+    (SPARSE + SPARSE_ADD) and the library path (OVERWRITE + ACCUMULATE), with and without the snapshot hint."""
+    d = make_random_dataset(950 + n_pix, 9001, 3, n_pix, 5, 7, wavelengths=False, fill=1.02, w_span=30.0, cell_rad=0.5 / n_pix)
+    plan = U.make_plan(d)
+    if hint:
+        plan.set_snapshot_rows(hint)
+    plan.set_e2e_chunk_bytes(40000)
+    prm = U.oracle_params(oracle, d, 32)
+    D = oracle.dirty_image(prm, *_np(d))
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis)
+    dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device="cuda")
+    uvw_h, vis_h, wt_h = (t.pin_memory() for t in (d.uvw, d.vis, d.weights))
+    dirty_h = torch.full((n_pix, n_pix), float("nan"), dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        grid.fill_(float("nan"))
+        plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+        rel = np.linalg.norm(dirty_h.numpy() - D.real) / np.linalg.norm(D.real)
+        mx = np.abs(dirty_h.numpy() - D.real).max() / np.abs(D).max()
+        assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL, (rel, mx)
