@@ -284,6 +284,8 @@ int ws_plan_destroy(ws_plan* plan) {
     if (plan->e2e_ready) {
         cudaStreamDestroy(plan->copy_stream);
         cudaEventDestroy(plan->ev_start);
+        cudaEventDestroy(plan->ev_orient);
+        cudaFreeHost(plan->h_orient);
         for (int i = 0; i < WS_E2E_MAX_CHUNKS; ++i) cudaEventDestroy(plan->ev_chunk[i]);
     }
     if (plan->fft_ok) cufftDestroy(plan->fft);
@@ -640,7 +642,7 @@ int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t a
     if (!plan->fft_own) return fail(plan, WS_ERR_UNSUPPORTED, "ws_fft_rows_wcorrect: this plan uses the library FFT");
     const int sparse = fft_sparse_flag(plan, grid, fft_flags, "ws_fft_rows_wcorrect: bad fft_flags, or no occupancy recorded for this mesh");
     if (sparse < 0) return sparse;
-    const int rc = ws_launch_fft_rows(plan, (const float2*)grid, (float2*)image, dirty, accumulate, sparse != 0,
+    const int rc = ws_launch_fft_rows(plan, (const float2*)grid, (float2*)image, dirty, accumulate, sparse != 0, 0, 1,
                                       (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_fft_rows_wcorrect: launch failed");
     plan->launches += rc;
@@ -711,7 +713,9 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
     if (!plan->e2e_ready) {
         if ((e = cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
             return cuda_fail(plan, e, "ws_image_from_host: stream");
-        bool ok = cudaEventCreateWithFlags(&plan->ev_start, cudaEventDisableTiming) == cudaSuccess;
+        bool ok = cudaEventCreateWithFlags(&plan->ev_start, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&plan->ev_orient, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaHostAlloc((void**)&plan->h_orient, 64, cudaHostAllocDefault) == cudaSuccess;
         for (int i = 0; i < WS_E2E_MAX_CHUNKS; ++i)
             ok = ok && cudaEventCreateWithFlags(&plan->ev_chunk[i], cudaEventDisableTiming) == cudaSuccess;
         if (!ok) return fail(plan, WS_ERR_CUDA, "ws_image_from_host: events");
@@ -755,8 +759,41 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
         const int rc = ws_grid_visibilities(plan, uvw_d + 3 * r0, vis_d + v0 * 8, wt_d + v0, freq_hz, nr, n_chan, grid, mode,
                                             workspace, workspace_bytes, stream);
         if (rc != WS_OK) return rc;
+        if (c == 0 && plan->fft_own &&        // the orientation the sparse mesh took, for the copy out (read back asynchronously)
+            ((e = cudaMemcpyAsync(plan->h_orient, ws_fft_orientation_flag(plan), 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+             (e = cudaEventRecord(plan->ev_orient, st)) != cudaSuccess))
+            return cuda_fail(plan, e, "ws_image_from_host: orientation read");
     }
     int rc;
+    const size_t N = (size_t)plan->prm.n_pix;
+    const int n_parts = 4;
+    if (plan->fft_own && N >= 8192) {     // (N >= 8192: one row position per item, items ordered by the line they produce)
+        // The row pass in four launches, each producing a quarter of the image lines: the lines of part p travel to
+        // the host (copy stream) while part p + 1 is computed.  Item = v-frequency F, line (F + N/2) mod N; a
+        // transposed mesh yields columns instead, copied as a strided block.
+        if ((rc = ws_fft_columns(plan, grid, WS_FFT_USE_OCCUPANCY, stream)) != WS_OK) return rc;
+        if (cudaEventSynchronize(plan->ev_orient) != cudaSuccess)      // (decided by the first chunk: long since known)
+            return fail(plan, WS_ERR_CUDA, "ws_image_from_host: orientation read");
+        const int32_t tr = *plan->h_orient;
+        for (int p = 0; p < n_parts; ++p) {
+            rc = ws_launch_fft_rows(plan, (const float2*)grid, (float2*)image, dirty_d, 0, true, p, n_parts, st);
+            if (rc < 0) return fail(plan, rc, "ws_image_from_host: launch failed");
+            plan->launches += rc;
+            if ((e = cudaEventRecord(plan->ev_chunk[p], st)) != cudaSuccess ||
+                (e = cudaStreamWaitEvent(plan->copy_stream, plan->ev_chunk[p], 0)) != cudaSuccess)
+                return cuda_fail(plan, e, "ws_image_from_host: event");
+            const size_t l0 = ((size_t)p * (N / n_parts) + N / 2) % N, nl = N / n_parts;     // lines (or columns) of this part
+            if (!tr)
+                e = cudaMemcpyAsync(dirty_h + l0 * N, dirty_d + l0 * N, nl * N * 4, cudaMemcpyDeviceToHost, plan->copy_stream);
+            else
+                e = cudaMemcpy2DAsync(dirty_h + l0, N * 4, dirty_d + l0, N * 4, nl * 4, N, cudaMemcpyDeviceToHost, plan->copy_stream);
+            if (e != cudaSuccess) return cuda_fail(plan, e, "ws_image_from_host: D2H copy");
+        }
+        if ((e = cudaEventRecord(plan->ev_start, plan->copy_stream)) != cudaSuccess ||
+            (e = cudaStreamWaitEvent(st, plan->ev_start, 0)) != cudaSuccess)
+            return cuda_fail(plan, e, "ws_image_from_host: event");
+        return ws_async_status(plan, stream);
+    }
     if ((rc = ws_fft_wcorrect(plan, grid, image, 0, dirty_d, plan->fft_own ? WS_FFT_USE_OCCUPANCY : 0u, workspace,
                               workspace_bytes, stream)) != WS_OK)
         return rc;

@@ -750,7 +750,7 @@ template <int LOGN>
 __global__ void __launch_bounds__(FT + PT, 1)
 k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ planes, float2* __restrict__ image,
            float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g, const float2* __restrict__ tc_g,
-           const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_super) {
+           const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t item_lo, uint32_t n_super) {
     using C = RowCfg<LOGN>;
     constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0, LAND = C::LAND, BW = C::BW;
     // occupancy: the band masks of the orientation the mesh is stored in; transposed: the mesh is [k][u][v], i.e. a
@@ -783,7 +783,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         mbar_init(empty, C::GROUPED ? 2 : 1);
     }
     __syncthreads();
-    if (blockIdx.x >= n_super) return;
+    if (item_lo + blockIdx.x >= n_super) return;       // items [item_lo, n_super) belong to this launch
 
     if (u >= FT) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
@@ -794,7 +794,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         const int lane = u & 31;
         uint32_t was = 0, e_parity = 0;
         bool first = true;
-        for (uint32_t it = blockIdx.x; it < n_super; it += gridDim.x) {
+        for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
             const uint32_t sr = super_row_of<LOGN>(it);
             for (int k = nw - 1; k >= 0; --k) {
                 if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
@@ -866,7 +866,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         for (int i = 0; i < 3; ++i) tc[4 + i] = __ldg(tc_g + (16 + i) * 256 + (u & 255));
     }
 
-    for (uint32_t it = blockIdx.x; it < n_super; it += gridDim.x) {
+    for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
         const uint32_t sr = super_row_of<LOGN>(it);
         float2 rot[EPT], h[EPT];
 #pragma unroll
@@ -1066,9 +1066,11 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
     return cudaGetLastError() == cudaSuccess ? launches : WS_ERR_CUDA;
 }
 
+// part / n_parts: the launch covers that share of the image lines (items are ordered by the line they produce), so
+// that a caller can start copying finished lines out while the rest is computed; 0 / 1: everything
 template <int LOGN>
 int launch_rows_n(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
-                  cudaStream_t st) {
+                  int part, int n_parts, cudaStream_t st) {
     constexpr int N = 1 << LOGN;
     const ws_params& P = plan->prm;
     WcParams prm;
@@ -1077,14 +1079,16 @@ int launch_rows_n(ws_plan* plan, const float2* grid, float2* image, float* dirty
     prm.cell = P.cell_rad;
     prm.dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
     prm.w0 = P.w_min + 0.5 * prm.dw;
-    const uint32_t n_super = (uint32_t)(((size_t)N * N) / RowCfg<LOGN>::LAND) * RowCfg<LOGN>::ITEMS_PER_ROW;
-    uint32_t ctas = n_super < (uint32_t)plan->sm_count ? n_super : (uint32_t)plan->sm_count;
-    if (RowCfg<LOGN>::ITEMS_PER_ROW == 2) ctas &= ~1u;      // even grid: a CTA keeps the parity of its first item
+    const uint32_t n_all = (uint32_t)(((size_t)N * N) / RowCfg<LOGN>::LAND) * RowCfg<LOGN>::ITEMS_PER_ROW;
+    if (n_parts < 1 || part < 0 || part >= n_parts || n_all % (uint32_t)(2 * n_parts) != 0) return WS_ERR_INVALID_ARG;
+    const uint32_t lo = n_all / (uint32_t)n_parts * (uint32_t)part, hi = lo + n_all / (uint32_t)n_parts, n_items = hi - lo;
+    uint32_t ctas = n_items < (uint32_t)plan->sm_count ? n_items : (uint32_t)plan->sm_count;
+    if (RowCfg<LOGN>::ITEMS_PER_ROW == 2) ctas &= ~1u;      // even grid (and even item_lo): a CTA keeps the parity of its first item
     const uint32_t* bm = sparse ? (const uint32_t*)plan->d_masks : nullptr;
     k_fft_rows<LOGN><<<ctas, FT + PT, rows_smem<LOGN>(), st>>>(prm, grid, image, dirty, accumulate,
                                                           (const float2*)plan->d_twiddles,
                                                           (const float2*)plan->d_twiddles + plan->tw_off_c, bm,
-                                                          (uint32_t)plan->mask_set_words, n_super);
+                                                          (uint32_t)plan->mask_set_words, lo, hi);
     return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
 }
 
@@ -1117,8 +1121,8 @@ int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st
 }
 
 int ws_launch_fft_rows(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
-                       cudaStream_t st) {
-    WS_FFT_DISPATCH(launch_rows_n, plan, grid, image, dirty, accumulate, sparse, st)
+                       int part, int n_parts, cudaStream_t st) {
+    WS_FFT_DISPATCH(launch_rows_n, plan, grid, image, dirty, accumulate, sparse, part, n_parts, st)
 }
 
 int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st) {

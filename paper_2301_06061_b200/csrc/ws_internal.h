@@ -109,6 +109,8 @@ struct ws_plan {
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
     cudaStream_t copy_stream;                   // ws_image_from_host: the H2D copies of the next chunk run beside the gridding
     cudaEvent_t ev_start, ev_chunk[WS_E2E_MAX_CHUNKS];    // of this one (created on first use)
+    cudaEvent_t ev_orient;
+    int32_t* h_orient;                          // pinned host word: the orientation flag of the sparse mesh, read back asynchronously
     bool e2e_ready;
     size_t e2e_chunk_bytes;                     // input bytes per chunk (0: 160 MiB)
     const void* occ_grid;                       // mesh the masks describe (NULL: none)
@@ -164,7 +166,7 @@ bool ws_fft_own_supported(int n_pix, int n_wplanes);
 int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error
 int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st);
 int ws_launch_fft_rows(ws_plan* plan, const float2* grid, float2* image, float* dirty, int accumulate, bool sparse,
-                       cudaStream_t st);
+                       int part, int n_parts, cudaStream_t st);
 int ws_launch_fft_masks_clear(ws_plan* plan, cudaStream_t st);
 int ws_launch_fft_masks(ws_plan* plan, const uint32_t* rec_start, int decide, cudaStream_t st);
 const uint32_t* ws_fft_orientation_flag(const ws_plan* plan);   // device word: 1 = the sparse mesh is stored transposed

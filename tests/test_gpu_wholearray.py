@@ -227,3 +227,28 @@ def test_extreme_whole_mesh_and_image(oracle):
     """Extreme (4 x 10^8 visibilities, 16384^2 x 32, S = 9) in ONE call: all 32 planes of the sparse mesh, the whole
     16384^2 image of the timed path (own FFT for N = 16384) and of the dense own FFT, four planes of the OVERWRITE mesh."""
     _whole_config(oracle, "extreme", one_mesh=True, dup_factor=2.0)
+
+
+@pytest.mark.parametrize("squeeze_axis", [0, 1])
+def test_image_from_host_at_8192_both_orientations(oracle, squeeze_axis):
+    """The end-to-end entry at N = 8192: pipelined input chunks, the row pass in four launches whose image lines (or
+    columns, for a transposed mesh) are copied out while the next part is computed."""
+    n_pix = 8192
+    d = make_random_dataset(70 + squeeze_axis, 150000, 2, n_pix, 3, 7, wavelengths=False, fill=0.9, w_span=80.0, cell_rad=0.5 / n_pix)
+    d.uvw[:, squeeze_axis] *= 0.15
+    plan = U.make_plan(d)
+    plan.set_e2e_chunk_bytes(1 << 20)
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = plan.alloc_workspace(d.n_vis)
+    dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device="cuda")
+    uvw_h, vis_h, wt_h = (t.pin_memory() for t in (d.uvw, d.vis, d.weights))
+    dirty_h = torch.full((n_pix, n_pix), float("nan"), dtype=torch.float32).pin_memory()
+    grid.fill_(float("nan"))
+    plan.image_from_host(uvw_h, vis_h, wt_h, d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+    assert bool(plan.occupancy()["transposed"]) == (squeeze_axis == 1)
+    prm = U.oracle_params(oracle, d, plan.tile)
+    D = torch.from_numpy(oracle.dirty_image(prm, *_np(d))).cuda()
+    e = Running(f"image_from_host at 8192, squeezed along axis {squeeze_axis}")
+    e.add(image, D)
+    e.check()
+    assert torch.equal(dirty_h.cuda(), image.real)
