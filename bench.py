@@ -184,6 +184,69 @@ def workload_config(d, cfg_name):
                   ((12 * d.n_rows + 12 * d.n_vis) / 1e9, 8.0 * d.n_pix ** 2 * d.n_wplanes / 1e9)}
 
 
+def run_f64(args, ws, d, cfg, local_rank, world, dist):
+    """The path in the paper's own arithmetic (PAPER.md:392, Table 3: fp64 mesh; :207, :219: one thread per measurement,
+    atomicAdd on the mesh): zero -> grid -> cuFFT Z2Z -> w-correction, all fp64.  Context against the paper's Table 4
+    (other hardware, its own data), not the headline."""
+    presum = d.freqs_hz is None and d.n_chan > 1
+    flags = ws.WS_FLAG_MESH_F64 | (ws.WS_FLAG_PRESUM_CHANNELS if presum else 0)
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells, device=local_rank, flags=flags)
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    wsp = torch.empty(max(plan.fft_workspace_bytes(), 256), dtype=torch.uint8, device=f"cuda:{local_rank}")
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        plan.grid_zero(grid)
+        if ev: ev[1].record()
+        plan.grid_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_ACCUMULATE)
+        if ev: ev[2].record()
+        plan.fft_planes(grid, wsp)
+        if ev: ev[3].record()
+        plan.wcorrect_accumulate(grid, image, accumulate=False, dirty=dirty)
+        if ev: ev[4].record()
+
+    for _ in range(args.warmup):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    clocks = ClockSampler(local_rank)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    clocks.start()
+    l0 = plan.launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for i in range(args.steps):
+        step(evs[i])
+    t1.record()
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    launches = plan.launch_count() - l0
+    clk = clocks.stop()
+    ms_step = reduce_max_ms(t0.elapsed_time(t1), dist, f"cuda:{local_rank}") / args.steps
+    med = np.median(np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs]), axis=0)
+    peak, peak_src = peaks()
+    mesh_b = 16.0 * d.n_pix ** 2 * d.n_wplanes
+    alg = {"zero": mesh_b, "k_grid_f64": 12.0 * d.n_rows + 12.0 * d.n_vis + mesh_b, "cufft_z2z": 2 * mesh_b,
+           "k_wcorrect_f64": mesh_b + 24.0 * d.n_pix ** 2}
+    names = list(alg)
+    own_k = {"k_grid_f64": med[1], "k_wcorrect_f64": med[3]}
+    dom = max(own_k, key=own_k.get)
+    ach = alg[dom] / (own_k[dom] * 1e-3) / 1e9
+    return {"metric": METRIC, "value": whole_job_value(d.n_vis, world, ms_step), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(d, cfg.name), "clocks": clk,
+            "gpu_launches": int(launches), "stages_ms_median": {n: float(v) for n, v in zip(names, med)},
+            "fft": "cuFFT Z2Z", "presummed_channels": bool(presum),
+            "ggpas": d.n_vis * d.support ** 2 / (med[1] * 1e-3) / 1e9,
+            "mvis_per_s_gridding": d.n_vis / (med[1] * 1e-3) / 1e6,
+            "kernels": {n: {"ms": float(t), "alg_GB": alg[n] / 1e9, "GBps": alg[n] / (t * 1e-3) / 1e9} for n, t in zip(names, med)},
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                         "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
+                         "launch_ms": float(own_k[dom]),
+                         "note": "atomicAdd(double) gridder: bound by the L2 atomic rate on the dense core, not by HBM"}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -197,6 +260,8 @@ def main():
     ap.add_argument("--no-degrid", action="store_true")
     ap.add_argument("--no-snapshot-hint", action="store_true")
     ap.add_argument("--chunked", action="store_true", help="configs with n_chunks > 1: grid the row chunks one call at a time")
+    ap.add_argument("--mesh-f64", action="store_true",
+                    help="the paper's arithmetic (WS_FLAG_MESH_F64: fp64 mesh, atomicAdd gridder, cuFFT Z2Z): context line, see run_f64()")
     args = ap.parse_args()
     global KERNEL
     KERNEL = args.kernel
@@ -225,6 +290,13 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
 
     d = make_dataset(cfg, device=f"cuda:{local_rank}")
+    if args.mesh_f64:
+        out = run_f64(args, ws, d, cfg, local_rank, world, dist)
+        if rank == 0:
+            print(json.dumps(out), flush=True)
+        if dist:
+            dist.destroy_process_group()
+        return
     # the paper's narrow-band mode (shared uvw): sum the channels of a row first, bin rows
     presum = d.freqs_hz is None and d.n_chan > 1
     flags = ws.WS_FLAG_PRESUM_CHANNELS if presum else 0

@@ -88,6 +88,15 @@ extern "C" {
                                      exports are then per row (n_vis = n_rows).  Ignored by ws_degrid_visibilities; a
                                      gridding call with freq_hz != NULL on such a plan is WS_ERR_INVALID_ARG */
 
+#define WS_FLAG_MESH_F64 16u /* the paper's own arithmetic (Table 3: fp64 mesh, real and imaginary part): grid, image
+                               and dirty image are complex128 / complex128 / float64 (sizes from ws_grid_bytes etc.), taps and phases
+                               are evaluated in fp64.  For like-for-like context against the paper's Table 4, not for speed: the
+                               gridder is the paper's own kernel shape, one thread per measurement with atomicAdd on the mesh
+                               (:207, :219; nothing is binned, no workspace needed, ws_get_bins has nothing to export), the FFT is
+                               cuFFT Z2Z.  Calls: ws_grid_zero, ws_grid_visibilities (ACCUMULATE / OVERWRITE), ws_fft_planes,
+                               ws_wcorrect_accumulate, ws_fft_wcorrect (= the two), ws_dirty_image, ws_get_sum_weights; every
+                               other entry returns WS_ERR_UNSUPPORTED.  With WS_FLAG_PRESUM_CHANNELS a thread takes a whole row */
+
 /* kernel_type: the separable 1-D convolution function g(x), x in cells, unit integral (R2, R28) */
 #define WS_KERNEL_GAUSSIAN 0      /* g(x) = exp(-x^2 / (2 sigma^2)) / (sigma sqrt(2 pi)), kernel_param = sigma */
 #define WS_KERNEL_KAISER_BESSEL 1 /* g(x) = I0(beta sqrt(1 - (2x/S)^2)) beta / (S sinh beta) on |x| <= S/2, kernel_param =

@@ -71,7 +71,7 @@ bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out,
 
 int make_fft_plan(ws_plan* plan) {
     const long long n[2] = {plan->prm.n_pix, plan->prm.n_pix};
-    const size_t plane_bytes = (size_t)plan->prm.n_pix * plan->prm.n_pix * 8;
+    const size_t plane_bytes = (size_t)plan->prm.n_pix * plan->prm.n_pix * ((plan->prm.flags & WS_FLAG_MESH_F64) ? 16 : 8);
     // all planes in one batched transform unless its work area is out of proportion; else plane by plane
     for (int attempt = 0; attempt < 2; ++attempt) {
         const int batch = attempt == 0 ? plan->prm.n_wplanes : 1;
@@ -79,8 +79,8 @@ int make_fft_plan(ws_plan* plan) {
         if (cufftCreate(&h) != CUFFT_SUCCESS) return WS_ERR_CUFFT;
         size_t work = 0;
         if (cufftSetAutoAllocation(h, 0) != CUFFT_SUCCESS ||
-            cufftMakePlanMany64(h, 2, const_cast<long long*>(n), nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2C, batch, &work) !=
-                CUFFT_SUCCESS) {
+            cufftMakePlanMany64(h, 2, const_cast<long long*>(n), nullptr, 1, 0, nullptr, 1, 0,
+                                (plan->prm.flags & WS_FLAG_MESH_F64) ? CUFFT_Z2Z : CUFFT_C2C, batch, &work) != CUFFT_SUCCESS) {
             cufftDestroy(h);
             if (attempt == 0) continue;
             return WS_ERR_CUFFT;
@@ -170,7 +170,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     if (p->n_pix <= 0 || p->n_wplanes <= 0 || p->support <= 0 || (p->support & 1) == 0) return WS_ERR_INVALID_ARG;
     if (!(p->kernel_param > 0.0) || !(p->cell_rad > 0.0) || !(p->w_max > p->w_min)) return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->w_min) || !std::isfinite(p->w_max) || !std::isfinite(p->cell_rad)) return WS_ERR_INVALID_ARG;
-    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE | WS_FLAG_TRACK_SUMWT | WS_FLAG_PRESUM_CHANNELS)) != 0 ||
+    if ((p->flags & ~(uint32_t)(WS_FLAG_LIBRARY_FFT | WS_FLAG_NO_TRANSPOSE | WS_FLAG_TRACK_SUMWT | WS_FLAG_PRESUM_CHANNELS |
+                                WS_FLAG_MESH_F64)) != 0 ||
         p->device < 0)
         return WS_ERR_INVALID_ARG;
     if (!std::isfinite(p->kernel_param)) return WS_ERR_INVALID_ARG;
@@ -236,7 +237,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
         }
     }
     // a3: the FFT of ws_fft.cu where it exists (N = 2^8 .. 2^13), else (or on request) the library's
-    plan->fft_own = !(p->flags & WS_FLAG_LIBRARY_FFT) && ws_fft_own_supported(p->n_pix, p->n_wplanes);
+    plan->fft_own = !(p->flags & (WS_FLAG_LIBRARY_FFT | WS_FLAG_MESH_F64)) && ws_fft_own_supported(p->n_pix, p->n_wplanes);
     plan->e2e_ready = false;
     plan->e2e_chunk_bytes = 0;
     plan->d_twiddles = nullptr;
@@ -313,11 +314,13 @@ int ws_plan_set_e2e_chunk_bytes(ws_plan* plan, size_t bytes) {
     return WS_OK;
 }
 
+static inline size_t f64_factor(const ws_plan* plan) { return (plan->prm.flags & WS_FLAG_MESH_F64) ? 2 : 1; }
+static inline bool is_f64(const ws_plan* plan) { return (plan->prm.flags & WS_FLAG_MESH_F64) != 0; }
 size_t ws_grid_bytes(const ws_plan* plan) {
-    return plan ? (size_t)8 * plan->prm.n_pix * plan->prm.n_pix * plan->prm.n_wplanes : 0;
+    return plan ? f64_factor(plan) * 8 * plan->prm.n_pix * plan->prm.n_pix * plan->prm.n_wplanes : 0;
 }
-size_t ws_image_bytes(const ws_plan* plan) { return plan ? (size_t)8 * plan->prm.n_pix * plan->prm.n_pix : 0; }
-size_t ws_dirty_bytes(const ws_plan* plan) { return plan ? (size_t)4 * plan->prm.n_pix * plan->prm.n_pix : 0; }
+size_t ws_image_bytes(const ws_plan* plan) { return plan ? f64_factor(plan) * 8 * plan->prm.n_pix * plan->prm.n_pix : 0; }
+size_t ws_dirty_bytes(const ws_plan* plan) { return plan ? f64_factor(plan) * 4 * plan->prm.n_pix * plan->prm.n_pix : 0; }
 size_t ws_fft_workspace_bytes(const ws_plan* plan) { return plan ? plan->fft_work_bytes : 0; }
 int ws_plan_tile(const ws_plan* plan) { return plan ? WS_TILE : 0; }
 int ws_plan_fft_is_own(const ws_plan* plan) { return plan && plan->fft_own ? 1 : 0; }
@@ -347,10 +350,32 @@ int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     return WS_OK;
 }
 
+// O1: per-channel constants, fp64, in exactly this operation order (the bit-exact bin contract)
+static int make_chan_consts(ws_plan* plan, const double* freq_hz, int32_t n_chan, WsChanConsts& cc) {
+    const ws_params& P = plan->prm;
+    std::memset(&cc, 0, sizeof(cc));
+    const double dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
+    for (int c = 0; c < n_chan; ++c) {
+        if (freq_hz) {
+            if (!(freq_hz[c] > 0.0) || !std::isfinite(freq_hz[c]))
+                return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad frequency");
+            cc.su[c] = (freq_hz[c] / C_LIGHT) * ((double)P.n_pix * P.cell_rad);
+            cc.sw[c] = (freq_hz[c] / C_LIGHT) / dw;
+        } else {
+            cc.su[c] = (double)P.n_pix * P.cell_rad;
+            cc.sw[c] = 1.0 / dw;
+        }
+    }
+    cc.ow = -P.w_min / dw;
+    cc.half = (double)(P.n_pix / 2);
+    return WS_OK;
+}
+
 // a1 for the gridder (with_values) and for the degridder (positions only: vis and weights are not read)
 static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const float* weights, const double* freq_hz,
                     int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values) {
     if (!plan) return WS_ERR_INVALID_ARG;
+    if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "WS_FLAG_MESH_F64: nothing is binned (ws_grid_visibilities grids directly); no degridding");
     if (n_rows < 0 || n_chan <= 0) return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad n_rows / n_chan");
     if (n_chan > WS_MAX_CHAN) return fail(plan, WS_ERR_UNSUPPORTED, "ws_bin_visibilities: n_chan > 128");
     if (n_rows > MAX_VIS || n_rows * n_chan > MAX_VIS)
@@ -383,24 +408,9 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
         n_chan = 1;
     }
 
-    // O1: per-channel constants, fp64, in exactly this operation order (the bit-exact bin contract)
-    const ws_params& P = plan->prm;
     WsChanConsts cc;
-    std::memset(&cc, 0, sizeof(cc));
-    const double dw = (P.w_max - P.w_min) / (double)P.n_wplanes;
-    for (int c = 0; c < n_chan; ++c) {
-        if (freq_hz) {
-            if (!(freq_hz[c] > 0.0) || !std::isfinite(freq_hz[c]))
-                return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad frequency");
-            cc.su[c] = (freq_hz[c] / C_LIGHT) * ((double)P.n_pix * P.cell_rad);
-            cc.sw[c] = (freq_hz[c] / C_LIGHT) / dw;
-        } else {
-            cc.su[c] = (double)P.n_pix * P.cell_rad;
-            cc.sw[c] = 1.0 / dw;
-        }
-    }
-    cc.ow = -P.w_min / dw;
-    cc.half = (double)(P.n_pix / 2);
+    const int crc = make_chan_consts(plan, freq_hz, n_chan, cc);
+    if (crc != WS_OK) return crc;
 
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
@@ -485,6 +495,32 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
     if (!grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
     if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: bad mode");
+    if (is_f64(plan)) {    // fp64 mesh: one thread per measurement, atomicAdd on the mesh (ws_f64.cu); nothing is binned
+        if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE)
+            return fail(plan, WS_ERR_UNSUPPORTED, "ws_grid_visibilities: WS_FLAG_MESH_F64 grids with WS_GRID_ACCUMULATE or WS_GRID_OVERWRITE");
+        if (n_rows < 0 || n_chan <= 0 || n_chan > WS_MAX_CHAN || n_rows > MAX_VIS || n_rows * n_chan > MAX_VIS)
+            return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: bad n_rows / n_chan");
+        if (n_rows > 0 && (!uvw || !vis || !weights)) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
+        if (((uintptr_t)uvw | (uintptr_t)vis | (uintptr_t)weights | (uintptr_t)grid) & 15)
+            return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: pointers must be 16-byte aligned");
+        const bool presum = (plan->prm.flags & WS_FLAG_PRESUM_CHANNELS) != 0;
+        if (presum && freq_hz)
+            return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: WS_FLAG_PRESUM_CHANNELS needs freq_hz == NULL (shared uvw)");
+        WsChanConsts cc;
+        int rc = make_chan_consts(plan, freq_hz, n_chan, cc);
+        if (rc != WS_OK) return rc;
+        cudaStream_t st = (cudaStream_t)stream;
+        if (mode == WS_GRID_OVERWRITE) {
+            if (cudaMemsetAsync(grid, 0, ws_grid_bytes(plan), st) != cudaSuccess ||
+                cudaMemsetAsync(plan->d_sumwt, 0, sizeof(double), st) != cudaSuccess)
+                return fail(plan, WS_ERR_CUDA, "ws_grid_visibilities: memset failed");
+        }
+        plan->last_valid = false;
+        rc = ws_launch_grid_f64(plan, cc, uvw, (const float2*)vis, weights, n_rows, n_chan, presum ? 1 : 0, (double*)grid, st);
+        if (rc < 0) return fail(plan, rc, "ws_grid_visibilities: launch failed");
+        plan->launches += rc;
+        return WS_OK;
+    }
     const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
     return ws_grid_binned(plan, grid, mode, workspace, workspace_bytes, stream);
@@ -503,6 +539,12 @@ static int fft_planes_dir(ws_plan* plan, void* grid, void* workspace, size_t wor
     plan->last_valid = plan->last_valid && plan->fft_work_bytes == 0;
     const size_t plane = (size_t)plan->prm.n_pix * plan->prm.n_pix;
     for (int k = 0; k < plan->prm.n_wplanes; k += plan->fft_batch) {
+        if (is_f64(plan)) {
+            cufftDoubleComplex* p = (cufftDoubleComplex*)grid + (size_t)k * plane;
+            if (cufftExecZ2Z(plan->fft, p, p, direction) != CUFFT_SUCCESS)
+                return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftExecZ2Z");
+            continue;
+        }
         cufftComplex* p = (cufftComplex*)grid + (size_t)k * plane;
         if (cufftExecC2C(plan->fft, p, p, direction) != CUFFT_SUCCESS)
             return fail(plan, WS_ERR_CUFFT, "ws_fft_planes: cufftExecC2C");
@@ -517,6 +559,7 @@ int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_b
 int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void* workspace, size_t workspace_bytes,
                       void* stream) {
     if (!plan || !model_image || !planes) return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_planes: null argument");
+    if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "ws_predict_planes: no degridding with WS_FLAG_MESH_F64");
     if (((uintptr_t)model_image | (uintptr_t)planes) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_planes: pointers must be 16-byte aligned");
     if (plan->fft_work_bytes > 0 && (!workspace || workspace_bytes < plan->fft_work_bytes))
@@ -607,7 +650,8 @@ int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32
     if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: bad flag");
     if (((uintptr_t)planes | (uintptr_t)image | (uintptr_t)dirty) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: pointers must be 16-byte aligned");
-    const int rc = ws_launch_wcorrect(plan, (const float2*)planes, (float2*)image, accumulate, dirty, (cudaStream_t)stream);
+    const int rc = is_f64(plan) ? ws_launch_wcorrect_f64(plan, planes, image, accumulate, dirty, (cudaStream_t)stream)
+                                : ws_launch_wcorrect(plan, (const float2*)planes, (float2*)image, accumulate, dirty, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_wcorrect_accumulate: launch failed");
     plan->launches += rc;
     return WS_OK;
@@ -671,7 +715,8 @@ int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm
         return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: WS_NORM_SUMWT needs a plan created with WS_FLAG_TRACK_SUMWT");
     if (((uintptr_t)image | (uintptr_t)dirty) & 15)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: pointers must be 16-byte aligned");
-    const int rc = ws_launch_dirty(plan, (const float2*)image, dirty, norm_flags, (cudaStream_t)stream);
+    const int rc = is_f64(plan) ? ws_launch_dirty_f64(plan, image, dirty, norm_flags, (cudaStream_t)stream)
+                                : ws_launch_dirty(plan, (const float2*)image, dirty, norm_flags, (cudaStream_t)stream);
     if (rc < 0) return fail(plan, rc, "ws_dirty_image: launch failed");
     plan->launches += rc;
     return WS_OK;
@@ -703,6 +748,7 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
         return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: null argument");
     if (n_rows <= 0 || n_chan <= 0 || n_rows * n_chan > MAX_VIS)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: bad sizes");
+    if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "ws_image_from_host: not with WS_FLAG_MESH_F64");
     const size_t n_vis = (size_t)n_rows * n_chan;
     // every sub-buffer starts on a 16-byte boundary (bin_impl's alignment rule): uvw | vis | weights
     const size_t b_uvw = ws_align_up((size_t)n_rows * 12, 16), b_vis = ws_align_up(n_vis * 8, 16), b_wt = n_vis * 4;

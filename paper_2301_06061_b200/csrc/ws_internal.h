@@ -162,6 +162,11 @@ int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const floa
 int ws_launch_presum(ws_plan* plan, const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, float2* out,
                      cudaStream_t st);
 int ws_launch_zero(ws_plan* plan, void* ptr, size_t bytes, cudaStream_t st);
+// WS_FLAG_MESH_F64 (ws_f64.cu): fp64 mesh, image and dirty image
+int ws_launch_grid_f64(ws_plan* plan, const WsChanConsts& cc, const float* uvw, const float2* vis, const float* wt,
+                       int64_t n_rows, int32_t n_chan, int presum, double* grid, cudaStream_t st);
+int ws_launch_wcorrect_f64(ws_plan* plan, const void* planes, void* image, int accumulate, void* dirty, cudaStream_t st);
+int ws_launch_dirty_f64(ws_plan* plan, const void* image, void* dirty, uint32_t norm_flags, cudaStream_t st);
 bool ws_fft_own_supported(int n_pix, int n_wplanes);
 int ws_fft_own_init(ws_plan* plan);             // twiddle table + kernel attributes; WS_OK or an error
 int ws_launch_fft_cols(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st);

@@ -20,6 +20,7 @@ WS_GRID_SPARSE_ADD = 3
 WS_FFT_USE_OCCUPANCY = 1
 WS_FLAG_TRACK_SUMWT = 4
 WS_FLAG_PRESUM_CHANNELS = 8
+WS_FLAG_MESH_F64 = 16
 WS_KERNEL_GAUSSIAN = 0
 WS_KERNEL_KAISER_BESSEL = 1
 WS_NORM_SUMWT, WS_NORM_N, WS_NORM_TAPER = 1, 2, 4
@@ -140,6 +141,8 @@ class Plan:
             self._h = C.c_void_p()
             raise WStackError(rc, lib().ws_strerror(rc).decode())
         self.n_pix, self.n_wplanes, self.support, self.device = n_pix, n_wplanes, support, device
+        f64 = bool(flags & WS_FLAG_MESH_F64)        # fp64 mesh: complex128 grid / image, float64 dirty image
+        self._c, self._r = (torch.complex128, torch.float64) if f64 else (torch.complex64, torch.float32)
 
     # -- plumbing ---------------------------------------------------------------------------------------
     def _check(self, rc: int):
@@ -193,13 +196,13 @@ class Plan:
 
     # -- allocation helpers (torch owns the memory) ------------------------------------------------------
     def alloc_grid(self) -> torch.Tensor:
-        return torch.empty((self.n_wplanes, self.n_pix, self.n_pix), dtype=torch.complex64, device=f"cuda:{self.device}")
+        return torch.empty((self.n_wplanes, self.n_pix, self.n_pix), dtype=self._c, device=f"cuda:{self.device}")
 
     def alloc_image(self) -> torch.Tensor:
-        return torch.empty((self.n_pix, self.n_pix), dtype=torch.complex64, device=f"cuda:{self.device}")
+        return torch.empty((self.n_pix, self.n_pix), dtype=self._c, device=f"cuda:{self.device}")
 
     def alloc_dirty(self) -> torch.Tensor:
-        return torch.empty((self.n_pix, self.n_pix), dtype=torch.float32, device=f"cuda:{self.device}")
+        return torch.empty((self.n_pix, self.n_pix), dtype=self._r, device=f"cuda:{self.device}")
 
     def alloc_workspace(self, max_vis: int, dup_factor: Optional[float] = None) -> torch.Tensor:
         n = self.workspace_bytes(max_vis, dup_factor)
@@ -207,7 +210,7 @@ class Plan:
 
     # -- the chain --------------------------------------------------------------------------------------
     def grid_zero(self, grid: torch.Tensor, stream=None):
-        self._check(lib().ws_grid_zero(self._h, _dev(grid, torch.complex64, "grid"), _stream(stream)))
+        self._check(lib().ws_grid_zero(self._h, _dev(grid, self._c, "grid"), _stream(stream)))
 
     def grid_visibilities(self, uvw, vis, weights, freq_hz, grid, workspace, mode: int = WS_GRID_OVERWRITE, stream=None):
         n_rows = int(uvw.shape[0])
@@ -215,7 +218,7 @@ class Plan:
         keep, fp = _freq(freq_hz, n_chan)
         self._check(lib().ws_grid_visibilities(
             self._h, _dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"),
-            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan, _dev(grid, torch.complex64, "grid"), mode,
+            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan, _dev(grid, self._c, "grid"), mode,
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
 
@@ -230,43 +233,43 @@ class Plan:
         self._ws = workspace
 
     def grid_binned(self, grid, workspace, mode: int = WS_GRID_OVERWRITE, stream=None):
-        self._check(lib().ws_grid_binned(self._h, _dev(grid, torch.complex64, "grid"), mode,
+        self._check(lib().ws_grid_binned(self._h, _dev(grid, self._c, "grid"), mode,
                                          _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
 
     def fft_planes(self, grid, workspace, stream=None):
-        self._check(lib().ws_fft_planes(self._h, _dev(grid, torch.complex64, "grid"),
+        self._check(lib().ws_fft_planes(self._h, _dev(grid, self._c, "grid"),
                                         _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
 
     def wcorrect_accumulate(self, planes, image, accumulate: bool = False, dirty=None, stream=None):
-        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
-        self._check(lib().ws_wcorrect_accumulate(self._h, _dev(planes, torch.complex64, "planes"),
-                                                 _dev(image, torch.complex64, "image"), int(accumulate), d,
+        d = None if dirty is None else _dev(dirty, self._r, "dirty")
+        self._check(lib().ws_wcorrect_accumulate(self._h, _dev(planes, self._c, "planes"),
+                                                 _dev(image, self._c, "image"), int(accumulate), d,
                                                  _stream(stream)))
 
     def fft_wcorrect(self, grid, image, workspace, accumulate: bool = False, dirty=None, fft_flags: int = 0, stream=None):
         """a3 + a4 in one call (the mesh is destroyed)."""
-        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
-        self._check(lib().ws_fft_wcorrect(self._h, _dev(grid, torch.complex64, "grid"),
-                                          _dev(image, torch.complex64, "image"), int(accumulate), d, fft_flags,
+        d = None if dirty is None else _dev(dirty, self._r, "dirty")
+        self._check(lib().ws_fft_wcorrect(self._h, _dev(grid, self._c, "grid"),
+                                          _dev(image, self._c, "image"), int(accumulate), d, fft_flags,
                                           _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
 
     def fft_columns(self, grid, fft_flags: int = 0, stream=None):
-        self._check(lib().ws_fft_columns(self._h, _dev(grid, torch.complex64, "grid"), fft_flags, _stream(stream)))
+        self._check(lib().ws_fft_columns(self._h, _dev(grid, self._c, "grid"), fft_flags, _stream(stream)))
 
     def fft_rows_wcorrect(self, grid, image, accumulate: bool = False, dirty=None, fft_flags: int = 0, stream=None):
-        d = None if dirty is None else _dev(dirty, torch.float32, "dirty")
-        self._check(lib().ws_fft_rows_wcorrect(self._h, _dev(grid, torch.complex64, "grid"),
-                                               _dev(image, torch.complex64, "image"), int(accumulate), d, fft_flags,
+        d = None if dirty is None else _dev(dirty, self._r, "dirty")
+        self._check(lib().ws_fft_rows_wcorrect(self._h, _dev(grid, self._c, "grid"),
+                                               _dev(image, self._c, "image"), int(accumulate), d, fft_flags,
                                                _stream(stream)))
 
     def dirty_image(self, image, dirty, norm_flags: int = 0, stream=None):
-        self._check(lib().ws_dirty_image(self._h, _dev(image, torch.complex64, "image"),
-                                         _dev(dirty, torch.float32, "dirty"), norm_flags, _stream(stream)))
+        self._check(lib().ws_dirty_image(self._h, _dev(image, self._c, "image"),
+                                         _dev(dirty, self._r, "dirty"), norm_flags, _stream(stream)))
 
     def predict_planes(self, model_image, planes, workspace, stream=None):
         """Degridding steps 1-2: planes[k] = forward FFT of model_image x exp(-2 pi i w_k (n - 1))."""
         self._check(lib().ws_predict_planes(self._h, _dev(model_image, torch.complex64, "model_image"),
-                                            _dev(planes, torch.complex64, "planes"),
+                                            _dev(planes, self._c, "planes"),
                                             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
 
     def degrid_visibilities(self, uvw, freq_hz, n_chan: int, planes, vis_out, workspace, scale: float = 1.0,
@@ -275,7 +278,7 @@ class Plan:
         n_rows = int(uvw.shape[0])
         keep, fp = _freq(freq_hz, n_chan)
         self._check(lib().ws_degrid_visibilities(
-            self._h, _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan, _dev(planes, torch.complex64, "planes"),
+            self._h, _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan, _dev(planes, self._c, "planes"),
             _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
@@ -287,7 +290,7 @@ class Plan:
         keep, fp = _freq(freq_hz, n_chan)
         self._check(lib().ws_predict_visibilities(
             self._h, _dev(model_image, torch.complex64, "model_image"), _dev(uvw, torch.float32, "uvw"), fp, n_rows, n_chan,
-            _dev(planes, torch.complex64, "planes"), _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
+            _dev(planes, self._c, "planes"), _dev(vis_out, torch.complex64, "vis_out"), float(scale), int(accumulate),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
 
@@ -315,8 +318,8 @@ class Plan:
         keep, fp = _freq(freq_hz, n_chan)
         self._check(lib().ws_image_from_host(
             self._h, uvw_h.data_ptr(), vis_h.data_ptr(), weights_h.data_ptr(), fp, n_rows, n_chan,
-            _dev(dev_inputs, torch.uint8, "dev_inputs"), dev_inputs.numel(), _dev(grid, torch.complex64, "grid"),
-            _dev(image, torch.complex64, "image"), _dev(dirty_d, torch.float32, "dirty_d"), dirty_h.data_ptr(),
+            _dev(dev_inputs, torch.uint8, "dev_inputs"), dev_inputs.numel(), _dev(grid, self._c, "grid"),
+            _dev(image, self._c, "image"), _dev(dirty_d, torch.float32, "dirty_d"), dirty_h.data_ptr(),
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
 
     def measure_fp32_tflops(self, stream=None) -> float:
