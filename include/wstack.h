@@ -140,6 +140,14 @@ int ws_plan_destroy(ws_plan* plan);
  * is unspecified in both cases); a wrong hint only costs speed. */
 int ws_plan_set_snapshot_rows(ws_plan* plan, int64_t rows_per_snapshot);
 
+/* Plane-sharded imaging over several GPUs (one plan per rank; the paper distributes slabs of the mesh over
+ * MPI ranks and reduces the WHOLE mesh, Eq. 8 at :180): after this call the plan keeps only the
+ * visibilities whose w-plane k (computed with the GLOBAL w_min, w_max, n_wplanes of the plan: the keys stay bit-exact)
+ * lies in [plane_lo, plane_hi); all others are dropped like visibilities off the mesh.  Every rank runs the unchanged
+ * chain on all the data and its own plane range -- planes outside it stay empty and cost nothing on the sparse path --
+ * and the N x N images of the ranks are summed (one reduce of 8 N^2 bytes instead of the mesh).  Default: all planes. */
+int ws_plan_set_plane_range(ws_plan* plan, int32_t plane_lo, int32_t plane_hi);
+
 /* ---- sizes: all device memory is allocated by the caller ---------------------------------------------- */
 size_t ws_grid_bytes(const ws_plan* plan);   /* 8 N^2 N_w */
 size_t ws_image_bytes(const ws_plan* plan);  /* 8 N^2     */

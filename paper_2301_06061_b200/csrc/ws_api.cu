@@ -194,6 +194,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     g.n_wplanes = p->n_wplanes;
     g.support = p->support;
     g.halo = (p->support - 1) / 2;
+    g.plane_lo = 0;
+    g.plane_hi = p->n_wplanes;
     g.nt = (int32_t)nt;
     g.n_bins = (uint32_t)(nt * nt * (uint64_t)p->n_wplanes);
     const int taps_rc = make_taps(*p, g);
@@ -305,6 +307,15 @@ int ws_plan_set_snapshot_rows(ws_plan* plan, int64_t rows_per_snapshot) {
     if (rows_per_snapshot < 0 || rows_per_snapshot > MAX_VIS)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_plan_set_snapshot_rows: bad count");
     plan->snapshot_rows = rows_per_snapshot;
+    return WS_OK;
+}
+
+int ws_plan_set_plane_range(ws_plan* plan, int32_t plane_lo, int32_t plane_hi) {
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (plane_lo < 0 || plane_hi > plan->prm.n_wplanes || plane_lo >= plane_hi)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_plan_set_plane_range: need 0 <= plane_lo < plane_hi <= n_wplanes");
+    plan->geom.plane_lo = plane_lo;
+    plan->geom.plane_hi = plane_hi;
     return WS_OK;
 }
 

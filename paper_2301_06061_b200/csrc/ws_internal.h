@@ -27,6 +27,7 @@ struct WsChanConsts {
 // Geometry the binning and gridding kernels need.
 struct WsGeom {
     int32_t n_pix, n_wplanes, support, halo;   // N, N_w, S, h
+    int32_t plane_lo, plane_hi;                 // only visibilities whose plane k lies in [plane_lo, plane_hi) are kept (default: all)
     int32_t nt;                                 // N / T
     uint32_t n_bins;                            // N_w nt^2
     float tap_c;                                // -log2(e) / (2 sigma^2): g(x) = norm1 * 2^(tap_c x^2)

@@ -23,6 +23,7 @@ __device__ __forceinline__ bool place(const WsChanConsts& cc, const WsGeom& g, f
     ck = ck > ktop ? ktop : ck;
     const double lo = (double)g.halo, hi = (double)(g.n_pix - 1 - g.halo);
     if (!(ci >= lo && ci <= hi && cj >= lo && cj <= hi && pw == pw)) return false;   // drop rule O3 (R5); a NaN in u, v or w drops (R33)
+    if (ck < (double)g.plane_lo || ck >= (double)g.plane_hi) return false;           // another rank's planes (ws_plan_set_plane_range)
     o.k = (int)ck;
     o.i0 = (int)ci;
     o.j0 = (int)cj;

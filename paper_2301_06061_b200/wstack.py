@@ -26,7 +26,7 @@ WS_KERNEL_KAISER_BESSEL = 1
 WS_NORM_SUMWT, WS_NORM_N, WS_NORM_TAPER = 1, 2, 4
 
 EXPORTED_SYMBOLS = [
-    "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_grid_bytes",
+    "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_plan_set_plane_range", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
     "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_plan_set_e2e_chunk_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
@@ -68,6 +68,7 @@ def lib():
         "ws_plan_create": (C.c_int, [C.POINTER(_Params), C.POINTER(vp)]),
         "ws_plan_destroy": (C.c_int, [vp]),
         "ws_plan_set_snapshot_rows": (C.c_int, [vp, i64]),
+        "ws_plan_set_plane_range": (C.c_int, [vp, i32, i32]),
         "ws_grid_bytes": (sz, [vp]), "ws_image_bytes": (sz, [vp]), "ws_dirty_bytes": (sz, [vp]),
         "ws_workspace_bytes": (sz, [vp, i64]),
         "ws_workspace_bytes_for": (sz, [vp, i64, C.c_double]),
@@ -163,6 +164,10 @@ class Plan:
     def set_snapshot_rows(self, rows_per_snapshot: int):
         """Performance hint: the input rows are time-major with this many rows (baselines) per snapshot."""
         self._check(lib().ws_plan_set_snapshot_rows(self._h, int(rows_per_snapshot)))
+
+    def set_plane_range(self, plane_lo: int, plane_hi: int):
+        """Keep only the visibilities of w-planes [plane_lo, plane_hi): this rank's share of a plane-sharded image."""
+        self._check(lib().ws_plan_set_plane_range(self._h, int(plane_lo), int(plane_hi)))
 
     # -- sizes ------------------------------------------------------------------------------------------
     @property
