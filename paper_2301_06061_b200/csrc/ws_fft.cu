@@ -327,132 +327,148 @@ __global__ void k_fft_orient(uint32_t* __restrict__ masks, int allow) { masks[2]
 // Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
 // row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
 template <int LOGN>
+__device__ __forceinline__ void colA_item(float2* __restrict__ grid, const float2* __restrict__ tw,
+                                          const uint32_t* __restrict__ class_mask, uint32_t ktx, uint32_t jb) {
+    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32, CW = class_words(R0);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t tx = ktx % NT, k = ktx / NT;
+    const int j = (int)jb * 8 + w;
+    float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
+    if constexpr (LOGN == 14) {
+        // radix 64 = one radix-2 step over the two halves of the column, then radix 32 on the sum and on the
+        // (twiddled) difference: a[r] = Y[2 brev5(r)], b[r] = Y[2 brev5(r) + 1]
+        const uint32_t m_lo = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW] : 0xFFFFFFFFu;
+        const uint32_t m_hi = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW + 1] : 0xFFFFFFFFu;
+        if ((m_lo | m_hi) == 0) return;
+        float2 a[32], b[32];
+#pragma unroll
+        for (int m = 0; m < 32; ++m) {
+            a[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+            b[m] = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int m = 0; m < 32; ++m) {
+            const float2 d = ssub(a[m], b[m]);
+            a[m] = sadd(a[m], b[m]);
+            b[m] = mul_w64(d, m);
+        }
+        bfly<float2, 5, false>(a);
+        bfly<float2, 5, false>(b);
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const int f0 = 2 * brev(r, 5);
+            if (f0) {
+                const float2 tv = __ldg(tw + (f0 - 1) * 256 + j);
+                a[r] = emul(a[r], tv.x, tv.y);
+            }
+            const float2 tu = __ldg(tw + f0 * 256 + j);
+            b[r] = emul(b[r], tu.x, tu.y);
+        }
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const int f0 = 2 * brev(r, 5);
+            p[(size_t)f0 * 256 * N] = a[r];
+            p[(size_t)(f0 + 1) * 256 * N] = b[r];
+        }
+    } else {
+        const uint32_t mask = class_mask ? class_mask[ktx * 8 + (jb >> 2)] : 0xFFFFFFFFu;
+        if (mask == 0) return;
+        float2 x[R0];
+#pragma unroll
+        for (int m = 0; m < R0; ++m)
+            x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+        bfly<float2, LR0, false>(x);
+#pragma unroll
+        for (int r = 1; r < R0; ++r) {
+            const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
+            x[r] = emul(x[r], tv.x, tv.y);
+        }
+#pragma unroll
+        for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
+    }
+}
+
+template <int LOGN>
 __global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
-    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32, CW = class_words(R0);
     const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const uint32_t jb = item & 31, ktx = item >> 5;            // 32 groups of 8 rows per (plane, band)
-        const uint32_t tx = ktx % NT, k = ktx / NT;
-        const int j = (int)jb * 8 + w;
-        float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
-        if constexpr (LOGN == 14) {
-            // radix 64 = one radix-2 step over the two halves of the column, then radix 32 on the sum and on the
-            // (twiddled) difference: a[r] = Y[2 brev5(r)], b[r] = Y[2 brev5(r) + 1]
-            const uint32_t m_lo = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW] : 0xFFFFFFFFu;
-            const uint32_t m_hi = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW + 1] : 0xFFFFFFFFu;
-            if ((m_lo | m_hi) == 0) continue;
-            float2 a[32], b[32];
-#pragma unroll
-            for (int m = 0; m < 32; ++m) {
-                a[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-                b[m] = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
-            }
-#pragma unroll
-            for (int m = 0; m < 32; ++m) {
-                const float2 d = ssub(a[m], b[m]);
-                a[m] = sadd(a[m], b[m]);
-                b[m] = mul_w64(d, m);
-            }
-            bfly<float2, 5, false>(a);
-            bfly<float2, 5, false>(b);
-#pragma unroll
-            for (int r = 0; r < 32; ++r) {
-                const int f0 = 2 * brev(r, 5);
-                if (f0) {
-                    const float2 tv = __ldg(tw + (f0 - 1) * 256 + j);
-                    a[r] = emul(a[r], tv.x, tv.y);
-                }
-                const float2 tu = __ldg(tw + f0 * 256 + j);
-                b[r] = emul(b[r], tu.x, tu.y);
-            }
-#pragma unroll
-            for (int r = 0; r < 32; ++r) {
-                const int f0 = 2 * brev(r, 5);
-                p[(size_t)f0 * 256 * N] = a[r];
-                p[(size_t)(f0 + 1) * 256 * N] = b[r];
-            }
-        } else {
-            const uint32_t mask = class_mask ? class_mask[ktx * 8 + (jb >> 2)] : 0xFFFFFFFFu;
-            if (mask == 0) continue;
-            float2 x[R0];
-#pragma unroll
-            for (int m = 0; m < R0; ++m)
-                x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-            bfly<float2, LR0, false>(x);
-#pragma unroll
-            for (int r = 1; r < R0; ++r) {
-                const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
-                x[r] = emul(x[r], tv.x, tv.y);
-            }
-#pragma unroll
-            for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
-        }
-    }
+    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x)
+        colA_item<LOGN>(grid, tw, class_mask, item >> 5, item & 31);      // 32 groups of 8 rows per (plane, band)
 }
 
 // ---- pass 1b: the 256-point column transforms -------------------------------------------------------------------
 // Item = (plane, column band tx, block m0 of 256 rows).  Warp w, lane = column.  Stage 1: j in {w, w + 8}, rows
 // j + 16 m; stage 2: blocks b in {w, w + 8}, rows 16 b + m; frequency f = b + 16 m' is stored at row 256 m0 + f.
+// bit c of the result: class c of the band holds data (0: nothing to do)
+template <int LOGN>
+__device__ __forceinline__ uint32_t band_classes(const uint32_t* __restrict__ class_mask, uint32_t ktx) {
+    constexpr int CW = class_words(1 << (LOGN - 8));
+    if (!class_mask) return 0xFFu;
+    uint32_t cmask = 0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        uint32_t any = class_mask[(ktx * 8 + c) * CW];
+        if (CW > 1) any |= class_mask[(ktx * 8 + c) * CW + 1];
+        cmask |= (any != 0 ? 1u : 0u) << c;
+    }
+    return cmask;
+}
+template <int LOGN>
+__device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float2* __restrict__ tw, float2* __restrict__ blk,
+                                          uint32_t cmask, uint32_t ktx, uint32_t m0) {
+    constexpr int N = 1 << LOGN, NT = N / 32;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t tx = ktx % NT, k = ktx / NT;
+    float2* p = grid + ((size_t)k * N + m0 * 256) * N + tx * 32 + lane;
+    float2 x[32];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int j = w + 8 * i;
+#pragma unroll
+        for (int m = 0; m < 16; ++m)
+            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? __ldcs(p + (size_t)(j + 16 * m) * N) : make_float2(0.f, 0.f);
+    }
+    __syncthreads();          // the previous item's second stage has read `blk`
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int j = w + 8 * i;
+        bfly<float2, 4, false>(x + i * 16);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            float2 v = x[i * 16 + r];
+            if (r) {
+                const float2 tv = __ldg(tw + (brev(r, 4) - 1) * 16 + j);
+                v = emul(v, tv.x, tv.y);
+            }
+            blk[(j + 16 * brev(r, 4)) * 32 + lane] = v;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int b = w + 8 * i;
+#pragma unroll
+        for (int m = 0; m < 16; ++m) x[i * 16 + m] = blk[(16 * b + m) * 32 + lane];
+        bfly<float2, 4, false>(x + i * 16);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) __stcs(p + (size_t)(b + 16 * brev(r, 4)) * N, x[i * 16 + r]);   // read next by pass 2, long after
+    }
+}
+
 template <int LOGN>
 __global__ void __launch_bounds__(CT, 2)
 k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
-    constexpr int N = 1 << LOGN, R0 = 1 << (LOGN - 8), NT = N / 32, CW = class_words(R0);
+    constexpr int R0 = 1 << (LOGN - 8);
     const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
         const uint32_t m0 = item % R0, ktx = item / R0;
-        const uint32_t tx = ktx % NT, k = ktx / NT;
-        uint32_t cmask = 0xFFu;
-        if (class_mask) {
-            cmask = 0;
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                uint32_t any = class_mask[(ktx * 8 + c) * CW];
-                if (CW > 1) any |= class_mask[(ktx * 8 + c) * CW + 1];
-                cmask |= (any != 0 ? 1u : 0u) << c;
-            }
-        }
+        const uint32_t cmask = band_classes<LOGN>(class_mask, ktx);
         if (cmask == 0) continue;
-        float2* p = grid + ((size_t)k * N + m0 * 256) * N + tx * 32 + lane;
-        float2 x[32];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int j = w + 8 * i;
-#pragma unroll
-            for (int m = 0; m < 16; ++m)
-                x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? __ldcs(p + (size_t)(j + 16 * m) * N) : make_float2(0.f, 0.f);
-        }
-        __syncthreads();          // the previous item's second stage has read `blk`
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int j = w + 8 * i;
-            bfly<float2, 4, false>(x + i * 16);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                float2 v = x[i * 16 + r];
-                if (r) {
-                    const float2 tv = __ldg(tw + (brev(r, 4) - 1) * 16 + j);
-                    v = emul(v, tv.x, tv.y);
-                }
-                blk[(j + 16 * brev(r, 4)) * 32 + lane] = v;
-            }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int b = w + 8 * i;
-#pragma unroll
-            for (int m = 0; m < 16; ++m) x[i * 16 + m] = blk[(16 * b + m) * 32 + lane];
-            bfly<float2, 4, false>(x + i * 16);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) p[(size_t)(b + 16 * brev(r, 4)) * N] = x[i * 16 + r];
-        }
+        colB_item<LOGN>(grid, tw, blk, cmask, ktx, m0);
     }
 }
 

@@ -239,7 +239,7 @@ def test_small_workspace_reports_overflow(oracle):
 def test_argument_validation():
     import paper_2301_06061_b200 as ws
     for bad in (dict(n_pix=250), dict(support=8), dict(support=17), dict(w_max=-5.0), dict(cell_rad=0.0), dict(tile=64),
-                dict(flags=16)):
+                dict(flags=32)):
         kw = dict(n_pix=256, n_wplanes=4, support=7, cell_rad=1e-3, w_min=-1.0, w_max=1.0)
         kw.update(bad)
         with pytest.raises(ws.WStackError):
