@@ -69,9 +69,13 @@ __host__ __device__ constexpr int tw_offset(int logn, int s) {
 }
 __host__ __device__ constexpr int tw_entries(int logn) { return tw_offset(logn, n_stages(logn) - 1); }   // last stage: Q = 1, none
 // what of it the row kernel keeps in shared memory: everything, except for N = 16384, whose first-stage twiddles are
-// thread constants held in registers (the 128 KB landing buffer leaves no room for a table): only stage 1 then
-__host__ __device__ constexpr int tw_smem_entries(int logn) { return logn == 14 ? tw_entries(logn) - tw_offset(logn, 1) : tw_entries(logn); }
-__host__ __device__ constexpr int tw_smem_off1(int logn) { return logn == 14 ? 0 : tw_offset(logn, 1); }
+// thread constants held in registers (7 exact values, the 16 twiddles of a thread are products of two of them) because
+// the 128 KB landing buffer leaves no room for a table: only stage 1 then.  (Measured at N = 8192: register twiddles +
+// a second landing buffer in the freed shared memory, 12.06 ms against 11.72 with the table -- the two dependent
+// complex multiplies per output cost more issue slots and latency than the table's loads; not used there.)
+__host__ __device__ constexpr bool tw_in_regs(int logn) { return logn >= 14; }
+__host__ __device__ constexpr int tw_smem_entries(int logn) { return tw_in_regs(logn) ? tw_entries(logn) - tw_offset(logn, 1) : tw_entries(logn); }
+__host__ __device__ constexpr int tw_smem_off1(int logn) { return tw_in_regs(logn) ? 0 : tw_offset(logn, 1); }
 
 __host__ __device__ constexpr int brev(int i, int bits) {
     int r = 0;
@@ -534,6 +538,7 @@ struct RowCfg {
     static constexpr bool SPLIT64 = LOGN == 14;       // first stage: radix 64 split over the groups of TWO CTAs (by output parity)
     static constexpr int ITEMS_PER_ROW = SPLIT64 ? 2 : 1;
     static constexpr int BW = band_words(NT);
+    static constexpr int NBUF = 1;                    // landing buffers (2 works where the shared memory allows it; see tw_in_regs)
     static constexpr int LRL = log2r(LOGN, S - 1);    // last stage
 };
 
@@ -681,12 +686,13 @@ struct Grouped {
             for (int m = 0; m < 16; ++m) x[m] = in[256 * m];
         }
     }
-    // tc (N = 16384 only): the thread's first-stage twiddles as 7 register constants, tc[b] = W_N^(ug (4 b + q)), b < 4,
-    // tc[3 + a] = W_N^(16 a ug), a = 1..3: output d = 16 a + 4 b + q is multiplied by tc[b] tc[3 + a].
+    // tc (N >= 8192): the thread's first-stage twiddles as 7 register constants.  Its outputs are the digits d = M p + q,
+    // p = 4 a + b < 16 (N = 8192: M = 2, q = g; N = 16384: M = 4, q = 2 g + parity): tc[b] = W_N^(ug (M b + q)), b < 4,
+    // tc[3 + a] = W_N^(4 M a ug), a = 1..3, and output d is multiplied by tc[b] tc[3 + a] (two roundings instead of one).
     __device__ static __forceinline__ void finish_first(float2* x, float2* __restrict__ work, const float2* __restrict__ tw,
                                                         int ug, int g, const float2* tc) {
         bfly<float2, 4>(x);
-        if constexpr (SPLIT64) {
+        if constexpr (SPLIT && tw_in_regs(LOGN)) {
             float2* out = work + g * 272 + ug + (ug >> 4);
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
@@ -768,24 +774,24 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
            float* __restrict__ dirty, int accumulate, const float2* __restrict__ tw_g, const float2* __restrict__ tc_g,
            const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t item_lo, uint32_t n_super) {
     using C = RowCfg<LOGN>;
-    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0, LAND = C::LAND, BW = C::BW;
+    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0, LAND = C::LAND, BW = C::BW, NBUF = C::NBUF;
     // occupancy: the band masks of the orientation the mesh is stored in; transposed: the mesh is [k][u][v], i.e. a
     // row position is a u-frequency and the image comes out transposed (the phase screen is symmetric in l and m)
     const uint32_t* band_mask = masks ? mask_set(masks, set_words) + (set_words - (uint32_t)BW * (uint32_t)prm.n_wplanes) : nullptr;
     const bool transposed = masks && masks[2];
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2* landing = (float2*)smem_raw;
-    float2* work = landing + LAND;
+    float2* landing0 = (float2*)smem_raw;                               // NBUF buffers of LAND points
+    float2* work = landing0 + NBUF * LAND;
     float2* tw = work + PAD_PTS;
-    uint64_t* full = (uint64_t*)(tw + ((tw_smem_entries(LOGN) + 1) & ~1));   // the copy of a plane has landed
-    uint64_t* empty = full + 1;                                         // every group has consumed it
-    uint32_t* s_any = (uint32_t*)(empty + 1);                           // bit k: plane k has a non-empty band
+    uint64_t* full = (uint64_t*)(tw + ((tw_smem_entries(LOGN) + 1) & ~1));   // [NBUF] the copy of a plane has landed
+    uint64_t* empty = full + NBUF;                                      // [NBUF] every group has consumed it
+    uint32_t* s_any = (uint32_t*)(empty + NBUF);                        // bit k: plane k has a non-empty band
     const int u = threadIdx.x, g = u >> 8;
     const int par = C::SPLIT64 ? (int)(blockIdx.x & 1u) : 0;           // (the grid is even: every item of a CTA has its parity)
     const int nw = prm.n_wplanes;
     const size_t plane_elems = (size_t)N * N;
     for (int i = u; i < tw_smem_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
-    for (int i = u; i < LAND; i += FT + PT) landing[i] = make_float2(0.f, 0.f);
+    for (int i = u; i < NBUF * LAND; i += FT + PT) landing0[i] = make_float2(0.f, 0.f);
     for (int k0 = 0; k0 < nw; k0 += FT + PT) {       // (FT + PT is a multiple of 32: one ballot per mask word)
         const int k = k0 + u;
         bool any = false;
@@ -795,8 +801,10 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (u == 0) {
-        mbar_init(full, 1);
-        mbar_init(empty, C::GROUPED ? 2 : 1);
+        for (int i = 0; i < NBUF; ++i) {
+            mbar_init(full + i, 1);
+            mbar_init(empty + i, C::GROUPED ? 2 : 1);
+        }
     }
     __syncthreads();
     if (item_lo + blockIdx.x >= n_super) return;       // items [item_lo, n_super) belong to this launch
@@ -808,8 +816,9 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         // brings the non-empty bands of the next plane in.  Lane wi < BW owns mask word wi (32 bands = 8 KB per row)
         // and issues one bulk copy per maximal run of set bits.
         const int lane = u & 31;
-        uint32_t was = 0, e_parity = 0;
-        bool first = true;
+        uint32_t was[NBUF], seq = 0;                      // seq: planes copied so far; plane seq lands in buffer seq % NBUF
+#pragma unroll
+        for (int i = 0; i < NBUF; ++i) was[i] = 0;
         for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
             const uint32_t sr = super_row_of<LOGN>(it);
             for (int k = nw - 1; k >= 0; --k) {
@@ -824,13 +833,13 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                 uint32_t n_bands = __popc(now);
 #pragma unroll
                 for (int d = 16; d >= 1; d >>= 1) n_bands += __shfl_xor_sync(0xffffffffu, n_bands, d);
-                const uint32_t stale = was & ~now;
+                const uint32_t buf = seq % NBUF, use = seq / NBUF;       // this buffer's use-th filling
+                float2* landing = landing0 + buf * LAND;
+                const uint32_t stale = (NBUF == 2 && buf ? was[NBUF - 1] : was[0]) & ~now;
                 const bool any_stale = __any_sync(0xffffffffu, stale != 0);
-                if (!first) {
-                    while (!mbar_try_wait(empty, e_parity)) {}
-                    e_parity ^= 1u;
+                if (use > 0) {
+                    while (!mbar_try_wait(empty + buf, (use - 1) & 1u)) {}
                 }
-                first = false;
                 // stale bands are cleared BEFORE the arrive: its release then orders the zeroing stores ahead of the
                 // consumers' reads (they acquire `full`), whatever the bulk copies' timing
                 if (any_stale) {
@@ -846,7 +855,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 }
                 __syncwarp();
-                if (lane == 0) mbar_expect_tx(full, n_bands * 256u * ROWS);     // (the previous phase is complete now)
+                if (lane == 0) mbar_expect_tx(full + buf, n_bands * 256u * ROWS);     // (the previous phase is complete now)
                 __syncwarp();
                 const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * LAND);
                 uint32_t m = now;
@@ -857,27 +866,31 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                     m &= ~((len == 32 ? 0xFFFFFFFFu : (1u << len) - 1u) << b0);
                     const size_t off = (size_t)(lane * 32 + b0) * 256;
                     for (int r = 0; r < ROWS; ++r)
-                        bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, full);
+                        bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, full + buf);
                 }
-                was = now;
+                if (NBUF == 2 && buf) was[NBUF - 1] = now;
+                else was[0] = now;
+                ++seq;
             }
         }
         return;
     }
 
-    // ---- the 16 compute warps (they take over the registers the producer's warpgroup gave back)
+    // ---- the 16 compute warps (they take over the registers the producer's warpgroup gave back: the pool is the CTA's
+    // launch allocation, 640 x 96 registers, so 112 is the most that 512 threads can take; asking for more blocks forever)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
     auto cta_sync = [&]() { asm volatile("bar.sync 3, %0;" ::"r"(FT) : "memory"); };     // (the producer is not part of it)
     auto group_sync = [&]() {
         if (C::GROUPED) asm volatile("bar.sync %0, %1;" ::"r"(1 + g), "r"(GT) : "memory");
         else cta_sync();
     };
-    uint32_t parity = 0;
+    uint32_t seq = 0;                      // planes consumed so far (the producer's count, same order)
     const int top_span_lo = ((nw - 1) / WC_SPAN) * WC_SPAN;
-    float2 tc[7];      // N = 16384: first-stage twiddles of this thread (Grouped::finish_first), constant for the whole kernel
-    if constexpr (C::SPLIT64) {
+    float2 tc[7];      // N >= 8192: first-stage twiddles of this thread (Grouped::finish_first), constant for the whole kernel
+    if constexpr (tw_in_regs(LOGN)) {
+        const int q = C::SPLIT64 ? 2 * g + par : g;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) tc[i] = __ldg(tc_g + ((2 * g + par) * 4 + i) * 256 + (u & 255));
+        for (int i = 0; i < 4; ++i) tc[i] = __ldg(tc_g + (q * 4 + i) * 256 + (u & 255));
 #pragma unroll
         for (int i = 0; i < 3; ++i) tc[4 + i] = __ldg(tc_g + (16 + i) * 256 + (u & 255));
     }
@@ -898,14 +911,16 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
         for (int k = nw - 1; k >= 0; --k) {
             float2 x[EPT];
             if ((s_any[k >> 5] >> (k & 31)) & 1u) {      // CTA-uniform: the plane has data, its copy is under way
-                while (!mbar_try_wait(full, parity)) {}
-                parity ^= 1u;
+                const uint32_t buf = seq % NBUF, use = seq / NBUF;
+                const float2* landing = landing0 + buf * LAND;
+                while (!mbar_try_wait(full + buf, use & 1u)) {}
+                ++seq;
                 // ---- first stage: inputs from the landing buffer
                 if constexpr (C::GROUPED) Grouped<LOGN>::load_first(x, landing, u & 255, g, par);
                 else row_stage<LOGN, 0, true, false>(x, landing, work, tw, u);
                 group_sync();          // this group is done with `landing` (and with last plane's reads of `work`)
                 if ((u & 255) == 0 && (C::GROUPED || g == 0))
-                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty)) : "memory");
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + buf)) : "memory");
                 // ---- arithmetic, twiddles, exchanges
                 if constexpr (C::GROUPED) {
                     Grouped<LOGN>::finish_first(x, work, tw, u & 255, g, tc);
@@ -1007,8 +1022,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
 // ---- host side ---------------------------------------------------------------------------------------------
 template <int LOGN>
 size_t rows_smem() {
-    return (size_t)RowCfg<LOGN>::LAND * sizeof(float2) + (size_t)PAD_PTS * sizeof(float2) +
-           (size_t)((tw_smem_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16 + MAX_PLANES / 8;
+    return (size_t)RowCfg<LOGN>::NBUF * RowCfg<LOGN>::LAND * sizeof(float2) + (size_t)PAD_PTS * sizeof(float2) +
+           (size_t)((tw_smem_entries(LOGN) + 1) & ~1) * sizeof(float2) + 16 * RowCfg<LOGN>::NBUF + MAX_PLANES / 8;
 }
 
 float2 unit(long long e, long long L) {      // exp(+2 pi i e / L), fp64 -> fp32
@@ -1017,13 +1032,13 @@ float2 unit(long long e, long long L) {      // exp(+2 pi i e / L), fp64 -> fp32
 }
 
 // Table = [pass 2: every stage but the last, (R-1) Q entries W_L^(j m') each (N = 16384: stage 1 only) | pass 1a:
-// (R0-1) x 256 entries W_N^(j m') | pass 1b: 15 x 16 entries W_256^(j m') | N = 16384: the first-stage register constants
-// of the row kernel, [q][b][ug] = W_N^(ug (4 b + q)) (4 x 4 x 256) then [a][ug] = W_N^(16 a ug), a = 1..3]
+// (R0-1) x 256 entries W_N^(j m') | pass 1b: 15 x 16 entries W_256^(j m') | N >= 8192: the first-stage register constants
+// of the row kernel, [q][b][ug] = W_N^(ug (M b + q)) (4 x 4 x 256) then [a][ug] = W_N^(4 M a ug), a = 1..3]
 template <int LOGN>
 int init_n(ws_plan* plan) {
     constexpr int N = 1 << LOGN, R0 = N / 256;
     std::vector<float2> tw;
-    for (int s = LOGN == 14 ? 1 : 0; s + 1 < n_stages(LOGN); ++s) {
+    for (int s = tw_in_regs(LOGN) ? 1 : 0; s + 1 < n_stages(LOGN); ++s) {
         const int L = 1 << log2l(LOGN, s), R = 1 << log2r(LOGN, s), Q = L / R;
         for (int m = 1; m < R; ++m)
             for (int j = 0; j < Q; ++j) tw.push_back(unit((long long)j * m, L));
@@ -1035,12 +1050,13 @@ int init_n(ws_plan* plan) {
     for (int m = 1; m < 16; ++m)
         for (int j = 0; j < 16; ++j) tw.push_back(unit((long long)j * m, 256));
     plan->tw_off_c = tw.size();
-    if (LOGN == 14) {
+    if (tw_in_regs(LOGN)) {
+        const int M = LOGN == 14 ? 4 : 2;          // first-stage digits of one thread: d = M p + q, q < M
         for (int q = 0; q < 4; ++q)
             for (int b = 0; b < 4; ++b)
-                for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * (4 * b + q), N));
+                for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * (M * b + (q % M)), N));
         for (int a = 1; a < 4; ++a)
-            for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * 16 * a, N));
+            for (int ug = 0; ug < 256; ++ug) tw.push_back(unit((long long)ug * 4 * M * a, N));
     }
     const size_t n_class = (size_t)plan->prm.n_wplanes * (N / 32) * 8 * class_words(R0),
                  n_band = (size_t)plan->prm.n_wplanes * band_words(N / 32);
