@@ -24,17 +24,30 @@ namespace {
 
 constexpr int T = WS_TILE;
 
+constexpr int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+// The warp's shared tile covers the 32 x 32 cells it owns PLUS a ring of H cells: the footprint of a record whose
+// centre lies inside the tile (a "home" record) then never leaves the buffer, and the inner loop over the home records
+// of a bin -- 71 % of all records on Large -- needs no bounds test at all.  The ring collects only part of what belongs
+// there (the neighbour tiles hold their own copies of the records that reach them) and is never stored.
 template <int S>
 struct TileCfg {
     static constexpr int H = (S - 1) / 2;
     static constexpr int P = T + S;                 // row pitch in complex cells: P = S mod 16 -> conflict-free taps
-    static constexpr int R = 32 / S;                // footprint rows a warp covers per round
+    static constexpr int ROWS = T + S - 1;          // rows (and used columns) of the buffer: tile + ring
+    static constexpr int R = 32 / S < S ? 32 / S : S;   // footprint rows a warp covers per round
     static constexpr int NR = (S + R - 1) / R;      // rounds per visibility
-    static constexpr int TILE_CELLS = T * P;
-    // per warp: tile | meta[32] float4 | gu[32][S] | gv[32][S]
+    static constexpr int NRP = pow2_ceil(NR);       // taps of one lane along v, padded: one vector load
+    static constexpr int SP = S;                    // pitch of the u taps of a record (odd: lane r's scalar stores are conflict-free)
+    static constexpr int GP = NRP * (R | 1);        // pitch of its v taps, [R][NRP] + padding: an odd number of NRP-vectors, so
+                                                    // that the lanes' vector stores of one br fall into distinct banks
+    static constexpr int TILE_CELLS = ROWS * P;
+    static constexpr int GU_FLOATS = (32 * SP + 3) / 4 * 4;    // (keeps gv 16-byte aligned)
+    // per warp: tile | meta[32] float4 | gu[32][SP] | gv[32][GP]
     static constexpr size_t WARP_BYTES =
-        ((size_t)TILE_CELLS * sizeof(float2) + 32 * sizeof(float4) + 2 * 32 * S * sizeof(float) + 15) / 16 * 16;
-    static constexpr int WARPS = (113 * 1024) / WARP_BYTES >= 8 ? 8 : (int)((113 * 1024) / WARP_BYTES);
+        ((size_t)TILE_CELLS * sizeof(float2) + 32 * sizeof(float4) + (GU_FLOATS + 32 * GP) * sizeof(float) + 15) / 16 * 16;
+    // one CTA per SM with as many (independent) warps as the 227 KB of shared memory hold, at most 16
+    static constexpr int WARPS = (227 * 1024) / WARP_BYTES >= 16 ? 16 : (int)((227 * 1024) / WARP_BYTES);
     static constexpr int THREADS = WARPS * 32;
 };
 
@@ -71,76 +84,146 @@ struct WarpSmem {
         tile = (float2*)base;
         meta = (float4*)(tile + C::TILE_CELLS);
         gu = (float*)(meta + 32);
-        gv = gu + 32 * S;
+        gv = gu + C::GU_FLOATS;
     }
 };
 
-// Accumulates records [lo, hi) into the warp's shared tile.
+template <int N>
+struct TapVec { float v[N]; };
+template <int N>
+__device__ __forceinline__ void store_taps(float* p, const TapVec<N>& t) {
+    if constexpr (N == 1) p[0] = t.v[0];
+    else if constexpr (N == 2) *(float2*)p = make_float2(t.v[0], t.v[1]);
+    else {
+#pragma unroll
+        for (int i = 0; i < N; i += 4) *(float4*)(p + i) = make_float4(t.v[i], t.v[i + 1], t.v[i + 2], t.v[i + 3]);
+    }
+}
+template <int N>
+__device__ __forceinline__ TapVec<N> load_taps(const float* p) {
+    TapVec<N> t;
+    if constexpr (N == 1) t.v[0] = p[0];
+    else if constexpr (N == 2) { const float2 q = *(const float2*)p; t.v[0] = q.x; t.v[1] = q.y; }
+    else {
+#pragma unroll
+        for (int i = 0; i < N; i += 4) {
+            const float4 q = *(const float4*)(p + i);
+            t.v[i] = q.x; t.v[i + 1] = q.y; t.v[i + 2] = q.z; t.v[i + 3] = q.w;
+        }
+    }
+    return t;
+}
+
+// vector phase of a batch: the 2 S taps of lane r's record, parked where the lanes (a, br) find them.  The Kaiser-Bessel
+// series is kept out of line: inlined, its register demand makes the compiler turn the predicated read-modify-writes of the
+// record loop into divergent branches (measured: 15.3 ms against 10.9 on Large).
+template <int S>
+__device__ __forceinline__ void park_store(const float* gu, const float* gv, const WarpSmem<S>& sm, int lane) {
+    using C = TileCfg<S>;
+#pragma unroll
+    for (int i = 0; i < S; ++i) sm.gu[lane * C::SP + i] = gu[i];
+#pragma unroll
+    for (int b0 = 0; b0 < C::R; ++b0) {                 // the taps lane (., b0) applies in its rounds, as one vector
+        TapVec<C::NRP> tv;
+#pragma unroll
+        for (int rr = 0; rr < C::NRP; ++rr) tv.v[rr] = b0 + rr * C::R < S ? gv[b0 + rr * C::R < S ? b0 + rr * C::R : 0] : 0.f;
+        store_taps<C::NRP>(sm.gv + lane * C::GP + b0 * C::NRP, tv);
+    }
+}
+template <int S>
+__device__ __noinline__ void park_taps_kb(const WsGeom& g, float fx, float fy, float* gu_s, float* gv_s, int lane) {
+    float gu[S], gv[S];
+    eval_taps<S, true>(g, fx, fy, gu, gv);
+    WarpSmem<S> sm(nullptr);
+    sm.gu = gu_s;
+    sm.gv = gv_s;
+    park_store<S>(gu, gv, sm, lane);
+}
 template <int S, bool KB>
-__device__ __forceinline__ void accumulate(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
-                                           const WarpSmem<S>& sm, int lane) {
+__device__ __forceinline__ void park_taps(const WsGeom& g, float fx, float fy, const WarpSmem<S>& sm, int lane) {
+    if constexpr (KB) {
+        park_taps_kb<S>(g, fx, fy, sm.gu, sm.gv, lane);
+    } else {
+        using C = TileCfg<S>;
+        float gu[S], gv[S];
+        const float tap_c = g.tap_c;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const float dx = (float)(i - C::H) - fx, dy = (float)(i - C::H) - fy;
+            gu[i] = ex2_approx(tap_c * dx * dx);
+            gv[i] = ex2_approx(tap_c * dy * dy);
+        }
+        park_store<S>(gu, gv, sm, lane);
+    }
+}
+
+// One record of the batch onto the tile: lane (a, br) applies its taps.  HOME: the record's centre cell lies inside the
+// tile, so its footprint stays inside the buffer (tile + ring): no bounds tests.  Otherwise (the copy of a neighbour's
+// record, centre in the ring) each tap is tested against the buffer.
+template <int S, bool HOME>
+__device__ __forceinline__ void apply_record(const WarpSmem<S>& sm, int r, int a, int br, const bool* okb, unsigned char* tile_b,
+                                             const float* gu_l, const float* gv_l) {
+    using C = TileCfg<S>;
+    const float4 m = sm.meta[r];                       // broadcast
+    const float u = gu_l[r * C::SP];
+    const TapVec<C::NRP> gvv = load_taps<C::NRP>(gv_l + r * C::GP);
+    float2* const cell0 = (float2*)(tile_b + __float_as_int(m.w));
+    bool ok[C::NR];
+    if constexpr (HOME) {
+#pragma unroll
+        for (int rr = 0; rr < C::NR; ++rr) ok[rr] = okb[rr];
+    } else {
+        const int xy = __float_as_int(m.z);
+        const int cx = (int)(short)(xy & 0xFFFF), cy = xy >> 16;
+        const bool okx = (unsigned)(cx + a) < (unsigned)C::ROWS;
+#pragma unroll
+        for (int rr = 0; rr < C::NR; ++rr) ok[rr] = okb[rr] && okx && (unsigned)(cy + br + rr * C::R) < (unsigned)C::ROWS;
+    }
+#pragma unroll
+    for (int rr = 0; rr < C::NR; ++rr) {
+        if (ok[rr]) {                                   // (distinct cells per round: the loads of all rounds can go first)
+            float2 c = cell0[rr * C::R * C::P];
+            const float t = u * gvv.v[rr];
+            c.x = fmaf(m.x, t, c.x);
+            c.y = fmaf(m.y, t, c.y);
+            cell0[rr * C::R * C::P] = c;
+        }
+    }
+    __syncwarp();
+}
+
+// Accumulates records [lo, hi) of a bin into the warp's shared tile; those before `home_end` are the bin's home records
+// (they come first in its list).
+template <int S, bool KB>
+__device__ __forceinline__ void accumulate_bin(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
+                                               uint32_t home_end, const WarpSmem<S>& sm, int lane) {
     using C = TileCfg<S>;
     const int a = lane % S, br = lane / S;
     const bool active = br < C::R;
-    const int lane_idx = br * C::P + a;            // tap (a, br) relative to the footprint's first cell
+    bool okb[C::NR];                               // lane constants: this lane has a tap in round rr
+#pragma unroll
+    for (int rr = 0; rr < C::NR; ++rr) okb[rr] = active && br + rr * C::R < S;
+    unsigned char* const tile_b = (unsigned char*)sm.tile + (size_t)((active ? br : 0) * C::P + a) * sizeof(float2);
+    const float* const gu_l = sm.gu + a;
+    const float* const gv_l = sm.gv + (active ? br : 0) * C::NRP;
     float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lo + lane < hi) nxt = __ldcs(records + lo + lane);
     for (uint32_t base = lo; base < hi; base += 32) {
         const int n = (int)min(32u, hi - base);
+        const int n_home = home_end > base ? (int)min((uint32_t)n, home_end - base) : 0;
         {   // vector phase: lane r prepares record r of the batch
             const uint32_t X = __float_as_uint(nxt.x), Y = __float_as_uint(nxt.y);
-            const int cxp = ((int)X >> 24) - C::H, cyp = ((int)Y >> 24) - C::H;   // footprint's first cell, tile frame
+            const int cx = (int)X >> 24, cy = (int)Y >> 24;    // centre cell in the tile's frame = first footprint cell in the buffer's
             const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
             const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
-            if constexpr (!KB) {
-                const float tap_c = g.tap_c;
-#pragma unroll
-                for (int i = 0; i < S; ++i) {
-                    const float dx = (float)(i - C::H) - fx, dy = (float)(i - C::H) - fy;
-                    sm.gu[lane * S + i] = ex2_approx(tap_c * dx * dx);
-                    sm.gv[lane * S + i] = ex2_approx(tap_c * dy * dy);
-                }
-            } else {
-                float gu[S], gv[S];
-                eval_taps<S, true>(g, fx, fy, gu, gv);
-#pragma unroll
-                for (int i = 0; i < S; ++i) {
-                    sm.gu[lane * S + i] = gu[i];
-                    sm.gv[lane * S + i] = gv[i];
-                }
-            }
-            sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cxp & 0xFFFF) | (cyp << 16)),
-                                        __int_as_float(cyp * C::P + cxp));
+            park_taps<S, KB>(g, fx, fy, sm, lane);
+            sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cx & 0xFFFF) | (cy << 16)),
+                                        __int_as_float((cy * C::P + cx) * (int)sizeof(float2)));
         }
         if (base + 32 + lane < hi) nxt = __ldcs(records + base + 32 + lane);   // prefetch the next batch
         __syncwarp();
-        for (int r = 0; r < n; ++r) {
-            const float4 m = sm.meta[r];                       // broadcast
-            const float u = sm.gu[r * S + a];
-            const int xy = __float_as_int(m.z);
-            const int cxp = (int)(short)(xy & 0xFFFF), cyp = xy >> 16;
-            const bool okx = active && (unsigned)(cxp + a) < (unsigned)T;
-            const int idx0 = __float_as_int(m.w) + lane_idx;
-            float2 cell[C::NR];
-            float t[C::NR];
-            bool ok[C::NR];
-#pragma unroll
-            for (int rr = 0; rr < C::NR; ++rr) {
-                const int b = br + rr * C::R;
-                ok[rr] = okx && b < S && (unsigned)(cyp + b) < (unsigned)T;
-                t[rr] = u * sm.gv[r * S + (b < S ? b : 0)];
-                if (ok[rr]) cell[rr] = sm.tile[idx0 + rr * C::R * C::P];
-            }
-#pragma unroll
-            for (int rr = 0; rr < C::NR; ++rr) {
-                if (ok[rr]) {
-                    cell[rr].x = fmaf(m.x, t[rr], cell[rr].x);
-                    cell[rr].y = fmaf(m.y, t[rr], cell[rr].y);
-                    sm.tile[idx0 + rr * C::R * C::P] = cell[rr];
-                }
-            }
-            __syncwarp();
-        }
+        for (int r = 0; r < n_home; ++r) apply_record<S, true>(sm, r, a, br, okb, tile_b, gu_l, gv_l);
+        for (int r = n_home; r < n; ++r) apply_record<S, false>(sm, r, a, br, okb, tile_b, gu_l, gv_l);
     }
 }
 
@@ -199,16 +282,18 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
     }
 }
 
-// Persistent kernel: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
+// Persistent kernel, one CTA per SM: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
 template <int S, bool KB>
-__global__ void __launch_bounds__(TileCfg<S>::THREADS, 2)
-k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint4* __restrict__ items,
+__global__ void __launch_bounds__(TileCfg<S>::THREADS, 1)
+k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint32_t* __restrict__ bin_start,
+       const uint4* __restrict__ items,
        const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
        const uint32_t* __restrict__ orient, const WsMaskView mv) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const WarpSmem<S> sm(smem_raw + (size_t)wid * C::WARP_BYTES);
+    const float2* const inner = sm.tile + C::H * C::P + C::H;     // cell (0, 0) of the tile proper, inside the ring
     if (status->overflow) return;
     const bool tr = orient && *orient;          // transposed planes: lane = row of the tile, one tile column per store
     const uint32_t n_items = status->n_items;
@@ -225,10 +310,10 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         it += n_warps;
         float2* out = tile_origin(g, grid, w.x, tr);
         zero_tile<S>(sm.tile, lane);
-        accumulate<S, KB>(g, records, w.y, w.z, sm, lane);
+        accumulate_bin<S, KB>(g, records, w.y, w.z, rec_start[w.x] + (bin_start[w.x + 1] - bin_start[w.x]), sm, lane);
 #pragma unroll 4
         for (int y = 0; y < T; ++y) {
-            const float2 v = tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane];
+            const float2 v = tr ? inner[lane * C::P + y] : inner[y * C::P + lane];
             if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
         }
         __syncwarp();
@@ -248,7 +333,7 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
             continue;
         }
         zero_tile<S>(sm.tile, lane);
-        accumulate<S, KB>(g, records, s, e, sm, lane);
+        accumulate_bin<S, KB>(g, records, s, e, s + (bin_start[bin + 1] - bin_start[bin]), sm, lane);
         bool add = mode == WS_GRID_ACCUMULATE;
         if (mode == WS_GRID_SPARSE_ADD) {                       // warp-uniform: did an earlier chunk fill this tile?
             const uint32_t nt = (uint32_t)g.nt, tx = bin % nt, r = bin / nt;
@@ -256,11 +341,11 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         }
         if (!add) {
 #pragma unroll 4
-            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane]);
+            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? inner[lane * C::P + y] : inner[y * C::P + lane]);
         } else {        // no other warp writes this tile in this launch except through red: fire-and-forget vector adds
 #pragma unroll 4
             for (int y = 0; y < T; ++y) {
-                const float2 v = tr ? sm.tile[lane * C::P + y] : sm.tile[y * C::P + lane];
+                const float2 v = tr ? inner[lane * C::P + y] : inner[y * C::P + lane];
                 if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
             }
         }
@@ -285,7 +370,8 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
     k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient, mv);
-    k_grid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(g, rec_start, items, records, grid, mode, status, orient, mv);
+    k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, rec_start, (const uint32_t*)(ws + L.off_counts_home), items, records,
+                                                                 grid, mode, status, orient, mv);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }

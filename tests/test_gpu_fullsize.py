@@ -1,6 +1,6 @@
-"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (WS_GRID_OVERWRITE, split
-a1 / a2 calls, default workspace).  Medium is compared element by element; Large and Extreme on what the oracle can
-compute one by one: every key / bin offset (bit-exact), whole sampled w-planes of the mesh, sampled image pixels."""
+"""GPU parity at BASELINE.json's full sizes: Medium element by element through every path (run_chain); Kaiser-Bessel
+imaging and degridding at Large's size on sampled planes / pixels / visibilities plus the adjoint identity over all 10^8
+visibilities.  The Gaussian imaging path of Large, Extreme and paper_medium is compared as a WHOLE in test_gpu_wholearray.py."""
 import os
 
 import numpy as np
@@ -27,88 +27,8 @@ def test_medium_config_elementwise(oracle):
     print("medium grid", U.assert_close(out["grid"], G, "grid"), "image", U.assert_close(out["image"], D, "image"))
 
 
-def _bins_exact_without_sorting(oracle, prm, d, bins):
-    """keys, bin_start, sorted keys bit-exact; perm: a permutation of the kept indices whose keys are the sorted
-    keys, which is the same statement as 'every bin holds exactly its visibilities' (order inside a bin is free)."""
-    key = oracle.positions(prm, d.uvw.numpy(), d.n_chan, d.freqs_hz)["key"]
-    assert np.array_equal(bins["keys"], key)
-    bin_start, perm, dropped = oracle.bins(prm, key)
-    assert bins["n_dropped"] == dropped
-    assert np.array_equal(bins["bin_start"], bin_start)
-    assert np.array_equal(bins["sorted_keys"], key[perm])
-    gp = bins["perm"]
-    assert np.array_equal(key[gp], bins["sorted_keys"])
-    assert np.array_equal(np.sort(gp), np.flatnonzero(key != 0xFFFFFFFF).astype(np.uint32))
-
-
-def _sampled_check(oracle, cfg_name, planes_to_check, n_pix_samples, chunks=1):
-    import paper_2301_06061_b200 as ws
-    cfg = get_config(cfg_name)
-    dg = make_dataset(cfg, device="cuda")
-    d = dg.to("cpu")
-    plan = U.make_plan(d)
-    prm = U.oracle_params(oracle, d, plan.tile)
-    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
-    grid.fill_(float("nan"))
-    if chunks == 1:
-        wsp = plan.alloc_workspace(d.n_vis)
-        plan.bin_visibilities(dg.uvw, dg.vis, dg.weights, d.freqs_hz, wsp)
-        plan.grid_binned(grid, wsp, mode=ws.WS_GRID_OVERWRITE)
-        plan.async_status()
-        _bins_exact_without_sorting(oracle, prm, d, plan.get_bins())
-
-    else:   # row chunks streamed through repeated calls: first overwrites, the rest accumulate
-        rc = d.row_chunks()
-        wsp = plan.alloc_workspace(max(hi - lo for lo, hi in rc) * d.n_chan)
-        for i, (lo, hi) in enumerate(rc):
-            plan.grid_visibilities(dg.uvw[lo:hi], dg.vis[lo:hi], dg.weights[lo:hi], d.freqs_hz, grid, wsp,
-                                   mode=ws.WS_GRID_OVERWRITE if i == 0 else ws.WS_GRID_ACCUMULATE)
-            plan.async_status()
-    # whole sampled planes of the mesh, element by element
-    for k in planes_to_check:
-        G = oracle.grid(prm, *_np(d), plane_lo=k, plane_hi=k + 1)[0]
-        got = torch.fft.fftshift(grid[k], dim=(-2, -1)).cpu().numpy()
-        print(cfg_name, "plane", k, "errors", U.assert_close(got, G, f"mesh plane {k}"), "nonzero cells", np.count_nonzero(G))
-        del G, got
-    if chunks == 1 and plan.fft_is_own:
-        # what bench.py times: gridding that writes only the tiles holding visibilities (onto a NaN-filled mesh), then
-        # the own FFT with the fused w-correction, skipping what stayed empty
-        grid.fill_(float("nan"))
-        plan.grid_binned(grid, wsp, mode=ws.WS_GRID_SPARSE)
-        plan.fft_columns(grid, ws.WS_FFT_USE_OCCUPANCY)
-        plan.fft_rows_wcorrect(grid, image, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
-        plan.async_status()
-    else:
-        occ = ws.WS_FFT_USE_OCCUPANCY if plan.fft_is_own else 0
-        plan.fft_wcorrect(grid, image, wsp, accumulate=False, dirty=dirty, fft_flags=occ)
-    torch.cuda.synchronize()
-    img = image.cpu().numpy()
-    assert np.array_equal(dirty.cpu().numpy(), img.real)
-    # sampled pixels: the phase centre, the brightest model sources, the corners, random pixels
-    N, c = d.n_pix, d.n_pix // 2
-    rng = np.random.default_rng(99)
-    top = np.argsort(d.src_flux)[-4:]
-    q = [c, 0, N - 1, 0] + [int(round(d.src_m[i] / d.cell_rad)) + c for i in top]
-    p = [c, 0, N - 1, N - 1] + [int(round(d.src_l[i] / d.cell_rad)) + c for i in top]
-    q += list(rng.integers(0, N, n_pix_samples - len(q)))
-    p += list(rng.integers(0, N, n_pix_samples - len(p)))
-    q, p = np.clip(q, 0, N - 1), np.clip(p, 0, N - 1)
-    ref = oracle.image_samples(prm, *_np(d), q, p)
-    got = img[q, p].astype(np.complex128)
-    peak = max(np.abs(ref).max(), np.abs(img).max())
-    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
-    mx = np.abs(got - ref).max() / peak
-    print(cfg_name, "image samples: rel-L2 %.3e, max-abs/peak %.3e, peak %.4g" % (rel, mx, peak))
-    assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL
-    assert np.isfinite(img).all()
-
-
-# (Large as a whole -- all 64 planes of the mesh, the whole image, every bin -- is in test_gpu_wholearray.py.)
-
-
-@pytest.mark.skipif(os.environ.get("WS_SKIP_EXTREME") == "1", reason="WS_SKIP_EXTREME=1")
-def test_extreme_config_chunked_sampled(oracle):
-    _sampled_check(oracle, "extreme", planes_to_check=(16,), n_pix_samples=12, chunks=8)
+# (Large and Extreme as a whole -- every plane of the mesh, the whole image, every bin of Large -- and Extreme's streamed
+# chunks are in test_gpu_wholearray.py.)
 
 
 def _kb_beta(S, alpha=2.0):

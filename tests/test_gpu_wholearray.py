@@ -252,3 +252,57 @@ def test_image_from_host_at_8192_both_orientations(oracle, squeeze_axis):
     e.add(image, D)
     e.check()
     assert torch.equal(dirty_h.cuda(), image.real)
+
+
+@pytest.mark.skipif(os.environ.get("WS_SKIP_EXTREME") == "1", reason="WS_SKIP_EXTREME=1")
+def test_extreme_streamed_in_eight_chunks(oracle):
+    """Extreme's own recipe: eight row chunks of 775 snapshots through repeated gridding calls, as
+    bench.py --chunked times them -- first chunk WS_GRID_SPARSE, the others WS_GRID_SPARSE_ADD onto a mesh that is never
+    cleared (NaN-filled here) -- then the own FFT.  Compared: one whole plane of the mesh (written cells; unwritten ones
+    must be exact zeros of the oracle) and eight pixels of the image against the oracle's chain evaluated pixel by pixel
+    (the whole image of the same data is test_extreme_whole_mesh_and_image; the two GPU images must agree everywhere)."""
+    import paper_2301_06061_b200 as ws
+    dg = make_dataset(get_config("extreme"), device="cuda")
+    d = dg.to("cpu")
+    plan = U.make_plan(d)
+    prm = U.oracle_params(oracle, d, plan.tile)
+    grid, image, dirty = plan.alloc_grid(), plan.alloc_image(), plan.alloc_dirty()
+    rc = d.row_chunks()
+    assert len(rc) == 8
+    wsp = plan.alloc_workspace(max(hi - lo for lo, hi in rc) * d.n_chan)
+    grid.fill_(float("nan"))
+    for i, (lo, hi) in enumerate(rc):
+        plan.grid_visibilities(dg.uvw[lo:hi], dg.vis[lo:hi], dg.weights[lo:hi], d.freqs_hz, grid, wsp,
+                               mode=ws.WS_GRID_SPARSE if i == 0 else ws.WS_GRID_SPARSE_ADD)
+    plan.async_status()
+    transposed = bool(plan.occupancy()["transposed"])
+    k = 16
+    G = torch.from_numpy(oracle.grid(prm, *_np(d), plane_lo=k, plane_hi=k + 1)[0]).cuda()
+    got = _sparse_plane_logical(grid[k], transposed)
+    unwritten = torch.isnan(got.real)
+    assert not bool(torch.any(G[unwritten] != 0))
+    e = Running(f"extreme, 8 streamed chunks: mesh plane {k}")
+    e.add(torch.where(unwritten, torch.zeros_like(got), got), G)
+    e.check()
+    del G, got, unwritten
+    plan.fft_wcorrect(grid, image, wsp, accumulate=False, dirty=dirty, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    plan.async_status()
+    assert torch.equal(dirty, image.real)
+    N, c = d.n_pix, d.n_pix // 2
+    rng = np.random.default_rng(99)
+    q = np.array([c, 0, N - 1] + list(rng.integers(0, N, 5)))
+    p = np.array([c, N - 1, 0] + list(rng.integers(0, N, 5)))
+    ref = oracle.image_samples(prm, *_np(d), q, p)
+    got = image[torch.from_numpy(q).cuda(), torch.from_numpy(p).cuda()].cpu().numpy().astype(np.complex128)
+    peak = float(torch.abs(image).max())
+    rel, mx = np.linalg.norm(got - ref) / np.linalg.norm(ref), np.abs(got - ref).max() / peak
+    print("extreme, 8 streamed chunks: 8 image pixels rel-L2 %.3e, max-abs/peak %.3e" % (rel, mx))
+    assert rel <= U.REL_L2_TOL and mx <= U.MAX_ABS_TOL
+    # the one-call image of the same data (whole-array parity in test_extreme_whole_mesh_and_image) agrees everywhere
+    streamed = image.clone()
+    wsp1 = plan.alloc_workspace(d.n_vis, 2.0)
+    plan.grid_visibilities(dg.uvw, dg.vis, dg.weights, d.freqs_hz, grid, wsp1, mode=ws.WS_GRID_SPARSE)
+    plan.fft_wcorrect(grid, image, wsp1, accumulate=False, dirty=None, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    plan.async_status()
+    dd = torch.linalg.vector_norm((streamed - image).to(torch.complex128)) / torch.linalg.vector_norm(image.to(torch.complex128))
+    assert float(dd) <= 2e-6, float(dd)
