@@ -1,5 +1,7 @@
 """GPU parity over a seeded sweep of shapes and option combinations (-m gpu): support, kernel, channels, mesh size, plane
-count, frequency mode, snapshot hint, pre-summed channels -- mesh, image and the one-call degridding against the oracle."""
+count, frequency mode, snapshot hint, pre-summed channels -- mesh, image and the one-call degridding against the oracle,
+then the same image through streamed chunks (WS_GRID_SPARSE + WS_GRID_SPARSE_ADD), through the pipelined end-to-end
+entry, and as the sum of two plane ranges."""
 import numpy as np
 import pytest
 import torch
@@ -58,3 +60,32 @@ def test_random_shape(oracle, c):
     plan.predict_visibilities(torch.from_numpy(M).cuda(), dev.uvw, d.freqs_hz, d.n_chan, grid, pred, wsp)
     plan.async_status()
     U.assert_close(pred.cpu().numpy(), oracle.predict(prm, M, d.uvw.numpy(), d.n_chan, d.freqs_hz), "predicted visibilities")
+
+    # -- the same image from three streamed chunks onto a never-cleared mesh
+    cuts = sorted(set([0, d.n_rows // 3, d.n_rows // 3 + 7, d.n_rows]))
+    grid.fill_(float("nan"))
+    for i, (lo, hi) in enumerate(zip(cuts[:-1], cuts[1:])):
+        plan.grid_visibilities(dev.uvw[lo:hi].clone(), dev.vis[lo:hi].clone(), dev.weights[lo:hi].clone(), d.freqs_hz,   # (clone: 16-byte aligned)
+                               grid, wsp, mode=ws.WS_GRID_SPARSE if i == 0 else ws.WS_GRID_SPARSE_ADD)
+    plan.fft_wcorrect(grid, image, wsp, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+    plan.async_status()
+    U.assert_close(image.cpu().numpy(), D, "image from streamed chunks")
+    # -- the pipelined end-to-end entry with small chunks
+    plan.set_e2e_chunk_bytes(30000)
+    dirty, dirty_h = plan.alloc_dirty(), torch.full((d.n_pix, d.n_pix), float("nan"), dtype=torch.float32).pin_memory()
+    dev_in = torch.empty(plan.dev_inputs_bytes(d.n_rows, d.n_chan), dtype=torch.uint8, device="cuda")
+    grid.fill_(float("nan"))
+    plan.image_from_host(d.uvw.pin_memory(), d.vis.pin_memory(), d.weights.pin_memory(), d.freqs_hz, dev_in, grid, image, dirty, dirty_h, wsp)
+    rel = np.linalg.norm(dirty_h.numpy() - D.real) / np.linalg.norm(D.real)
+    assert rel <= U.REL_L2_TOL and np.abs(dirty_h.numpy() - D.real).max() <= U.MAX_ABS_TOL * np.abs(D).max(), rel
+    # -- two plane ranges (the rank-local half of the plane-sharded variant) sum to the image
+    if d.n_wplanes >= 2:
+        total = torch.zeros_like(image)
+        for lo, hi in ((0, d.n_wplanes // 2), (d.n_wplanes // 2, d.n_wplanes)):
+            plan.set_plane_range(lo, hi)
+            grid.fill_(float("nan"))
+            plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_SPARSE)
+            plan.fft_wcorrect(grid, image, wsp, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+            total += image
+        plan.async_status()
+        U.assert_close(total.cpu().numpy(), D, "sum over two plane ranges")
