@@ -768,6 +768,75 @@ __device__ __forceinline__ uint32_t super_row_of(uint32_t item) {
     else return item;
 }
 
+// ---- producer warp of the row kernels: clears the bands of a landing buffer that the last copy filled and the next one
+// will not, then brings the non-empty bands of the next plane in.  Lane wi < BW owns mask word wi (32 bands = 8 KB per row)
+// and issues one bulk copy per maximal run of set bits.
+template <int LOGN>
+__device__ __forceinline__ void rows_producer(float2* landing0, uint64_t* full, uint64_t* empty, const uint32_t* s_any,
+                                              const uint32_t* __restrict__ band_mask, const float2* __restrict__ planes, int nw,
+                                              uint32_t item_lo, uint32_t n_super, int lane) {
+    using C = RowCfg<LOGN>;
+    constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, LAND = C::LAND, BW = C::BW, NBUF = C::NBUF;
+    const size_t plane_elems = (size_t)N * N;
+    uint32_t was[NBUF], seq = 0;                      // seq: planes copied so far; plane seq lands in buffer seq % NBUF
+#pragma unroll
+    for (int i = 0; i < NBUF; ++i) was[i] = 0;
+    for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
+        const uint32_t sr = super_row_of<LOGN>(it);
+        for (int k = nw - 1; k >= 0; --k) {
+            if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
+            uint32_t now = 0;
+            if (lane < BW) {
+                const int lo = 32 * lane;
+                const uint32_t fullw = NT >= lo + 32 ? 0xFFFFFFFFu : (NT > lo ? (1u << (NT - lo)) - 1u : 0u);
+                now = band_mask ? (__ldg(band_mask + k * BW + lane) & fullw) : fullw;
+            }
+            // what needs neither `landing` nor the barrier happens before the wait for the consumers
+            uint32_t n_bands = __popc(now);
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) n_bands += __shfl_xor_sync(0xffffffffu, n_bands, d);
+            const uint32_t buf = seq % NBUF, use = seq / NBUF;       // this buffer's use-th filling
+            float2* landing = landing0 + buf * LAND;
+            const uint32_t stale = (NBUF == 2 && buf ? was[NBUF - 1] : was[0]) & ~now;
+            const bool any_stale = __any_sync(0xffffffffu, stale != 0);
+            if (use > 0) {
+                while (!mbar_try_wait(empty + buf, (use - 1) & 1u)) {}
+            }
+            // stale bands are cleared BEFORE the arrive: its release then orders the zeroing stores ahead of the
+            // consumers' reads (they acquire `full`), whatever the bulk copies' timing
+            if (any_stale) {
+#pragma unroll
+                for (int wi = 0; wi < BW; ++wi) {
+                    uint32_t z = __shfl_sync(0xffffffffu, stale, wi);
+                    while (z) {
+                        const int b = wi * 32 + __ffs(z) - 1;
+                        z &= z - 1;
+                        for (int r = 0; r < ROWS; ++r) landing[r * N + b * 32 + lane] = make_float2(0.f, 0.f);
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            __syncwarp();
+            if (lane == 0) mbar_expect_tx(full + buf, n_bands * 256u * ROWS);     // (the previous phase is complete now)
+            __syncwarp();
+            const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * LAND);
+            uint32_t m = now;
+            while (m) {
+                const int b0 = __ffs(m) - 1;
+                const uint32_t inv = ~(m >> b0);
+                const int len = inv ? __ffs(inv) - 1 : 32;
+                m &= ~((len == 32 ? 0xFFFFFFFFu : (1u << len) - 1u) << b0);
+                const size_t off = (size_t)(lane * 32 + b0) * 256;
+                for (int r = 0; r < ROWS; ++r)
+                    bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, full + buf);
+            }
+            if (NBUF == 2 && buf) was[NBUF - 1] = now;
+            else was[0] = now;
+            ++seq;
+        }
+    }
+}
+
 template <int LOGN>
 __global__ void __launch_bounds__(FT + PT, 1)
 k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ planes, float2* __restrict__ image,
@@ -812,67 +881,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     if (u >= FT) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
         if (u >= FT + 32) return;
-        // ---- producer warp: clears the bands of `landing` that the last copy filled and the next one will not, then
-        // brings the non-empty bands of the next plane in.  Lane wi < BW owns mask word wi (32 bands = 8 KB per row)
-        // and issues one bulk copy per maximal run of set bits.
-        const int lane = u & 31;
-        uint32_t was[NBUF], seq = 0;                      // seq: planes copied so far; plane seq lands in buffer seq % NBUF
-#pragma unroll
-        for (int i = 0; i < NBUF; ++i) was[i] = 0;
-        for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
-            const uint32_t sr = super_row_of<LOGN>(it);
-            for (int k = nw - 1; k >= 0; --k) {
-                if (!((s_any[k >> 5] >> (k & 31)) & 1u)) continue;
-                uint32_t now = 0;
-                if (lane < BW) {
-                    const int lo = 32 * lane;
-                    const uint32_t fullw = NT >= lo + 32 ? 0xFFFFFFFFu : (NT > lo ? (1u << (NT - lo)) - 1u : 0u);
-                    now = band_mask ? (__ldg(band_mask + k * BW + lane) & fullw) : fullw;
-                }
-                // what needs neither `landing` nor the barrier happens before the wait for the consumers
-                uint32_t n_bands = __popc(now);
-#pragma unroll
-                for (int d = 16; d >= 1; d >>= 1) n_bands += __shfl_xor_sync(0xffffffffu, n_bands, d);
-                const uint32_t buf = seq % NBUF, use = seq / NBUF;       // this buffer's use-th filling
-                float2* landing = landing0 + buf * LAND;
-                const uint32_t stale = (NBUF == 2 && buf ? was[NBUF - 1] : was[0]) & ~now;
-                const bool any_stale = __any_sync(0xffffffffu, stale != 0);
-                if (use > 0) {
-                    while (!mbar_try_wait(empty + buf, (use - 1) & 1u)) {}
-                }
-                // stale bands are cleared BEFORE the arrive: its release then orders the zeroing stores ahead of the
-                // consumers' reads (they acquire `full`), whatever the bulk copies' timing
-                if (any_stale) {
-#pragma unroll
-                    for (int wi = 0; wi < BW; ++wi) {
-                        uint32_t z = __shfl_sync(0xffffffffu, stale, wi);
-                        while (z) {
-                            const int b = wi * 32 + __ffs(z) - 1;
-                            z &= z - 1;
-                            for (int r = 0; r < ROWS; ++r) landing[r * N + b * 32 + lane] = make_float2(0.f, 0.f);
-                        }
-                    }
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                }
-                __syncwarp();
-                if (lane == 0) mbar_expect_tx(full + buf, n_bands * 256u * ROWS);     // (the previous phase is complete now)
-                __syncwarp();
-                const char* src = (const char*)(planes + (size_t)k * plane_elems + (size_t)sr * LAND);
-                uint32_t m = now;
-                while (m) {
-                    const int b0 = __ffs(m) - 1;
-                    const uint32_t inv = ~(m >> b0);
-                    const int len = inv ? __ffs(inv) - 1 : 32;
-                    m &= ~((len == 32 ? 0xFFFFFFFFu : (1u << len) - 1u) << b0);
-                    const size_t off = (size_t)(lane * 32 + b0) * 256;
-                    for (int r = 0; r < ROWS; ++r)
-                        bulk_g2s((char*)landing + (size_t)r * N * 8 + off, src + (size_t)r * N * 8 + off, len * 256, full + buf);
-                }
-                if (NBUF == 2 && buf) was[NBUF - 1] = now;
-                else was[0] = now;
-                ++seq;
-            }
-        }
+        rows_producer<LOGN>(landing0, full, empty, s_any, band_mask, planes, nw, item_lo, n_super, u & 31);
         return;
     }
 
