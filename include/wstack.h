@@ -29,7 +29,10 @@
  *     row (j + N/2) mod N, column (i + N/2) mod N, so that the FFT needs no shift pass.  After
  *     ws_fft_planes logical pixel (q, p) of plane k sits at the same wrapped position.
  *   - Image layout: complex64 [n_pix][n_pix], CENTRED: pixel (q, p) <-> (m, l) = ((q-N/2), (p-N/2)) cell_rad.
- *   - One plan per host thread.
+ *   - One plan per host thread.  Every call that touches the device makes the plan's device current for its duration and
+ *     restores the caller's afterwards (ws_plan_create leaves the plan's device current).
+ *   - With WS_FLAG_MESH_F64 the mesh, image and dirty image are complex128 / complex128 / float64 wherever this header says
+ *     complex64 / complex64 / float32 (the `float* dirty` arguments then point to doubles).
  */
 #ifndef WSTACK_H
 #define WSTACK_H

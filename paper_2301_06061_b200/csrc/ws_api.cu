@@ -15,6 +15,20 @@ constexpr double C_LIGHT = 299792458.0;
 constexpr double PI = 3.14159265358979323846264338327950288;
 constexpr int64_t MAX_VIS = (int64_t)1 << 30;
 
+// Makes the plan's device current for the duration of a call and restores the caller's afterwards: a process that holds
+// plans on several devices (or whose current device simply differs) must not launch against another device's pointers.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const ws_plan* plan) {
+        if (!plan) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != plan->prm.device) switched = cudaSetDevice(plan->prm.device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
 int fail(ws_plan* plan, int code, const char* msg) {
     if (plan) plan->last_error = msg;
     return code;
@@ -283,6 +297,7 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
 }
 
 int ws_plan_destroy(ws_plan* plan) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (plan->e2e_ready) {
         cudaStreamDestroy(plan->copy_stream);
@@ -351,6 +366,7 @@ size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_f
 size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis) { return ws_workspace_bytes_for(plan, max_vis, 4.0); }
 
 int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_zero: null argument");
     int rc = ws_launch_zero(plan, grid, ws_grid_bytes(plan), (cudaStream_t)stream);
     if (rc >= 0) rc = ws_launch_fft_masks_clear(plan, (cudaStream_t)stream);
@@ -442,10 +458,12 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
 int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
                         const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
                         size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true);
 }
 
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid || !workspace) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: null pointer");
     if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
@@ -502,6 +520,7 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
 int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
                          const double* freq_hz, int64_t n_rows, int32_t n_chan, void* grid, int32_t mode,
                          void* workspace, size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_visibilities: null pointer");
     if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
@@ -564,11 +583,13 @@ static int fft_planes_dir(ws_plan* plan, void* grid, void* workspace, size_t wor
 }
 
 int ws_fft_planes(ws_plan* plan, void* grid, void* workspace, size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     return fft_planes_dir(plan, grid, workspace, workspace_bytes, stream, CUFFT_INVERSE);
 }
 
 int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void* workspace, size_t workspace_bytes,
                       void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !model_image || !planes) return fail(plan, WS_ERR_INVALID_ARG, "ws_predict_planes: null argument");
     if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "ws_predict_planes: no degridding with WS_FLAG_MESH_F64");
     if (((uintptr_t)model_image | (uintptr_t)planes) & 15)
@@ -585,6 +606,7 @@ int ws_predict_planes(ws_plan* plan, const void* model_image, void* planes, void
 int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_hz, int64_t n_rows, int32_t n_chan,
                            const void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
                            size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!planes || (n_rows > 0 && !vis_out)) return fail(plan, WS_ERR_INVALID_ARG, "ws_degrid_visibilities: null pointer");
     if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_degrid_visibilities: bad flag");
@@ -606,6 +628,7 @@ int ws_degrid_visibilities(ws_plan* plan, const float* uvw, const double* freq_h
 int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float* uvw, const double* freq_hz, int64_t n_rows,
                             int32_t n_chan, void* planes, void* vis_out, float scale, int32_t accumulate, void* workspace,
                             size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!plan->fft_own || !plan->fft_rows1d_ok) {      // the two library calls in sequence
         const int rc = ws_predict_planes(plan, model_image, planes, workspace, workspace_bytes, stream);
@@ -657,6 +680,7 @@ int ws_predict_visibilities(ws_plan* plan, const void* model_image, const float*
 
 int ws_wcorrect_accumulate(ws_plan* plan, const void* planes, void* image, int32_t accumulate, float* dirty,
                            void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !planes || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: null argument");
     if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_wcorrect_accumulate: bad flag");
     if (((uintptr_t)planes | (uintptr_t)image | (uintptr_t)dirty) & 15)
@@ -677,6 +701,7 @@ static int fft_sparse_flag(ws_plan* plan, const void* grid, uint32_t fft_flags, 
 }
 
 int ws_fft_columns(ws_plan* plan, void* grid, uint32_t fft_flags, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_columns: null argument");
     if ((uintptr_t)grid & 15) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_columns: grid must be 16-byte aligned");
     if (!plan->fft_own) return fail(plan, WS_ERR_UNSUPPORTED, "ws_fft_columns: this plan uses the library FFT");
@@ -690,6 +715,7 @@ int ws_fft_columns(ws_plan* plan, void* grid, uint32_t fft_flags, void* stream) 
 
 int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t accumulate, float* dirty,
                          uint32_t fft_flags, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !grid || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_rows_wcorrect: null argument");
     if (accumulate != 0 && accumulate != 1) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_rows_wcorrect: bad flag");
     if (((uintptr_t)grid | (uintptr_t)image | (uintptr_t)dirty) & 15)
@@ -706,6 +732,7 @@ int ws_fft_rows_wcorrect(ws_plan* plan, const void* grid, void* image, int32_t a
 
 int ws_fft_wcorrect(ws_plan* plan, void* grid, void* image, int32_t accumulate, float* dirty, uint32_t fft_flags,
                     void* workspace, size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !grid || !image) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_wcorrect: null argument");
     if (!plan->fft_own) {     // library FFT (needs a fully written mesh), then the stand-alone a4 pass
         if (fft_flags & ~(uint32_t)WS_FFT_USE_OCCUPANCY) return fail(plan, WS_ERR_INVALID_ARG, "ws_fft_wcorrect: bad fft_flags");
@@ -719,6 +746,7 @@ int ws_fft_wcorrect(ws_plan* plan, void* grid, void* image, int32_t accumulate, 
 }
 
 int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm_flags, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !image || !dirty) return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: null argument");
     if (norm_flags & ~(uint32_t)(WS_NORM_SUMWT | WS_NORM_N | WS_NORM_TAPER))
         return fail(plan, WS_ERR_INVALID_ARG, "ws_dirty_image: unknown norm_flags");
@@ -734,6 +762,7 @@ int ws_dirty_image(ws_plan* plan, const void* image, float* dirty, uint32_t norm
 }
 
 int ws_get_sum_weights(ws_plan* plan, double* sum_weights, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan || !sum_weights) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_sum_weights: null argument");
     if (!(plan->prm.flags & WS_FLAG_TRACK_SUMWT))
         return fail(plan, WS_ERR_INVALID_ARG, "ws_get_sum_weights: plan was not created with WS_FLAG_TRACK_SUMWT");
@@ -754,6 +783,7 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
                        const double* freq_hz, int64_t n_rows, int32_t n_chan, void* dev_inputs,
                        size_t dev_inputs_bytes, void* grid, void* image, float* dirty_d, float* dirty_h,
                        void* workspace, size_t workspace_bytes, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!uvw_h || !vis_h || !weights_h || !dev_inputs || !grid || !image || !dirty_d || !dirty_h || !workspace)
         return fail(plan, WS_ERR_INVALID_ARG, "ws_image_from_host: null argument");
@@ -861,6 +891,7 @@ int ws_image_from_host(ws_plan* plan, const float* uvw_h, const void* vis_h, con
 }
 
 int ws_async_status(ws_plan* plan, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(plan, e, "ws_async_status: synchronize");
@@ -877,6 +908,7 @@ int ws_async_status(ws_plan* plan, void* stream) {
 int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_keys, const uint32_t** perm,
                 const uint32_t** bin_start, int64_t* n_vis, int64_t* n_bins, int64_t* n_dropped,
                 int64_t* n_records, void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!plan->last_valid) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_bins: no bins (no grid call, or workspace reused by the FFT)");
     cudaStream_t st = (cudaStream_t)stream;
@@ -907,6 +939,7 @@ int ws_get_bins(ws_plan* plan, const uint32_t** keys, const uint32_t** sorted_ke
 
 int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* bands, double* planes, int32_t* transposed,
                      void* stream) {
+    const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
     if (!plan->d_masks || !plan->occ_grid) return fail(plan, WS_ERR_INVALID_ARG, "ws_get_occupancy: no occupancy recorded");
     cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);

@@ -23,6 +23,9 @@ k_probe_ffma(float* __restrict__ out, int iters, float a, float b) {
 
 extern "C" int ws_measure_fp32_tflops(ws_plan* plan, double* tflops, void* stream) {
     if (!plan || !tflops) return WS_ERR_INVALID_ARG;
+    int prev = -1;
+    const bool switched = cudaGetDevice(&prev) == cudaSuccess && prev != plan->prm.device && cudaSetDevice(plan->prm.device) == cudaSuccess;
+    struct Restore { int d; bool on; ~Restore() { if (on) cudaSetDevice(d); } } restore{prev, switched};
     cudaStream_t st = (cudaStream_t)stream;
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return WS_ERR_CUDA;
