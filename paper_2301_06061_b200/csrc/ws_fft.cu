@@ -858,7 +858,6 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     const int u = threadIdx.x, g = u >> 8;
     const int par = C::SPLIT64 ? (int)(blockIdx.x & 1u) : 0;           // (the grid is even: every item of a CTA has its parity)
     const int nw = prm.n_wplanes;
-    const size_t plane_elems = (size_t)N * N;
     for (int i = u; i < tw_smem_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
     for (int i = u; i < NBUF * LAND; i += FT + PT) landing0[i] = make_float2(0.f, 0.f);
     for (int k0 = 0; k0 < nw; k0 += FT + PT) {       // (FT + PT is a multiple of 32: one ballot per mask word)
