@@ -68,14 +68,17 @@ __host__ __device__ constexpr int tw_offset(int logn, int s) {
     return o;
 }
 __host__ __device__ constexpr int tw_entries(int logn) { return tw_offset(logn, n_stages(logn) - 1); }   // last stage: Q = 1, none
-// what of it the row kernel keeps in shared memory: everything, except for N = 16384, whose first-stage twiddles are
-// thread constants held in registers (7 exact values, the 16 twiddles of a thread are products of two of them) because
-// the 128 KB landing buffer leaves no room for a table: only stage 1 then.  (Measured at N = 8192: register twiddles +
-// a second landing buffer in the freed shared memory, 12.06 ms against 11.72 with the table -- the two dependent
-// complex multiplies per output cost more issue slots and latency than the table's loads; not used there.)
-__host__ __device__ constexpr bool tw_in_regs(int logn) { return logn >= 14; }
-__host__ __device__ constexpr int tw_smem_entries(int logn) { return tw_in_regs(logn) ? tw_entries(logn) - tw_offset(logn, 1) : tw_entries(logn); }
-__host__ __device__ constexpr int tw_smem_off1(int logn) { return tw_in_regs(logn) ? 0 : tw_offset(logn, 1); }
+// what of it the row kernel keeps in shared memory: everything, except for N = 16384, where the 128 KB landing buffer
+// leaves no room for the first-stage table (63 x 256 entries): there the first-stage twiddle of output digit d = 4 (4 a + b) + q
+// is the product of two factors from two small tables, W_N^(ug (4 b + q)) (the two q of the CTA: 2 x 4 x 256 entries) and
+// W_N^(16 a ug) (3 x 256), beside the stage-1 table.  (Measured at N = 8192: factored twiddles + a second landing buffer in the
+// freed shared memory, 12.06 ms against 11.72 with the full table -- the second, dependent complex multiply per output costs
+// more issue slots and latency than the table's loads; not used there.)
+__host__ __device__ constexpr bool tw_factored(int logn) { return logn >= 14; }
+// (+ 3 x 256 entries W_N^(4 M a ug), a = 1..3: the second factor of the register twiddles, fetched per use)
+// and 2 x 4 x 256 entries W_N^(ug (M b + q)) for the two q of the CTA's groups: the first factor)
+__host__ __device__ constexpr int tw_smem_entries(int logn) { return tw_factored(logn) ? tw_entries(logn) - tw_offset(logn, 1) + 768 + 2048 : tw_entries(logn); }
+__host__ __device__ constexpr int tw_smem_off1(int logn) { return tw_factored(logn) ? 0 : tw_offset(logn, 1); }
 
 __host__ __device__ constexpr int brev(int i, int bits) {
     int r = 0;
@@ -538,7 +541,7 @@ struct RowCfg {
     static constexpr bool SPLIT64 = LOGN == 14;       // first stage: radix 64 split over the groups of TWO CTAs (by output parity)
     static constexpr int ITEMS_PER_ROW = SPLIT64 ? 2 : 1;
     static constexpr int BW = band_words(NT);
-    static constexpr int NBUF = 1;                    // landing buffers (2 works where the shared memory allows it; see tw_in_regs)
+    static constexpr int NBUF = 1;                    // landing buffers (2 works where the shared memory allows it; see tw_factored)
     static constexpr int LRL = log2r(LOGN, S - 1);    // last stage
 };
 
@@ -686,20 +689,29 @@ struct Grouped {
             for (int m = 0; m < 16; ++m) x[m] = in[256 * m];
         }
     }
-    // tc (N >= 8192): the thread's first-stage twiddles as 7 register constants.  Its outputs are the digits d = M p + q,
-    // p = 4 a + b < 16 (N = 8192: M = 2, q = g; N = 16384: M = 4, q = 2 g + parity): tc[b] = W_N^(ug (M b + q)), b < 4,
-    // tc[3 + a] = W_N^(4 M a ug), a = 1..3, and output d is multiplied by tc[b] tc[3 + a] (two roundings instead of one).
+    // tw_factored (N = 16384): no room for the whole first-stage table (63 x 256 entries) beside the 128 KB landing buffer.  A
+    // thread's outputs are the digits d = M p + q, p = 4 a + b < 16 (M = 4, q = 2 g + parity of the CTA), and
+    // W_N^(ug d) = W_N^(ug (M b + q)) W_N^(4 M a ug): two factors from two small tables in shared memory (8 + 3 x 256 entries
+    // per CTA, 7 loads per thread and plane instead of 15; two roundings instead of one).  As register constants they spilled.
     __device__ static __forceinline__ void finish_first(float2* x, float2* __restrict__ work, const float2* __restrict__ tw,
-                                                        int ug, int g, const float2* tc) {
+                                                        int ug, int g) {
         bfly<float2, 4>(x);
-        if constexpr (SPLIT && tw_in_regs(LOGN)) {
+        if constexpr (SPLIT && tw_factored(LOGN)) {
             float2* out = work + g * 272 + ug + (ug >> 4);
 #pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                const int pq = brev(r, 4), b = pq & 3, a = pq >> 2;
-                float2 v = emul(x[r], tc[b].x, tc[b].y);
-                if (a) v = emul(v, tc[3 + a].x, tc[3 + a].y);
-                out[pq * 544] = v;
+            for (int b = 0; b < 4; ++b) {
+                constexpr int n1 = tw_entries(LOGN) - tw_offset(LOGN, 1);
+                const float2 tb = tw[n1 + 768 + (g * 4 + b) * 256 + ug];                  // W_N^(ug (M b + q))
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    const int pq = 4 * a + b, r = brev(pq, 4);
+                    float2 v = emul(x[r], tb.x, tb.y);
+                    if (a) {
+                        const float2 pa = tw[n1 + (a - 1) * 256 + ug];                     // W_N^(4 M a ug)
+                        v = emul(v, pa.x, pa.y);
+                    }
+                    out[pq * 544] = v;
+                }
             }
         } else if constexpr (SPLIT32) {
             float2* out = work + g * 272 + ug + (ug >> 4);
@@ -858,7 +870,15 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     const int u = threadIdx.x, g = u >> 8;
     const int par = C::SPLIT64 ? (int)(blockIdx.x & 1u) : 0;           // (the grid is even: every item of a CTA has its parity)
     const int nw = prm.n_wplanes;
-    for (int i = u; i < tw_smem_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
+    if constexpr (tw_factored(LOGN)) {
+        constexpr int n1 = tw_entries(LOGN) - tw_offset(LOGN, 1);
+        for (int i = u; i < n1; i += FT + PT) tw[i] = tw_g[i];
+        for (int i = u; i < 768; i += FT + PT) tw[n1 + i] = tc_g[16 * 256 + i];
+        for (int i = u; i < 2048; i += FT + PT)        // [g][b][ug] <- [q = 2 g + par][b][ug]
+            tw[n1 + 768 + i] = tc_g[((2 * (i >> 10) + par) * 4 + ((i >> 8) & 3)) * 256 + (i & 255)];
+    } else {
+        for (int i = u; i < tw_smem_entries(LOGN); i += FT + PT) tw[i] = tw_g[i];
+    }
     for (int i = u; i < NBUF * LAND; i += FT + PT) landing0[i] = make_float2(0.f, 0.f);
     for (int k0 = 0; k0 < nw; k0 += FT + PT) {       // (FT + PT is a multiple of 32: one ballot per mask word)
         const int k = k0 + u;
@@ -885,7 +905,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     }
 
     // ---- the 16 compute warps (they take over the registers the producer's warpgroup gave back: the pool is the CTA's
-    // launch allocation, 640 x 96 registers, so 112 is the most that 512 threads can take; asking for more blocks forever)
+    // launch allocation, 640 x 96 registers, so 112 is the most that 512 threads can take; asking for more blocks forever.
+    // ptxas honours the raised budget in this region -- without setmaxnreg, 544 threads compile to 96 registers and spill)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
     auto cta_sync = [&]() { asm volatile("bar.sync 3, %0;" ::"r"(FT) : "memory"); };     // (the producer is not part of it)
     auto group_sync = [&]() {
@@ -894,15 +915,6 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     };
     uint32_t seq = 0;                      // planes consumed so far (the producer's count, same order)
     const int top_span_lo = ((nw - 1) / WC_SPAN) * WC_SPAN;
-    float2 tc[7];      // N >= 8192: first-stage twiddles of this thread (Grouped::finish_first), constant for the whole kernel
-    if constexpr (tw_in_regs(LOGN)) {
-        const int q = C::SPLIT64 ? 2 * g + par : g;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) tc[i] = __ldg(tc_g + (q * 4 + i) * 256 + (u & 255));
-#pragma unroll
-        for (int i = 0; i < 3; ++i) tc[4 + i] = __ldg(tc_g + (16 + i) * 256 + (u & 255));
-    }
-
     for (uint32_t it = item_lo + blockIdx.x; it < n_super; it += gridDim.x) {
         const uint32_t sr = super_row_of<LOGN>(it);
         float2 rot[EPT], h[EPT];
@@ -931,7 +943,7 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
                     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + buf)) : "memory");
                 // ---- arithmetic, twiddles, exchanges
                 if constexpr (C::GROUPED) {
-                    Grouped<LOGN>::finish_first(x, work, tw, u & 255, g, tc);
+                    Grouped<LOGN>::finish_first(x, work, tw, u & 255, g);
                     group_sync();
                     Grouped<LOGN>::second_third(x, work, tw, u & 255, g);
                 } else {
@@ -1046,7 +1058,7 @@ template <int LOGN>
 int init_n(ws_plan* plan) {
     constexpr int N = 1 << LOGN, R0 = N / 256;
     std::vector<float2> tw;
-    for (int s = tw_in_regs(LOGN) ? 1 : 0; s + 1 < n_stages(LOGN); ++s) {
+    for (int s = tw_factored(LOGN) ? 1 : 0; s + 1 < n_stages(LOGN); ++s) {
         const int L = 1 << log2l(LOGN, s), R = 1 << log2r(LOGN, s), Q = L / R;
         for (int m = 1; m < R; ++m)
             for (int j = 0; j < Q; ++j) tw.push_back(unit((long long)j * m, L));
@@ -1058,7 +1070,7 @@ int init_n(ws_plan* plan) {
     for (int m = 1; m < 16; ++m)
         for (int j = 0; j < 16; ++j) tw.push_back(unit((long long)j * m, 256));
     plan->tw_off_c = tw.size();
-    if (tw_in_regs(LOGN)) {
+    if (tw_factored(LOGN)) {
         const int M = LOGN == 14 ? 4 : 2;          // first-stage digits of one thread: d = M p + q, q < M
         for (int q = 0; q < 4; ++q)
             for (int b = 0; b < 4; ++b)
