@@ -361,7 +361,8 @@ def main():
         if chunks:
             return step_chunked(ev)
         if ev: ev[0].record()
-        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+        # (bins for the mode that follows: the sparse modes store home records only and spread each tile's ring)
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else ws.WS_GRID_OVERWRITE)
         if ev: ev[1].record()
         if own:     # the mesh is neither cleared nor completely written: the FFT passes skip what stayed empty
             plan.grid_binned(grid, wsp, mode=ws.WS_GRID_SPARSE)
@@ -383,9 +384,9 @@ def main():
     bins_info = None
     if chunks:      # statistics of the first chunk stand for all (same recipe per chunk)
         lo0, hi0 = chunks[0]
-        plan.bin_visibilities(d.uvw[lo0:hi0], d.vis[lo0:hi0], d.weights[lo0:hi0], d.freqs_hz, wsp)
+        plan.bin_visibilities(d.uvw[lo0:hi0], d.vis[lo0:hi0], d.weights[lo0:hi0], d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else None)
     else:
-        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else None)
     b = plan.get_bins(fields=("bin_start",))
     bins_info = {"n_dropped": b["n_dropped"], "n_records": b["n_records"],
                  "max_bin": int(np.diff(b["bin_start"].astype(np.int64)).max()),

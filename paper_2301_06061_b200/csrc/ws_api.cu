@@ -223,6 +223,8 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->last_weights = nullptr;
     plan->snapshot_rows = 0;
     plan->last_has_values = false;
+    plan->bin_ring = false;
+    plan->last_ring = false;
     plan->last_chan_per_key = 1;
     plan->launches = 0;
     plan->last_valid = false;
@@ -399,8 +401,10 @@ static int make_chan_consts(ws_plan* plan, const double* freq_hz, int32_t n_chan
 }
 
 // a1 for the gridder (with_values) and for the degridder (positions only: vis and weights are not read)
+// ring: only the home records are stored (the sparse gridding modes spread each tile's ring onto its neighbours)
 static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const float* weights, const double* freq_hz,
-                    int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values) {
+                    int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values,
+                    bool ring = false) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "WS_FLAG_MESH_F64: nothing is binned (ws_grid_visibilities grids directly); no degridding");
     if (n_rows < 0 || n_chan <= 0) return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad n_rows / n_chan");
@@ -420,7 +424,7 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
     const int32_t n_chan_in = n_chan;
     WsLayout L;
     // positions only (degridding): home records alone, so that the rest of the workspace stays free for the caller's use
-    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0, with_values ? 4 : 1) ||
+    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0, with_values && !ring ? 4 : 1) ||
         (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
         return fail(plan, WS_ERR_WORKSPACE, "ws_bin_visibilities: workspace too small (see ws_workspace_bytes_for)");
     const void* vis_in = vis;
@@ -441,8 +445,11 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
 
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
+    plan->bin_ring = with_values && ring;
     const int rc = ws_launch_bin(plan, L, (char*)workspace, cc, uvw, (const float2*)vis_in, wt_in, n_rows, n_chan,
                                  (cudaStream_t)stream);
+    plan->last_ring = plan->bin_ring;
+    plan->bin_ring = false;
     if (rc < 0) return fail(plan, rc, "ws_bin_visibilities: launch failed");
     plan->launches += rc;
     plan->last_ws = workspace;
@@ -462,6 +469,17 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
     return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true);
 }
 
+int ws_bin_visibilities_for(ws_plan* plan, int32_t mode, const float* uvw, const void* vis, const float* weights,
+                            const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes,
+                            void* stream) {
+    const DeviceGuard device_guard(plan);
+    if (!plan) return WS_ERR_INVALID_ARG;
+    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities_for: bad mode");
+    const bool ring = (mode == WS_GRID_SPARSE || mode == WS_GRID_SPARSE_ADD) && plan->fft_own;
+    return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true, ring);
+}
+
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
     const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
@@ -478,6 +496,8 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written): use WS_GRID_SPARSE_ADD");
     if (mode == WS_GRID_SPARSE_ADD && !(plan->occ_sparse && plan->occ_grid == grid))
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: WS_GRID_SPARSE_ADD needs a mesh this plan wrote with WS_GRID_SPARSE");
+    if (plan->last_ring && !sparse_mode)
+        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: these bins hold home records only (ws_bin_visibilities_for a sparse mode)");
     cudaStream_t st = (cudaStream_t)stream;
     // Tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE /
     // SPARSE_ADD.  It comes BEFORE the gridding kernel -- a SPARSE mesh is stored in the orientation the masks favour --
@@ -551,7 +571,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
         plan->launches += rc;
         return WS_OK;
     }
-    const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
+    const int rc = ws_bin_visibilities_for(plan, mode, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
     return ws_grid_binned(plan, grid, mode, workspace, workspace_bytes, stream);
 }

@@ -95,7 +95,8 @@ k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsG
         // tiles the footprint overlaps: own, and the neighbour on each side it sticks out of
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-        if (home_only) dx = dy = 0;               // bins for the degridder: a gather needs no copies in neighbour tiles
+        if (home_only == 1) dx = dy = 0;          // bins for the degridder: a gather needs no copies in neighbour tiles
+                                                  // (2: the ring scheme of the gridder counts the halo -- occupancy -- but stores no copies)
     }
     if (m < n_vis) keys[m] = home;
     // two histograms: visibilities per home bin (-> bin_start) and halo copies received per bin; the record
@@ -195,7 +196,7 @@ k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t n, c
 __global__ void __launch_bounds__(256)
 k_finish_offsets(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
                  uint32_t* __restrict__ rec_start, uint32_t* __restrict__ cursor_home, uint32_t* __restrict__ cursor_halo,
-                 uint32_t n_bins, WsStatus* __restrict__ status, uint64_t rec_capacity) {
+                 uint32_t n_bins, WsStatus* __restrict__ status, uint64_t rec_capacity, int home_only) {
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
     if (b > n_bins) return;
     const uint32_t bs = bin_start[b], hs = halo_start[b];
@@ -204,9 +205,10 @@ k_finish_offsets(const uint32_t* __restrict__ bin_start, const uint32_t* __restr
         cursor_home[b] = bs;
         cursor_halo[b] = bin_start[b + 1] + hs;
     } else {
+        const uint64_t n_rec = home_only == 2 ? (uint64_t)bs : (uint64_t)bs + (uint64_t)hs;   // (2: only home records are stored)
         status->n_kept = bs;
-        status->n_records = bs + hs;
-        if ((uint64_t)bs + (uint64_t)hs > rec_capacity) status->overflow = status->sticky_overflow = 1u;
+        status->n_records = (uint32_t)n_rec;
+        if (n_rec > rec_capacity) status->overflow = status->sticky_overflow = 1u;
     }
 }
 
@@ -249,7 +251,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         hs = __ldg(halo_start + home);
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-        if (home_only) dx = dy = 0;
+        if (home_only) dx = dy = 0;               // (1: degridder; 2: ring scheme -- no copies in neighbour tiles either way)
     }
     // slots: every group leader issues its atomics back to back, the results are broadcast afterwards.  The home
     // copy needs no second atomic: its record slot is its perm slot shifted by the bin's halo_start.
@@ -282,7 +284,7 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         records[slot] = make_float4(__uint_as_float(X), __uint_as_float(Y), vr, vi);
     };
     perm[bh] = m;
-    emit(bh + hs, 0, 0);
+    emit(home_only == 2 ? bh : bh + hs, 0, 0);      // (ring scheme: the record lists hold home records only, indexed by bin_start)
     if (q.nx) emit(bx, dx, 0);
     if (q.ny) emit(by, 0, dy);
     if (q.nc) emit(bc, dx, dy);
@@ -364,7 +366,7 @@ int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const floa
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {
     const WsGeom& g = plan->geom;
-    const int home_only = vis == nullptr;          // positions only: the degridder's gather
+    const int home_only = vis == nullptr ? 1 : (plan->bin_ring ? 2 : 0);   // 1: positions only (degridder); 2: home records only (ring scheme)
     WsRemap rm = {0u, 0u, 0u, 0u, 0u};
     if (plan->snapshot_rows > 0 && n_rows >= 2 * plan->snapshot_rows) {
         const uint64_t F = (uint64_t)plan->snapshot_rows * (uint64_t)n_chan;
@@ -408,7 +410,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     k_scan_block_sums<<<dim3(1, 2), SCAN_THREADS, 0, st>>>(block_sums, n_blocks);
     k_scan_apply<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
     k_finish_offsets<<<(n_scan + 255) / 256, 256, 0, st>>>(counts_home, counts_halo, rec_start, cursor_home, cursor_halo,
-                                                          g.n_bins, status, L.rec_capacity);
+                                                          g.n_bins, status, L.rec_capacity, home_only);
     launches += 4;
     if (n_vis) {
         k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift,

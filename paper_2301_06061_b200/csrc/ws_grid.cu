@@ -234,23 +234,36 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
     __syncwarp();
 }
 
-// Queues the chunks of the heavy bins as work items and (OVERWRITE mode) clears their tiles.
+// Queues the chunks of the heavy bins as work items and clears the tiles that will be ADDED to: those of the heavy bins
+// (their chunks are added with red) and, in the ring scheme, every tile that receives anything at all -- its own records or
+// a neighbour's ring (occ_start: home + halo counts).  starts: offsets of the record lists ([n_bins + 1]).  In
+// WS_GRID_SPARSE_ADD mode a tile that earlier chunks filled is left alone; WS_GRID_ACCUMULATE clears nothing.
 __global__ void __launch_bounds__(256)
-k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, uint4* __restrict__ items,
-                uint32_t item_capacity, WsStatus* __restrict__ status, float2* __restrict__ grid, int mode,
-                const uint32_t* __restrict__ orient, const WsMaskView mv) {
+k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ starts, const uint32_t* __restrict__ occ_start,
+                int ring, uint4* __restrict__ items, uint32_t item_capacity, WsStatus* __restrict__ status,
+                float2* __restrict__ grid, int mode, const uint32_t* __restrict__ orient, const WsMaskView mv) {
     if (status->overflow) return;
     const bool tr = orient && *orient;
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    uint32_t s = 0, cnt = 0;
+    uint32_t s = 0, cnt = 0, occ = 0;
     if (b < g.n_bins) {
-        s = rec_start[b];
-        cnt = rec_start[b + 1] - s;
+        s = starts[b];
+        cnt = starts[b + 1] - s;
+        occ = ring ? occ_start[b + 1] - occ_start[b] : cnt;
     }
     const bool heavy = cnt > WS_CHUNK;
     const uint32_t chunks = heavy ? (cnt + WS_CHUNK - 1) / WS_CHUNK : 0u;
     const unsigned hm = __ballot_sync(0xffffffffu, heavy);
+    bool clear = mode != WS_GRID_ACCUMULATE && (ring ? occ > 0 : heavy);
+    if (clear && mode == WS_GRID_SPARSE_ADD) {              // a tile earlier chunks filled is added to, not cleared
+        const uint32_t nt = (uint32_t)g.nt, tx = b % nt, r = b / nt;
+        clear = !ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx);
+    }
+    for (unsigned m = __ballot_sync(0xffffffffu, clear); m; m &= m - 1) {
+        const uint32_t hb = (b - lane) + (__ffs(m) - 1);
+        store_zero_tile(tile_origin(g, grid, hb, tr), (size_t)g.n_pix, lane);
+    }
     if (!hm) return;
     uint32_t inc = chunks;                       // inclusive warp scan of the chunk counts
 #pragma unroll
@@ -270,16 +283,38 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ r
         uint32_t o = base + inc - chunks;
         for (uint32_t lo = s; lo < s + cnt; lo += WS_CHUNK) items[o++] = make_uint4(b, lo, min(lo + WS_CHUNK, s + cnt), 0u);
     }
-    if (mode != WS_GRID_ACCUMULATE) {
-        for (unsigned m = hm; m; m &= m - 1) {
-            const uint32_t hb = (b - lane) + (__ffs(m) - 1);
-            if (mode == WS_GRID_SPARSE_ADD) {                   // a tile earlier chunks filled is added to, not cleared
-                const uint32_t nt = (uint32_t)g.nt, tx = hb % nt, r = hb / nt;
-                if (ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx)) continue;
+}
+
+// Ring scheme: adds the whole shared buffer -- the 32 x 32 tile AND its ring, which holds what this tile's records put onto
+// the neighbours' cells -- to the mesh with red.global.add.v2.f32 (PAPER.md:191 names the accumulation as the bottleneck;
+// here the atomics are confined to this one flush per tile, and only the ring's share of it ever meets another writer).
+// Every target tile was cleared (or filled by an earlier chunk) before this kernel started.  Cells off the mesh cannot
+// hold anything (drop rule) and are skipped, like zeros.
+template <int S>
+__device__ __forceinline__ void flush_ring(const WsGeom& g, const WarpSmem<S>& sm, float2* __restrict__ grid, uint32_t bin, bool tr,
+                                           int lane) {
+    using C = TileCfg<S>;
+    const uint32_t nt = (uint32_t)g.nt, tx = bin % nt, r = bin / nt, ty = r % nt, k = r / nt;
+    const int N = g.n_pix, half = N >> 1;
+    const int gx0 = (int)tx * T - C::H, gy0 = (int)ty * T - C::H;     // logical cell of buffer cell (0, 0)
+    float2* const plane = grid + (size_t)k * N * N;
+    // lanes run along the storage line: x (rows of the plane are v) or, transposed, y
+    const int l0 = tr ? gx0 : gy0, c0 = tr ? gy0 : gx0;               // logical coordinate of buffer line 0 / of lane 0's cell
+    for (int line = 0; line < C::ROWS; ++line) {
+        const int gl = l0 + line;
+        if ((unsigned)gl >= (unsigned)N) continue;
+        float2* const row = plane + (size_t)((gl + half) & (N - 1)) * N;
+#pragma unroll
+        for (int seg = 0; seg < C::ROWS; seg += 32) {
+            const int i = seg + lane;
+            if (i < C::ROWS) {
+                const float2 v = tr ? sm.tile[i * C::P + line] : sm.tile[line * C::P + i];
+                const int gc = c0 + i;
+                if ((v.x != 0.f || v.y != 0.f) && (unsigned)gc < (unsigned)N) atomicAdd(row + ((gc + half) & (N - 1)), v);
             }
-            store_zero_tile(tile_origin(g, grid, hb, tr), (size_t)g.n_pix, lane);
         }
     }
+    __syncwarp();
 }
 
 // Persistent kernel, one CTA per SM: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
@@ -288,7 +323,7 @@ __global__ void __launch_bounds__(TileCfg<S>::THREADS, 1)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint32_t* __restrict__ bin_start,
        const uint4* __restrict__ items,
        const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
-       const uint32_t* __restrict__ orient, const WsMaskView mv) {
+       const uint32_t* __restrict__ orient, const WsMaskView mv, int ring) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -311,6 +346,10 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         float2* out = tile_origin(g, grid, w.x, tr);
         zero_tile<S>(sm.tile, lane);
         accumulate_bin<S, KB>(g, records, w.y, w.z, rec_start[w.x] + (bin_start[w.x + 1] - bin_start[w.x]), sm, lane);
+        if (ring) {
+            flush_ring<S>(g, sm, grid, w.x, tr, lane);
+            return;
+        }
 #pragma unroll 4
         for (int y = 0; y < T; ++y) {
             const float2 v = tr ? inner[lane * C::P + y] : inner[y * C::P + lane];
@@ -334,6 +373,10 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
         }
         zero_tile<S>(sm.tile, lane);
         accumulate_bin<S, KB>(g, records, s, e, s + (bin_start[bin + 1] - bin_start[bin]), sm, lane);
+        if (ring) {
+            flush_ring<S>(g, sm, grid, bin, tr, lane);
+            continue;
+        }
         bool add = mode == WS_GRID_ACCUMULATE;
         if (mode == WS_GRID_SPARSE_ADD) {                       // warp-uniform: did an earlier chunk fill this tile?
             const uint32_t nt = (uint32_t)g.nt, tx = bin % nt, r = bin / nt;
@@ -363,15 +406,20 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     const size_t smem = C::WARP_BYTES * C::WARPS;
     // per device, and cheap: set on every launch rather than cached in a process-wide flag
     if (cudaFuncSetAttribute(k_grid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return WS_ERR_CUDA;
-    const uint32_t* rec_start = (const uint32_t*)(ws + L.off_rec_start);
+    // ring scheme (bins of ws_bin_visibilities_for a sparse mode): the record lists hold home records only, indexed by
+    // bin_start; rec_start = home + halo counts then only says which tiles receive anything
+    const int ring = plan->last_ring ? 1 : 0;
+    const uint32_t* occ_start = (const uint32_t*)(ws + L.off_rec_start);
+    const uint32_t* rec_start = ring ? (const uint32_t*)(ws + L.off_counts_home) : occ_start;
     const float4* records = (const float4*)(ws + L.off_records);
     WsStatus* status = plan->d_status;
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, items, L.item_capacity, status, grid, mode, orient, mv);
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, occ_start, ring, items, L.item_capacity, status, grid, mode,
+                                                          orient, mv);
     k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, rec_start, (const uint32_t*)(ws + L.off_counts_home), items, records,
-                                                                 grid, mode, status, orient, mv);
+                                                                 grid, mode, status, orient, mv, ring);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }
@@ -382,7 +430,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st) {
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&plan->d_status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, items, item_capacity, plan->d_status, nullptr,
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, items, item_capacity, plan->d_status, nullptr,
                                                           WS_GRID_ACCUMULATE, nullptr, WsMaskView{nullptr, 0u, 1});
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;

@@ -107,6 +107,8 @@ struct ws_plan {
     int64_t snapshot_rows;                      // ws_plan_set_snapshot_rows hint (0: none)
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
     int32_t last_chan_per_key;                  // visibilities per binned entry: 1, or n_chan after a pre-summed call
+    bool bin_ring;                              // the binning call in progress stores home records only (ring scheme, sparse modes)
+    bool last_ring;                             // ... and so did the last one: ws_grid_binned must spread the rings
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
     cudaStream_t copy_stream;                   // ws_image_from_host: the H2D copies of the next chunk run beside the gridding
     cudaEvent_t ev_start, ev_chunk[WS_E2E_MAX_CHUNKS];    // of this one (created on first use)
