@@ -361,8 +361,7 @@ def main():
         if chunks:
             return step_chunked(ev)
         if ev: ev[0].record()
-        # (bins for the mode that follows: the sparse modes store home records only and spread each tile's ring)
-        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else ws.WS_GRID_OVERWRITE)
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
         if ev: ev[1].record()
         if own:     # the mesh is neither cleared nor completely written: the FFT passes skip what stayed empty
             plan.grid_binned(grid, wsp, mode=ws.WS_GRID_SPARSE)
@@ -384,9 +383,9 @@ def main():
     bins_info = None
     if chunks:      # statistics of the first chunk stand for all (same recipe per chunk)
         lo0, hi0 = chunks[0]
-        plan.bin_visibilities(d.uvw[lo0:hi0], d.vis[lo0:hi0], d.weights[lo0:hi0], d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else None)
+        plan.bin_visibilities(d.uvw[lo0:hi0], d.vis[lo0:hi0], d.weights[lo0:hi0], d.freqs_hz, wsp)
     else:
-        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE if own else None)
+        plan.bin_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, wsp)
     b = plan.get_bins(fields=("bin_start",))
     bins_info = {"n_dropped": b["n_dropped"], "n_records": b["n_records"],
                  "max_bin": int(np.diff(b["bin_start"].astype(np.int64)).max()),

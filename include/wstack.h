@@ -50,7 +50,7 @@ extern "C" {
 #define WS_OK 0
 #define WS_ERR_INVALID_ARG (-1)
 #define WS_ERR_UNSUPPORTED (-2)
-#define WS_ERR_WORKSPACE (-3)   /* workspace too small / record capacity exceeded */
+#define WS_ERR_WORKSPACE (-3)   /* workspace too small */
 #define WS_ERR_CUDA (-4)
 #define WS_ERR_CUFFT (-5)
 
@@ -155,12 +155,12 @@ int ws_plan_set_plane_range(ws_plan* plan, int32_t plane_lo, int32_t plane_hi);
 size_t ws_grid_bytes(const ws_plan* plan);   /* 8 N^2 N_w */
 size_t ws_image_bytes(const ws_plan* plan);  /* 8 N^2     */
 size_t ws_dirty_bytes(const ws_plan* plan);  /* 4 N^2     */
-/* Workspace that is always enough for ws_grid_visibilities with up to max_vis_per_call visibilities
- * (worst-case halo duplication) and for ws_fft_planes.  A smaller workspace may be passed: the record
- * capacity is then what fits, and exceeding it is reported by ws_async_status as WS_ERR_WORKSPACE. */
+/* Workspace that is enough for ws_grid_visibilities with up to max_vis_per_call visibilities (keys, perm, one 16-byte
+ * record per visibility, the per-tile offset arrays) and for ws_fft_planes.  A workspace that cannot hold a call's
+ * visibilities is refused by that call (WS_ERR_WORKSPACE). */
 size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis_per_call);   /* WS_FLAG_PRESUM_CHANNELS: count ROWS */
-/* The least workspace ws_grid_visibilities accepts for max_vis_per_call visibilities when at most
- * `dup_factor` records per visibility are stored (1.0 .. 4.0; typical data needs (1 + (S-1)/T)^2). */
+/* The same (dup_factor is ignored: round 1 stored a copy of a record in every tile its footprint reaches and sized the
+ * workspace by that factor; since round 2 there is one record per visibility). */
 size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis_per_call, double dup_factor);
 size_t ws_fft_workspace_bytes(const ws_plan* plan);
 int ws_plan_tile(const ws_plan* plan);       /* T */
@@ -179,7 +179,10 @@ int ws_grid_zero(ws_plan* plan, void* grid, void* stream);
  * plane k = clamp(floor(fma(w, sw_c, ow))), dropped unless the S x S footprint lies on the mesh;
  * key = (k nt + j0/T) nt + i0/T, nt = N/T.  Contribution: weight * vis * g(a - fu) g(b - fv) at logical
  * cell (k, j0 + b, i0 + a), |a|,|b| <= (S-1)/2, fp32.  n_rows * n_chan <= 2^30, n_chan <= 128.
- * Non-finite uvw is a caller error (undefined).  mode: WS_GRID_ACCUMULATE or WS_GRID_OVERWRITE. */
+ * A visibility with a NaN coordinate is dropped (R33).  mode: one of WS_GRID_*.
+ * Every tile of the mesh is accumulated by one warp in shared memory together with a ring of (S-1)/2 cells and added to
+ * the mesh once (red.global.add: the ring is the only place where two writers meet); the tiles that receive anything
+ * are cleared first, except in WS_GRID_ACCUMULATE mode and for tiles earlier WS_GRID_SPARSE(_ADD) chunks filled. */
 int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
                          const double* freq_hz, int64_t n_rows, int32_t n_chan, void* grid, int32_t mode,
                          void* workspace, size_t workspace_bytes, void* stream);
@@ -190,15 +193,6 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
                         const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace,
                         size_t workspace_bytes, void* stream);
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream);
-/* a1 for a known gridding mode (what ws_grid_visibilities calls).  For WS_GRID_SPARSE / WS_GRID_SPARSE_ADD only the HOME record of
- * every visibility is stored -- no copies in the neighbour tiles its footprint reaches: ws_grid_binned then accumulates each tile
- * together with a ring of (S-1)/2 cells and adds the ring onto the neighbours' cells (red.global.add, "atomics only at tile
- * borders"), 29 % fewer records on Large, 36 % on Extreme (S = 9).  Such bins serve the two sparse modes only (else
- * WS_ERR_INVALID_ARG from ws_grid_binned); keys, bin_start and perm are the same either way, n_records = the kept visibilities.
- * For the other modes (and where the own FFT does not exist) it is ws_bin_visibilities. */
-int ws_bin_visibilities_for(ws_plan* plan, int32_t mode, const float* uvw, const void* vis, const float* weights,
-                            const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes,
-                            void* stream);
 
 /* ---- a3: per-plane un-normalised inverse 2-D FFT, in place -------------------------- */
 /* P_k[q][p] = sum_ji G_k[j][i] exp(+2 pi i ((i-N/2)(p-N/2) + (j-N/2)(q-N/2)) / N) in logical indices. */

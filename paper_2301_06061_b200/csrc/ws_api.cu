@@ -50,7 +50,6 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity, 
     L.off_counts_halo = take((nb + 1) * 4);
     L.off_rec_start = take((nb + 1) * 4);
     L.off_cursor_home = take(nb * 4);
-    L.off_cursor_halo = take(nb * 4);
     L.off_block_sums = take(2 * ((nb + 1) / 4096 + 2) * 4);
     L.off_keys = take((size_t)n_vis * 4);
     L.off_perm = take((size_t)n_vis * 4);
@@ -65,10 +64,10 @@ WsLayout make_layout(const ws_plan* plan, int64_t n_vis, uint64_t rec_capacity, 
 }
 
 // Largest record capacity whose layout fits into `bytes` (0 if even the fixed part does not fit).
-bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out, int64_t presum_rows = 0, int max_dup = 4) {
+bool fit_layout(const ws_plan* plan, int64_t n_vis, size_t bytes, WsLayout* out, int64_t presum_rows = 0) {
     WsLayout L0 = make_layout(plan, n_vis, 0, presum_rows);
     if (L0.total > bytes) return false;
-    const uint64_t want = (uint64_t)n_vis * (uint64_t)max_dup;      // worst case: every footprint in 4 tiles (home lists only: 1)
+    const uint64_t want = (uint64_t)n_vis;                          // one record per visibility
     const size_t spare = bytes - L0.total;
     // per record: 16 B + 32/WS_CHUNK B of items; keep a page of slack for the alignment of the two regions
     uint64_t cap = spare > 1024 ? (uint64_t)((spare - 1024) / (16.0 + 32.0 / WS_CHUNK)) : 0;
@@ -223,8 +222,6 @@ int ws_plan_create(const ws_params* p, ws_plan** out) {
     plan->last_weights = nullptr;
     plan->snapshot_rows = 0;
     plan->last_has_values = false;
-    plan->bin_ring = false;
-    plan->last_ring = false;
     plan->last_chan_per_key = 1;
     plan->launches = 0;
     plan->last_valid = false;
@@ -356,16 +353,15 @@ int64_t ws_plan_n_bins(const ws_plan* plan) { return plan ? (int64_t)plan->geom.
 
 size_t ws_workspace_bytes_for(const ws_plan* plan, int64_t max_vis, double dup_factor) {
     if (!plan || max_vis < 0 || max_vis > MAX_VIS) return 0;
-    if (!(dup_factor >= 1.0)) dup_factor = 1.0;
-    if (dup_factor > 4.0) dup_factor = 4.0;
-    const uint64_t cap = (uint64_t)std::ceil((double)max_vis * dup_factor) + 64;
+    (void)dup_factor;      // one record per visibility since round 2 (the gridder carries a ring instead of copies)
+    const uint64_t cap = (uint64_t)max_vis + 64;
     const bool presum = (plan->prm.flags & WS_FLAG_PRESUM_CHANNELS) != 0;          // sized for n_chan = 1, the worst case
     const size_t a = make_layout(plan, max_vis, cap, presum ? max_vis : 0).total + 4096 +   // slack for fit_layout's alignment margin
                      ws_align_up(plan->fft_rows1d_work, 256) + 256;                         // ws_predict_visibilities' row transforms
     return a > plan->fft_work_bytes ? a : plan->fft_work_bytes;
 }
 
-size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis) { return ws_workspace_bytes_for(plan, max_vis, 4.0); }
+size_t ws_workspace_bytes(const ws_plan* plan, int64_t max_vis) { return ws_workspace_bytes_for(plan, max_vis, 1.0); }
 
 int ws_grid_zero(ws_plan* plan, void* grid, void* stream) {
     const DeviceGuard device_guard(plan);
@@ -401,10 +397,8 @@ static int make_chan_consts(ws_plan* plan, const double* freq_hz, int32_t n_chan
 }
 
 // a1 for the gridder (with_values) and for the degridder (positions only: vis and weights are not read)
-// ring: only the home records are stored (the sparse gridding modes spread each tile's ring onto its neighbours)
 static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const float* weights, const double* freq_hz,
-                    int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values,
-                    bool ring = false) {
+                    int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes, void* stream, bool with_values) {
     if (!plan) return WS_ERR_INVALID_ARG;
     if (is_f64(plan)) return fail(plan, WS_ERR_UNSUPPORTED, "WS_FLAG_MESH_F64: nothing is binned (ws_grid_visibilities grids directly); no degridding");
     if (n_rows < 0 || n_chan <= 0) return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities: bad n_rows / n_chan");
@@ -423,8 +417,7 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
     const int64_t n_vis = presum ? n_rows : n_rows * n_chan;
     const int32_t n_chan_in = n_chan;
     WsLayout L;
-    // positions only (degridding): home records alone, so that the rest of the workspace stays free for the caller's use
-    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0, with_values && !ring ? 4 : 1) ||
+    if (!fit_layout(plan, n_vis, workspace_bytes, &L, presum ? n_rows : 0) ||
         (n_vis > 0 && L.rec_capacity < (uint64_t)n_vis))
         return fail(plan, WS_ERR_WORKSPACE, "ws_bin_visibilities: workspace too small (see ws_workspace_bytes_for)");
     const void* vis_in = vis;
@@ -445,11 +438,8 @@ static int bin_impl(ws_plan* plan, const float* uvw, const void* vis, const floa
 
     plan->last_valid = false;
     plan->sorted_keys_valid = false;
-    plan->bin_ring = with_values && ring;
     const int rc = ws_launch_bin(plan, L, (char*)workspace, cc, uvw, (const float2*)vis_in, wt_in, n_rows, n_chan,
                                  (cudaStream_t)stream);
-    plan->last_ring = plan->bin_ring;
-    plan->bin_ring = false;
     if (rc < 0) return fail(plan, rc, "ws_bin_visibilities: launch failed");
     plan->launches += rc;
     plan->last_ws = workspace;
@@ -469,17 +459,6 @@ int ws_bin_visibilities(ws_plan* plan, const float* uvw, const void* vis, const 
     return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true);
 }
 
-int ws_bin_visibilities_for(ws_plan* plan, int32_t mode, const float* uvw, const void* vis, const float* weights,
-                            const double* freq_hz, int64_t n_rows, int32_t n_chan, void* workspace, size_t workspace_bytes,
-                            void* stream) {
-    const DeviceGuard device_guard(plan);
-    if (!plan) return WS_ERR_INVALID_ARG;
-    if (mode != WS_GRID_ACCUMULATE && mode != WS_GRID_OVERWRITE && mode != WS_GRID_SPARSE && mode != WS_GRID_SPARSE_ADD)
-        return fail(plan, WS_ERR_INVALID_ARG, "ws_bin_visibilities_for: bad mode");
-    const bool ring = (mode == WS_GRID_SPARSE || mode == WS_GRID_SPARSE_ADD) && plan->fft_own;
-    return bin_impl(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream, true, ring);
-}
-
 int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, size_t workspace_bytes, void* stream) {
     const DeviceGuard device_guard(plan);
     if (!plan) return WS_ERR_INVALID_ARG;
@@ -496,8 +475,6 @@ int ws_grid_binned(ws_plan* plan, void* grid, int32_t mode, void* workspace, siz
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: cannot accumulate onto a WS_GRID_SPARSE mesh (its empty tiles were never written): use WS_GRID_SPARSE_ADD");
     if (mode == WS_GRID_SPARSE_ADD && !(plan->occ_sparse && plan->occ_grid == grid))
         return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: WS_GRID_SPARSE_ADD needs a mesh this plan wrote with WS_GRID_SPARSE");
-    if (plan->last_ring && !sparse_mode)
-        return fail(plan, WS_ERR_INVALID_ARG, "ws_grid_binned: these bins hold home records only (ws_bin_visibilities_for a sparse mode)");
     cudaStream_t st = (cudaStream_t)stream;
     // Tile occupancy of the mesh, for the sparse FFT passes: restarted by OVERWRITE / SPARSE, OR-ed by ACCUMULATE /
     // SPARSE_ADD.  It comes BEFORE the gridding kernel -- a SPARSE mesh is stored in the orientation the masks favour --
@@ -571,7 +548,7 @@ int ws_grid_visibilities(ws_plan* plan, const float* uvw, const void* vis, const
         plan->launches += rc;
         return WS_OK;
     }
-    const int rc = ws_bin_visibilities_for(plan, mode, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
+    const int rc = ws_bin_visibilities(plan, uvw, vis, weights, freq_hz, n_rows, n_chan, workspace, workspace_bytes, stream);
     if (rc != WS_OK) return rc;
     return ws_grid_binned(plan, grid, mode, workspace, workspace_bytes, stream);
 }

@@ -2,8 +2,9 @@
 // visibilities), :144-150 (bucketing then gather into contiguous arrays).  The paper builds linked lists on the
 // CPU; here it is a one-digit counting sort on the device (the whole key is the digit; the order INSIDE a bin is
 // unspecified, R19): histogram over all bins, exclusive prefix scan (warp shuffles), and a scatter that
-// writes, per bin, contiguous 16-byte records the gridder streams.  A visibility whose S x S footprint crosses a tile border is written into every tile
-// it touches (up to 4), so that each tile-plane of the mesh is produced by exactly one warp (ws_grid.cu).
+// writes, per bin, contiguous 16-byte records the gridder streams: one record per visibility, in the bin of the tile
+// that holds its centre cell.  (Round 1 copied a record into every tile its footprint reaches; the gridder now carries a
+// ring around each tile instead, ws_grid.cu.)
 #include <stddef.h>
 
 #include <algorithm>
@@ -95,8 +96,8 @@ k_keys_hist(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsG
         // tiles the footprint overlaps: own, and the neighbour on each side it sticks out of
         dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
         dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-        if (home_only == 1) dx = dy = 0;          // bins for the degridder: a gather needs no copies in neighbour tiles
-                                                  // (2: the ring scheme of the gridder counts the halo -- occupancy -- but stores no copies)
+        if (home_only) dx = dy = 0;               // bins for the degridder: a gather reaches nothing outside its staged region
+                                                  // (the gridder needs the halo counts: which tiles receive anything)
     }
     if (m < n_vis) keys[m] = home;
     // two histograms: visibilities per home bin (-> bin_start) and halo copies received per bin; the record
@@ -191,38 +192,37 @@ k_scan_apply(uint32_t* __restrict__ a0, uint32_t* __restrict__ a1, uint32_t n, c
     }
 }
 
-// rec_start = bin_start + halo_start; cursors: home slots start at bin_start[b] (perm), halo records of bin b
-// start after its home records, at rec_start[b] + count_home[b]; totals and the capacity check.
+// rec_start = bin_start + halo_start (home + halo counts, scanned: rec_start[b + 1] > rec_start[b] <=> tile b receives
+// something from its own visibilities or from a neighbour's footprints); slot cursors start at bin_start[b]; totals
+// and the capacity check.
 __global__ void __launch_bounds__(256)
 k_finish_offsets(const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
-                 uint32_t* __restrict__ rec_start, uint32_t* __restrict__ cursor_home, uint32_t* __restrict__ cursor_halo,
-                 uint32_t n_bins, WsStatus* __restrict__ status, uint64_t rec_capacity, int home_only) {
+                 uint32_t* __restrict__ rec_start, uint32_t* __restrict__ cursor_home,
+                 uint32_t n_bins, WsStatus* __restrict__ status, uint64_t rec_capacity) {
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
     if (b > n_bins) return;
     const uint32_t bs = bin_start[b], hs = halo_start[b];
     rec_start[b] = bs + hs;
     if (b < n_bins) {
         cursor_home[b] = bs;
-        cursor_halo[b] = bin_start[b + 1] + hs;
     } else {
-        const uint64_t n_rec = home_only == 2 ? (uint64_t)bs : (uint64_t)bs + (uint64_t)hs;   // (2: only home records are stored)
         status->n_kept = bs;
-        status->n_records = (uint32_t)n_rec;
-        if (n_rec > rec_capacity) status->overflow = status->sticky_overflow = 1u;
+        status->n_records = bs;                         // one record per kept visibility, in its home bin
+        if ((uint64_t)bs > rec_capacity) status->overflow = status->sticky_overflow = 1u;
     }
 }
 
 // ---- pass B: scatter into per-bin record lists ----------------------------------------------------------
-// Record (16 B): X, Y = position relative to the RECEIVING tile: signed 8-bit integer part = centre cell minus
-// tile origin (i0 - tile_x0, in [-h, T-1+h]) in the top byte, 24-bit fraction of fu + 1/2 below it; then
-// weight * norm * vis (re, im).
+// One record (16 B) per kept visibility, in the list of its HOME bin (the tile that holds its centre cell): X, Y = centre
+// cell minus tile origin (0 .. T-1) in the top byte, 24-bit fraction of fu + 1/2 below it; then weight * norm * vis
+// (re, im).  The record slot is the perm slot: the lists are indexed by bin_start.  What a footprint puts onto neighbour
+// tiles is the gridder's business (it accumulates every tile with a ring, ws_grid.cu); the halo HISTOGRAM of pass A only
+// tells which tiles receive anything.
 __global__ void __launch_bounds__(256)
 k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeom g,
           const float* __restrict__ uvw, const float2* __restrict__ vis, const float* __restrict__ wt,
-          uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home,
-          uint32_t* __restrict__ cursor_halo, const uint32_t* __restrict__ halo_start, uint32_t* __restrict__ perm,
-          float4* __restrict__ records, const WsStatus* __restrict__ status, int home_only,
-          const __grid_constant__ WsRemap rm) {
+          uint32_t n_vis, uint32_t n_chan, int chan_shift, uint32_t* __restrict__ cursor_home, uint32_t* __restrict__ perm,
+          float4* __restrict__ records, const WsStatus* __restrict__ status, const __grid_constant__ WsRemap rm) {
     if (status->overflow) return;
     __shared__ double s_su[WS_MAX_CHAN], s_sw[WS_MAX_CHAN];
     stage_consts(cc, n_chan, s_su, s_sw);
@@ -236,8 +236,8 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         const float* p = uvw + 3ull * row;
         kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), s_su[c], s_sw[c], pl);
     }
-    uint32_t home = 0xFFFFFFFFu, hs = 0;
-    int tx = 0, ty = 0, lx = 0, ly = 0, dx = 0, dy = 0, k = 0;
+    uint32_t home = 0xFFFFFFFFu;
+    int lx = 0, ly = 0;
     float2 v = make_float2(0.f, 0.f);
     float w = 0.f;
     if (kept) {
@@ -245,23 +245,13 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
             v = __ldcs(vis + m);
             w = wt ? __ldcs(wt + m) : 1.0f;         // NULL: pre-summed rows, the weights are already inside
         }
-        tx = pl.i0 >> T_LOG2; ty = pl.j0 >> T_LOG2; k = pl.k;
         lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
-        home = bin_of(g, k, ty, tx);
-        hs = __ldg(halo_start + home);
-        dx = lx < g.halo ? -1 : (lx >= T - g.halo ? 1 : 0);
-        dy = ly < g.halo ? -1 : (ly >= T - g.halo ? 1 : 0);
-        if (home_only) dx = dy = 0;               // (1: degridder; 2: ring scheme -- no copies in neighbour tiles either way)
+        home = bin_of(g, pl.k, pl.j0 >> T_LOG2, pl.i0 >> T_LOG2);
     }
-    // slots: every group leader issues its atomics back to back, the results are broadcast afterwards.  The home
-    // copy needs no second atomic: its record slot is its perm slot shifted by the bin's halo_start.
-    const Groups q = warp_groups(home, dx, dy);
-    uint32_t bh = 0, bx = 0, by = 0, bc = 0;
-    if (kept && leads(q.home, lane)) bh = atomicAdd(cursor_home + home, (uint32_t)__popc(q.home));
-    if (leads(q.nx, lane)) bx = atomicAdd(cursor_halo + bin_of(g, k, ty, tx + dx), (uint32_t)__popc(q.nx));
-    if (leads(q.ny, lane)) by = atomicAdd(cursor_halo + bin_of(g, k, ty + dy, tx), (uint32_t)__popc(q.ny));
-    if (leads(q.nc, lane)) bc = atomicAdd(cursor_halo + bin_of(g, k, ty + dy, tx + dx), (uint32_t)__popc(q.nc));
-
+    // slots: one atomic per group of lanes that share the bin, the result broadcast by shuffle
+    const unsigned peers = __match_any_sync(0xffffffffu, home);
+    uint32_t bh = 0;
+    if (kept && leads(peers, lane)) bh = atomicAdd(cursor_home + home, (uint32_t)__popc(peers));
     uint32_t qx = 0, qy = 0;
     float vr = 0.f, vi = 0.f;
     if (kept) {
@@ -272,22 +262,10 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
         qy = qy > 0xFFFFFFu ? 0xFFFFFFu : qy;
         vr = v.x * wn; vi = v.y * wn;
     }
-    bh = __shfl_sync(0xffffffffu, bh, __ffs(q.home) - 1) + rank_in(q.home, lane);
-    bx = __shfl_sync(0xffffffffu, bx, q.nx ? __ffs(q.nx) - 1 : lane) + rank_in(q.nx, lane);
-    by = __shfl_sync(0xffffffffu, by, q.ny ? __ffs(q.ny) - 1 : lane) + rank_in(q.ny, lane);
-    bc = __shfl_sync(0xffffffffu, bc, q.nc ? __ffs(q.nc) - 1 : lane) + rank_in(q.nc, lane);
+    bh = __shfl_sync(0xffffffffu, bh, __ffs(peers) - 1) + rank_in(peers, lane);
     if (!kept) return;
-    // centre cell relative to the receiving tile's origin: lx - ddx*T (negative wraps into the signed byte)
-    auto emit = [&](uint32_t slot, int ddx, int ddy) {
-        const uint32_t X = ((uint32_t)(lx - ddx * T) << 24) | qx;
-        const uint32_t Y = ((uint32_t)(ly - ddy * T) << 24) | qy;
-        records[slot] = make_float4(__uint_as_float(X), __uint_as_float(Y), vr, vi);
-    };
     perm[bh] = m;
-    emit(home_only == 2 ? bh : bh + hs, 0, 0);      // (ring scheme: the record lists hold home records only, indexed by bin_start)
-    if (q.nx) emit(bx, dx, 0);
-    if (q.ny) emit(by, 0, dy);
-    if (q.nc) emit(bc, dx, dy);
+    records[bh] = make_float4(__uint_as_float(((uint32_t)lx << 24) | qx), __uint_as_float(((uint32_t)ly << 24) | qy), vr, vi);
 }
 
 // ---- parity export: sorted_keys[] expanded from bin_start (run lengths) ---------------------------------
@@ -366,7 +344,7 @@ int ws_launch_sum_weights(ws_plan* plan, const WsLayout& L, char* ws, const floa
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st) {
     const WsGeom& g = plan->geom;
-    const int home_only = vis == nullptr ? 1 : (plan->bin_ring ? 2 : 0);   // 1: positions only (degridder); 2: home records only (ring scheme)
+    const int home_only = vis == nullptr;          // positions only: the degridder's gather (no halo histogram)
     WsRemap rm = {0u, 0u, 0u, 0u, 0u};
     if (plan->snapshot_rows > 0 && n_rows >= 2 * plan->snapshot_rows) {
         const uint64_t F = (uint64_t)plan->snapshot_rows * (uint64_t)n_chan;
@@ -384,7 +362,6 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     uint32_t* counts_halo = (uint32_t*)(ws + L.off_counts_halo);   // -> halo_start
     uint32_t* rec_start = (uint32_t*)(ws + L.off_rec_start);
     uint32_t* cursor_home = (uint32_t*)(ws + L.off_cursor_home);
-    uint32_t* cursor_halo = (uint32_t*)(ws + L.off_cursor_halo);
     uint32_t* block_sums = (uint32_t*)(ws + L.off_block_sums);
     WsStatus* status = plan->d_status;
     uint32_t* keys = (uint32_t*)(ws + L.off_keys);
@@ -409,12 +386,12 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
     k_scan_reduce<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
     k_scan_block_sums<<<dim3(1, 2), SCAN_THREADS, 0, st>>>(block_sums, n_blocks);
     k_scan_apply<<<dim3(n_blocks, 2), SCAN_THREADS, 0, st>>>(counts_home, counts_halo, n_scan, block_sums, n_blocks);
-    k_finish_offsets<<<(n_scan + 255) / 256, 256, 0, st>>>(counts_home, counts_halo, rec_start, cursor_home, cursor_halo,
-                                                          g.n_bins, status, L.rec_capacity, home_only);
+    k_finish_offsets<<<(n_scan + 255) / 256, 256, 0, st>>>(counts_home, counts_halo, rec_start, cursor_home,
+                                                          g.n_bins, status, L.rec_capacity);
     launches += 4;
     if (n_vis) {
         k_scatter<<<(n_vis + 255) / 256, 256, 0, st>>>(cc, g, uvw, vis, wt, n_vis, (uint32_t)n_chan, chan_shift,
-                                                       cursor_home, cursor_halo, counts_halo, perm, records, status, home_only, rm);
+                                                       cursor_home, perm, records, status, rm);
         ++launches;
     }
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;

@@ -4,19 +4,26 @@
 // The paper's GPU kernel gives one thread per measurement and resolves collisions with atomicAdd on the fp64
 // mesh in global memory, and names the accumulation as "the main potential bottleneck"
 // (:191).  Here the bins of ws_bin.cu make the mesh output-stationary instead:
-//   * one WARP owns one 32 x 32 tile of one w-plane, accumulates it in its private shared-memory tile with
-//     plain LDS / FFMA / STS (the lanes of a warp cover distinct taps of one visibility, so there are no
-//     collisions and no atomics), and writes it ONCE with coalesced stores -- in WS_GRID_OVERWRITE mode the
-//     tile (zeros included) is simply stored, so the mesh needs no memset and no read-modify-write;
+//   * one WARP owns one 32 x 32 tile of one w-plane and accumulates the records of the visibilities whose centre
+//     cell lies in it in a private shared-memory buffer -- the tile plus a ring of (S-1)/2 cells, so that no
+//     footprint leaves the buffer -- with plain LDS / FFMA / STS (the lanes of a warp cover distinct taps of one
+//     visibility: no collisions, no atomics, no bounds tests);
 //   * taps are evaluated in registers, 32 visibilities at a time (lane r evaluates the 2 S taps of record r
 //     -- Gaussian: ex2.approx; Kaiser-Bessel: the power series of I0 by Horner's rule, all 2 S
 //     taps side by side -- and parks them in shared memory), then lane (a, b) of the warp applies tap (a, b) of
 //     one record after the other;
+//   * the buffer is then ADDED to the mesh once, tile and ring alike (red.global.add.v2.f32, skipping zeros): the
+//     ring is what this tile's visibilities put onto the neighbours' cells, and it is the only place where two
+//     writers can meet ("atomics only at tile borders").  The tiles that receive anything -- from their own
+//     records or from a neighbour's ring: the halo histogram of ws_bin.cu knows -- are cleared first by
+//     k_prepare_heavy (WS_GRID_SPARSE_ADD: unless an earlier chunk filled them; WS_GRID_ACCUMULATE: never);
+//     WS_GRID_OVERWRITE also stores the zeros of the tiles that receive nothing, from inside the persistent kernel,
+//     so that their store stream overlaps the arithmetic of the dense tiles.  (Round 1 copied a record into every
+//     tile its footprint reaches and let one owner store each tile: 1.41 records per visibility on Large, 1.56
+//     with S = 9.)
 //   * a bin with more than WS_CHUNK records ("heavy": the dense core of the uv plane) is cut
-//     into chunks that become work items of their own; k_prepare_heavy queues them and clears their tiles,
-//     and the chunks are added with vector red.global.add.f32x2.  Tiles and items are interleaved in ONE
-//     persistent kernel so that the store stream of the (mostly empty) tiles overlaps the arithmetic of the
-//     dense ones.
+//     into chunks that become work items of their own (k_prepare_heavy), interleaved with the tiles in ONE
+//     persistent kernel.
 #include "ws_internal.h"
 #include "ws_taps.cuh"
 
@@ -157,31 +164,19 @@ __device__ __forceinline__ void park_taps(const WsGeom& g, float fx, float fy, c
     }
 }
 
-// One record of the batch onto the tile: lane (a, br) applies its taps.  HOME: the record's centre cell lies inside the
-// tile, so its footprint stays inside the buffer (tile + ring): no bounds tests.  Otherwise (the copy of a neighbour's
-// record, centre in the ring) each tap is tested against the buffer.
-template <int S, bool HOME>
-__device__ __forceinline__ void apply_record(const WarpSmem<S>& sm, int r, int a, int br, const bool* okb, unsigned char* tile_b,
+// One record of the batch onto the buffer: lane (a, br) applies its taps.  The record's centre cell lies inside the tile,
+// so its footprint stays inside the buffer (tile + ring): no bounds tests.
+template <int S>
+__device__ __forceinline__ void apply_record(const WarpSmem<S>& sm, int r, const bool* okb, unsigned char* tile_b,
                                              const float* gu_l, const float* gv_l) {
     using C = TileCfg<S>;
     const float4 m = sm.meta[r];                       // broadcast
     const float u = gu_l[r * C::SP];
     const TapVec<C::NRP> gvv = load_taps<C::NRP>(gv_l + r * C::GP);
-    float2* const cell0 = (float2*)(tile_b + __float_as_int(m.w));
-    bool ok[C::NR];
-    if constexpr (HOME) {
-#pragma unroll
-        for (int rr = 0; rr < C::NR; ++rr) ok[rr] = okb[rr];
-    } else {
-        const int xy = __float_as_int(m.z);
-        const int cx = (int)(short)(xy & 0xFFFF), cy = xy >> 16;
-        const bool okx = (unsigned)(cx + a) < (unsigned)C::ROWS;
-#pragma unroll
-        for (int rr = 0; rr < C::NR; ++rr) ok[rr] = okb[rr] && okx && (unsigned)(cy + br + rr * C::R) < (unsigned)C::ROWS;
-    }
+    float2* const cell0 = (float2*)(tile_b + __float_as_int(m.z));
 #pragma unroll
     for (int rr = 0; rr < C::NR; ++rr) {
-        if (ok[rr]) {                                   // (distinct cells per round: the loads of all rounds can go first)
+        if (okb[rr]) {                                  // (distinct cells per round: the loads of all rounds can go first)
             float2 c = cell0[rr * C::R * C::P];
             const float t = u * gvv.v[rr];
             c.x = fmaf(m.x, t, c.x);
@@ -192,11 +187,10 @@ __device__ __forceinline__ void apply_record(const WarpSmem<S>& sm, int r, int a
     __syncwarp();
 }
 
-// Accumulates records [lo, hi) of a bin into the warp's shared tile; those before `home_end` are the bin's home records
-// (they come first in its list).
+// Accumulates records [lo, hi) (all of one tile) into the warp's shared buffer.
 template <int S, bool KB>
-__device__ __forceinline__ void accumulate_bin(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
-                                               uint32_t home_end, const WarpSmem<S>& sm, int lane) {
+__device__ __forceinline__ void accumulate_records(const WsGeom& g, const float4* __restrict__ records, uint32_t lo, uint32_t hi,
+                                                   const WarpSmem<S>& sm, int lane) {
     using C = TileCfg<S>;
     const int a = lane % S, br = lane / S;
     const bool active = br < C::R;
@@ -210,20 +204,17 @@ __device__ __forceinline__ void accumulate_bin(const WsGeom& g, const float4* __
     if (lo + lane < hi) nxt = __ldcs(records + lo + lane);
     for (uint32_t base = lo; base < hi; base += 32) {
         const int n = (int)min(32u, hi - base);
-        const int n_home = home_end > base ? (int)min((uint32_t)n, home_end - base) : 0;
         {   // vector phase: lane r prepares record r of the batch
             const uint32_t X = __float_as_uint(nxt.x), Y = __float_as_uint(nxt.y);
-            const int cx = (int)X >> 24, cy = (int)Y >> 24;    // centre cell in the tile's frame = first footprint cell in the buffer's
+            const int cx = (int)(X >> 24), cy = (int)(Y >> 24);   // centre cell in the tile's frame = first footprint cell in the buffer's
             const float fx = (float)(X & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
             const float fy = (float)(Y & 0xFFFFFFu) * (1.0f / 16777216.0f) - 0.5f;
             park_taps<S, KB>(g, fx, fy, sm, lane);
-            sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cx & 0xFFFF) | (cy << 16)),
-                                        __int_as_float((cy * C::P + cx) * (int)sizeof(float2)));
+            sm.meta[lane] = make_float4(nxt.z, nxt.w, __int_as_float((cy * C::P + cx) * (int)sizeof(float2)), 0.f);
         }
         if (base + 32 + lane < hi) nxt = __ldcs(records + base + 32 + lane);   // prefetch the next batch
         __syncwarp();
-        for (int r = 0; r < n_home; ++r) apply_record<S, true>(sm, r, a, br, okb, tile_b, gu_l, gv_l);
-        for (int r = n_home; r < n; ++r) apply_record<S, false>(sm, r, a, br, okb, tile_b, gu_l, gv_l);
+        for (int r = 0; r < n; ++r) apply_record<S>(sm, r, okb, tile_b, gu_l, gv_l);
     }
 }
 
@@ -234,13 +225,13 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
     __syncwarp();
 }
 
-// Queues the chunks of the heavy bins as work items and clears the tiles that will be ADDED to: those of the heavy bins
-// (their chunks are added with red) and, in the ring scheme, every tile that receives anything at all -- its own records or
-// a neighbour's ring (occ_start: home + halo counts).  starts: offsets of the record lists ([n_bins + 1]).  In
-// WS_GRID_SPARSE_ADD mode a tile that earlier chunks filled is left alone; WS_GRID_ACCUMULATE clears nothing.
+// Queues the chunks of the heavy bins (more than WS_CHUNK records) as work items and, for the gridder (clear_occupied),
+// clears every tile that will be ADDED to: every tile that receives anything at all -- its own records or a neighbour's
+// ring (occ_start: home + halo counts).  starts: offsets of the record lists ([n_bins + 1]).  In WS_GRID_SPARSE_ADD mode
+// a tile that earlier chunks filled is left alone; WS_GRID_ACCUMULATE clears nothing.
 __global__ void __launch_bounds__(256)
 k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ starts, const uint32_t* __restrict__ occ_start,
-                int ring, uint4* __restrict__ items, uint32_t item_capacity, WsStatus* __restrict__ status,
+                int clear_occupied, uint4* __restrict__ items, uint32_t item_capacity, WsStatus* __restrict__ status,
                 float2* __restrict__ grid, int mode, const uint32_t* __restrict__ orient, const WsMaskView mv) {
     if (status->overflow) return;
     const bool tr = orient && *orient;
@@ -250,12 +241,12 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ s
     if (b < g.n_bins) {
         s = starts[b];
         cnt = starts[b + 1] - s;
-        occ = ring ? occ_start[b + 1] - occ_start[b] : cnt;
+        occ = clear_occupied ? occ_start[b + 1] - occ_start[b] : 0u;
     }
     const bool heavy = cnt > WS_CHUNK;
     const uint32_t chunks = heavy ? (cnt + WS_CHUNK - 1) / WS_CHUNK : 0u;
     const unsigned hm = __ballot_sync(0xffffffffu, heavy);
-    bool clear = mode != WS_GRID_ACCUMULATE && (ring ? occ > 0 : heavy);
+    bool clear = mode != WS_GRID_ACCUMULATE && occ > 0;
     if (clear && mode == WS_GRID_SPARSE_ADD) {              // a tile earlier chunks filled is added to, not cleared
         const uint32_t nt = (uint32_t)g.nt, tx = b % nt, r = b / nt;
         clear = !ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx);
@@ -318,23 +309,23 @@ __device__ __forceinline__ void flush_ring(const WsGeom& g, const WarpSmem<S>& s
 }
 
 // Persistent kernel, one CTA per SM: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
+// bin_start: offsets of the record lists (one record per visibility, in its home bin); occ_start: home + halo counts,
+// scanned -- a tile whose entry does not grow receives nothing, and WS_GRID_OVERWRITE stores its zeros here (every other
+// tile was cleared by k_prepare_heavy, or holds what earlier calls put there, and is only ever added to).
 template <int S, bool KB>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 1)
-k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start, const uint32_t* __restrict__ bin_start,
-       const uint4* __restrict__ items,
-       const float4* __restrict__ records, float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status,
-       const uint32_t* __restrict__ orient, const WsMaskView mv, int ring) {
+k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ occ_start,
+       const uint4* __restrict__ items, const float4* __restrict__ records, float2* __restrict__ grid, int mode,
+       const WsStatus* __restrict__ status, const uint32_t* __restrict__ orient) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const WarpSmem<S> sm(smem_raw + (size_t)wid * C::WARP_BYTES);
-    const float2* const inner = sm.tile + C::H * C::P + C::H;     // cell (0, 0) of the tile proper, inside the ring
     if (status->overflow) return;
-    const bool tr = orient && *orient;          // transposed planes: lane = row of the tile, one tile column per store
+    const bool tr = orient && *orient;          // transposed planes: lanes run along v instead of u
     const uint32_t n_items = status->n_items;
     const uint32_t n_warps = gridDim.x * C::WARPS;
     const uint32_t gw = blockIdx.x * C::WARPS + wid;
-    const size_t N = (size_t)g.n_pix;
     const uint32_t my_tiles = gw < g.n_bins ? (g.n_bins - gw + n_warps - 1) / n_warps : 0u;
     const uint32_t my_items = gw < n_items ? (n_items - gw + n_warps - 1) / n_warps : 0u;
     const uint32_t gap = my_items ? max(1u, my_tiles / my_items) : 0xFFFFFFFFu;
@@ -343,19 +334,9 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
     auto do_item = [&]() {
         const uint4 w = items[it];
         it += n_warps;
-        float2* out = tile_origin(g, grid, w.x, tr);
         zero_tile<S>(sm.tile, lane);
-        accumulate_bin<S, KB>(g, records, w.y, w.z, rec_start[w.x] + (bin_start[w.x + 1] - bin_start[w.x]), sm, lane);
-        if (ring) {
-            flush_ring<S>(g, sm, grid, w.x, tr, lane);
-            return;
-        }
-#pragma unroll 4
-        for (int y = 0; y < T; ++y) {
-            const float2 v = tr ? inner[lane * C::P + y] : inner[y * C::P + lane];
-            if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
-        }
-        __syncwarp();
+        accumulate_records<S, KB>(g, records, w.y, w.z, sm, lane);
+        flush_ring<S>(g, sm, grid, w.x, tr, lane);
     };
 
     for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
@@ -364,35 +345,16 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ rec_start,
             since = 0;
         }
         ++since;
-        const uint32_t s = rec_start[bin], e = rec_start[bin + 1];
+        const uint32_t s = bin_start[bin], e = bin_start[bin + 1];
         if (e - s > WS_CHUNK) continue;                     // heavy: its chunks are items
-        float2* out = tile_origin(g, grid, bin, tr);
         if (s == e) {
-            if (mode == WS_GRID_OVERWRITE) store_zero_tile(out, N, lane);
+            if (mode == WS_GRID_OVERWRITE && occ_start[bin + 1] == occ_start[bin])
+                store_zero_tile(tile_origin(g, grid, bin, tr), (size_t)g.n_pix, lane);
             continue;
         }
         zero_tile<S>(sm.tile, lane);
-        accumulate_bin<S, KB>(g, records, s, e, s + (bin_start[bin + 1] - bin_start[bin]), sm, lane);
-        if (ring) {
-            flush_ring<S>(g, sm, grid, bin, tr, lane);
-            continue;
-        }
-        bool add = mode == WS_GRID_ACCUMULATE;
-        if (mode == WS_GRID_SPARSE_ADD) {                       // warp-uniform: did an earlier chunk fill this tile?
-            const uint32_t nt = (uint32_t)g.nt, tx = bin % nt, r = bin / nt;
-            add = ws_tile_occupied(mv, g.nt, r / nt, r % nt, tx);
-        }
-        if (!add) {
-#pragma unroll 4
-            for (int y = 0; y < T; ++y) __stcs(out + (size_t)y * N + lane, tr ? inner[lane * C::P + y] : inner[y * C::P + lane]);
-        } else {        // no other warp writes this tile in this launch except through red: fire-and-forget vector adds
-#pragma unroll 4
-            for (int y = 0; y < T; ++y) {
-                const float2 v = tr ? inner[lane * C::P + y] : inner[y * C::P + lane];
-                if (v.x != 0.f || v.y != 0.f) atomicAdd(out + (size_t)y * N + lane, v);   // RED.E.ADD.F32x2
-            }
-        }
-        __syncwarp();
+        accumulate_records<S, KB>(g, records, s, e, sm, lane);
+        flush_ring<S>(g, sm, grid, bin, tr, lane);
     }
     while (it < n_items) do_item();
 }
@@ -406,20 +368,16 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     const size_t smem = C::WARP_BYTES * C::WARPS;
     // per device, and cheap: set on every launch rather than cached in a process-wide flag
     if (cudaFuncSetAttribute(k_grid<S, KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return WS_ERR_CUDA;
-    // ring scheme (bins of ws_bin_visibilities_for a sparse mode): the record lists hold home records only, indexed by
-    // bin_start; rec_start = home + halo counts then only says which tiles receive anything
-    const int ring = plan->last_ring ? 1 : 0;
     const uint32_t* occ_start = (const uint32_t*)(ws + L.off_rec_start);
-    const uint32_t* rec_start = ring ? (const uint32_t*)(ws + L.off_counts_home) : occ_start;
+    const uint32_t* bin_start = (const uint32_t*)(ws + L.off_counts_home);
     const float4* records = (const float4*)(ws + L.off_records);
     WsStatus* status = plan->d_status;
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, rec_start, occ_start, ring, items, L.item_capacity, status, grid, mode,
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, bin_start, occ_start, 1, items, L.item_capacity, status, grid, mode,
                                                           orient, mv);
-    k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, rec_start, (const uint32_t*)(ws + L.off_counts_home), items, records,
-                                                                 grid, mode, status, orient, mv, ring);
+    k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, bin_start, occ_start, items, records, grid, mode, status, orient);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }

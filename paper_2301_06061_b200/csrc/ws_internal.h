@@ -53,13 +53,13 @@ struct WsRemap {
 // Workspace carve-up for one ws_grid_visibilities call (all offsets 256-byte aligned).
 struct WsLayout {
     size_t off_counts_home, off_counts_halo;    // [n_bins + 1] u32 each: histograms -> exclusive scans (bin_start / halo_start)
-    size_t off_rec_start;                       // [n_bins + 1] u32: bin_start + halo_start = first record of each bin
-    size_t off_cursor_home, off_cursor_halo;    // [n_bins] u32: running slot cursors of the scatter
+    size_t off_rec_start;                       // [n_bins + 1] u32: bin_start + halo_start: a tile receives something iff its entry grows
+    size_t off_cursor_home;                     // [n_bins] u32: running slot cursors of the scatter
     size_t off_block_sums;                      // scan scratch
     size_t off_keys, off_perm, off_sorted_keys; // [n_vis] u32 each
     size_t off_presum;                          // [presum_rows] float2: per-row sums of weight * vis (WS_FLAG_PRESUM_CHANNELS)
     size_t off_items;                           // heavy-chunk work items (uint4)
-    size_t off_records;                         // float4 records
+    size_t off_records;                         // float4 records, one per kept visibility, lists indexed by bin_start
     size_t total;                               // bytes used for capacity `rec_capacity`
     uint64_t rec_capacity;                      // records that fit
     uint32_t item_capacity;
@@ -107,8 +107,6 @@ struct ws_plan {
     int64_t snapshot_rows;                      // ws_plan_set_snapshot_rows hint (0: none)
     const float* last_weights;                  // weights of the last ws_bin_visibilities call
     int32_t last_chan_per_key;                  // visibilities per binned entry: 1, or n_chan after a pre-summed call
-    bool bin_ring;                              // the binning call in progress stores home records only (ring scheme, sparse modes)
-    bool last_ring;                             // ... and so did the last one: ws_grid_binned must spread the rings
     bool last_has_values;                       // false: the bins were made by ws_degrid_visibilities (records carry no visibilities)
     cudaStream_t copy_stream;                   // ws_image_from_host: the H2D copies of the next chunk run beside the gridding
     cudaEvent_t ev_start, ev_chunk[WS_E2E_MAX_CHUNKS];    // of this one (created on first use)

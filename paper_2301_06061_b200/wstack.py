@@ -28,7 +28,7 @@ WS_NORM_SUMWT, WS_NORM_N, WS_NORM_TAPER = 1, 2, 4
 EXPORTED_SYMBOLS = [
     "ws_version", "ws_strerror", "ws_last_error", "ws_plan_create", "ws_plan_destroy", "ws_plan_set_snapshot_rows", "ws_plan_set_plane_range", "ws_grid_bytes",
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
-    "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_bin_visibilities_for", "ws_grid_binned", "ws_fft_planes",
+    "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
     "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_plan_set_e2e_chunk_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
     "ws_launch_count", "ws_measure_fp32_tflops",
 ]
@@ -78,7 +78,6 @@ def lib():
         "ws_grid_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, i32, vp, sz, vp]),
         "ws_bin_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp]),
         "ws_grid_binned": (C.c_int, [vp, vp, i32, vp, sz, vp]),
-        "ws_bin_visibilities_for": (C.c_int, [vp, i32, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp]),
         "ws_fft_planes": (C.c_int, [vp, vp, vp, sz, vp]),
         "ws_wcorrect_accumulate": (C.c_int, [vp, vp, vp, i32, vp, vp]),
         "ws_fft_wcorrect": (C.c_int, [vp, vp, vp, i32, vp, u32, vp, sz, vp]),
@@ -228,18 +227,14 @@ class Plan:
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
 
-    def bin_visibilities(self, uvw, vis, weights, freq_hz, workspace, stream=None, mode: Optional[int] = None):
-        """a1.  mode None: bins that serve every gridding mode; a WS_GRID_* mode: bins for that mode (home records only for
-        the sparse modes, ws_bin_visibilities_for)."""
+    def bin_visibilities(self, uvw, vis, weights, freq_hz, workspace, stream=None):
         n_rows = int(uvw.shape[0])
         n_chan = int(vis.shape[1]) if vis.dim() == 2 else 1
         keep, fp = _freq(freq_hz, n_chan)
-        args = (_dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"), _dev(weights, torch.float32, "weights"), fp,
-                n_rows, n_chan, _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream))
-        if mode is None:
-            self._check(lib().ws_bin_visibilities(self._h, *args))
-        else:
-            self._check(lib().ws_bin_visibilities_for(self._h, int(mode), *args))
+        self._check(lib().ws_bin_visibilities(
+            self._h, _dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"),
+            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan,
+            _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
 
     def grid_binned(self, grid, workspace, mode: int = WS_GRID_OVERWRITE, stream=None):

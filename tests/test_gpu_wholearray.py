@@ -85,14 +85,11 @@ def _whole_config(oracle, cfg_name, presum=False, one_mesh=False, dup_factor=Non
 
     def grid_overwrite():
         grid_o.fill_(float("nan"))
-        plan.bin_visibilities(dg.uvw, dg.vis, dg.weights, d.freqs_hz, wsp)
         plan.grid_binned(grid_o, wsp, mode=ws.WS_GRID_OVERWRITE)
         plan.async_status()
 
     def grid_sparse():                                           # last: the plan's occupancy describes grid_s
         grid_s.fill_(float("nan"))
-        # bins for the sparse mode, as bench.py makes them: home records only, each tile's ring spread onto its neighbours
-        plan.bin_visibilities(dg.uvw, dg.vis, dg.weights, d.freqs_hz, wsp, mode=ws.WS_GRID_SPARSE)
         plan.grid_binned(grid_s, wsp, mode=ws.WS_GRID_SPARSE)
         plan.async_status()
         return bool(plan.occupancy()["transposed"])
