@@ -33,10 +33,9 @@ constexpr int T = WS_TILE;
 
 constexpr int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
-// The warp's shared tile covers the 32 x 32 cells it owns PLUS a ring of H cells: the footprint of a record whose
-// centre lies inside the tile (a "home" record) then never leaves the buffer, and the inner loop over the home records
-// of a bin -- 71 % of all records on Large -- needs no bounds test at all.  The ring collects only part of what belongs
-// there (the neighbour tiles hold their own copies of the records that reach them) and is never stored.
+// The warp's shared buffer covers the 32 x 32 cells of its tile PLUS a ring of H cells: the footprint of a record whose
+// centre lies inside the tile never leaves the buffer, so the inner loop needs no bounds test.  What lands in the ring
+// belongs to the neighbour tiles and reaches them when the whole buffer is added to the mesh (flush_ring).
 template <int S>
 struct TileCfg {
     static constexpr int H = (S - 1) / 2;
@@ -48,11 +47,13 @@ struct TileCfg {
     static constexpr int SP = S;                    // pitch of the u taps of a record (odd: lane r's scalar stores are conflict-free)
     static constexpr int GP = NRP * (R | 1);        // pitch of its v taps, [R][NRP] + padding: an odd number of NRP-vectors, so
                                                     // that the lanes' vector stores of one br fall into distinct banks
-    static constexpr int TILE_CELLS = ROWS * P;
+    static constexpr int TILE_CELLS = (ROWS - 1) * P + ROWS;   // (the last row needs no padding)
     static constexpr int GU_FLOATS = (32 * SP + 3) / 4 * 4;    // (keeps gv 16-byte aligned)
-    // per warp: tile | meta[32] float4 | gu[32][SP] | gv[32][GP]
+    static constexpr int GV_FLOATS = (31 * GP + R * NRP + 1) / 2 * 2;   // (the last record needs no padding; keeps the tile 8-byte aligned)
+    // per warp: meta[32] float4 | gu[32][SP] | gv[32][GP] | tile.  Sized to the byte: S = 7 comes to 14528 bytes, and sixteen of
+    // those are exactly the 227 KB a CTA may have
     static constexpr size_t WARP_BYTES =
-        ((size_t)TILE_CELLS * sizeof(float2) + 32 * sizeof(float4) + (GU_FLOATS + 32 * GP) * sizeof(float) + 15) / 16 * 16;
+        (32 * sizeof(float4) + (size_t)(GU_FLOATS + GV_FLOATS) * sizeof(float) + (size_t)TILE_CELLS * sizeof(float2) + 15) / 16 * 16;
     // one CTA per SM with as many (independent) warps as the 227 KB of shared memory hold, at most 16
     static constexpr int WARPS = (227 * 1024) / WARP_BYTES >= 16 ? 16 : (int)((227 * 1024) / WARP_BYTES);
     static constexpr int THREADS = WARPS * 32;
@@ -88,10 +89,10 @@ struct WarpSmem {
     float* gv;
     __device__ __forceinline__ WarpSmem(unsigned char* base) {
         using C = TileCfg<S>;
-        tile = (float2*)base;
-        meta = (float4*)(tile + C::TILE_CELLS);
+        meta = (float4*)base;
         gu = (float*)(meta + 32);
         gv = gu + C::GU_FLOATS;
+        tile = (float2*)(gv + C::GV_FLOATS);
     }
 };
 
