@@ -232,7 +232,8 @@ __device__ __forceinline__ void zero_tile(float2* tile, int lane) {
 // a tile that earlier chunks filled is left alone; WS_GRID_ACCUMULATE clears nothing.
 __global__ void __launch_bounds__(256)
 k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ starts, const uint32_t* __restrict__ occ_start,
-                int clear_occupied, uint4* __restrict__ items, uint32_t item_capacity, WsStatus* __restrict__ status,
+                int clear_occupied, uint32_t* __restrict__ light, uint4* __restrict__ items, uint32_t item_capacity,
+                WsStatus* __restrict__ status,
                 float2* __restrict__ grid, int mode, const uint32_t* __restrict__ orient, const WsMaskView mv) {
     if (status->overflow) return;
     const bool tr = orient && *orient;
@@ -255,6 +256,15 @@ k_prepare_heavy(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ s
     for (unsigned m = __ballot_sync(0xffffffffu, clear); m; m &= m - 1) {
         const uint32_t hb = (b - lane) + (__ffs(m) - 1);
         store_zero_tile(tile_origin(g, grid, hb, tr), (size_t)g.n_pix, lane);
+    }
+    if (light) {                                 // the bins the gridder takes whole, as a list: it need not walk the empty ones
+        const unsigned lm = __ballot_sync(0xffffffffu, cnt > 0 && !heavy);
+        if (lm) {
+            uint32_t base = 0;
+            if (lane == 0) base = atomicAdd(&status->n_light, (uint32_t)__popc(lm));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (cnt > 0 && !heavy) light[base + __popc(lm & ((1u << lane) - 1u))] = b;
+        }
     }
     if (!hm) return;
     uint32_t inc = chunks;                       // inclusive warp scan of the chunk counts
@@ -316,8 +326,8 @@ __device__ __forceinline__ void flush_ring(const WsGeom& g, const WarpSmem<S>& s
 template <int S, bool KB>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 1)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ occ_start,
-       const uint4* __restrict__ items, const float4* __restrict__ records, float2* __restrict__ grid, int mode,
-       const WsStatus* __restrict__ status, const uint32_t* __restrict__ orient) {
+       const uint32_t* __restrict__ light, const uint4* __restrict__ items, const float4* __restrict__ records,
+       float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status, const uint32_t* __restrict__ orient) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -340,6 +350,26 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start,
         flush_ring<S>(g, sm, grid, w.x, tr, lane);
     };
 
+    if (mode != WS_GRID_OVERWRITE) {
+        // only the listed bins matter (k_prepare_heavy: non-empty, not heavy); 96 % of the tiles of Large hold nothing, and
+        // walking them costs every warp a dependent load each -- again in every call of a chunked run
+        const uint32_t n_light = status->n_light;
+        const uint32_t my_light = gw < n_light ? (n_light - gw + n_warps - 1) / n_warps : 0u;
+        const uint32_t lgap = my_items ? max(1u, my_light / my_items) : 0xFFFFFFFFu;
+        for (uint32_t i = gw; i < n_light; i += n_warps) {
+            if (it < n_items && since >= lgap) {
+                do_item();
+                since = 0;
+            }
+            ++since;
+            const uint32_t bin = light[i];
+            zero_tile<S>(sm.tile, lane);
+            accumulate_records<S, KB>(g, records, bin_start[bin], bin_start[bin + 1], sm, lane);
+            flush_ring<S>(g, sm, grid, bin, tr, lane);
+        }
+        while (it < n_items) do_item();
+        return;
+    }
     for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
         if (it < n_items && since >= gap) {
             do_item();
@@ -375,10 +405,11 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     WsStatus* status = plan->d_status;
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
-    if (cudaMemsetAsync(&status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, bin_start, occ_start, 1, items, L.item_capacity, status, grid, mode,
-                                                          orient, mv);
-    k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, bin_start, occ_start, items, records, grid, mode, status, orient);
+    uint32_t* light = (uint32_t*)(ws + L.off_cursor_home);        // (the scatter's cursors are spent)
+    if (cudaMemsetAsync(&status->n_items, 0, 2 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, bin_start, occ_start, 1, light, items, L.item_capacity, status, grid,
+                                                          mode, orient, mv);
+    k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, bin_start, occ_start, light, items, records, grid, mode, status, orient);
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 2;
 }
@@ -389,7 +420,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st) {
     const WsGeom& g = plan->geom;
     if (cudaMemsetAsync(&plan->d_status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, items, item_capacity, plan->d_status, nullptr,
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, nullptr, items, item_capacity, plan->d_status, nullptr,
                                                           WS_GRID_ACCUMULATE, nullptr, WsMaskView{nullptr, 0u, 1});
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;

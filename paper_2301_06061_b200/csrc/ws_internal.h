@@ -54,7 +54,7 @@ struct WsRemap {
 struct WsLayout {
     size_t off_counts_home, off_counts_halo;    // [n_bins + 1] u32 each: histograms -> exclusive scans (bin_start / halo_start)
     size_t off_rec_start;                       // [n_bins + 1] u32: bin_start + halo_start: a tile receives something iff its entry grows
-    size_t off_cursor_home;                     // [n_bins] u32: running slot cursors of the scatter
+    size_t off_cursor_home;                     // [n_bins] u32: running slot cursors of the scatter; afterwards the gridder's list of light bins
     size_t off_block_sums;                      // scan scratch
     size_t off_keys, off_perm, off_sorted_keys; // [n_vis] u32 each
     size_t off_presum;                          // [presum_rows] float2: per-row sums of weight * vis (WS_FLAG_PRESUM_CHANNELS)
@@ -69,9 +69,10 @@ struct WsStatus {                               // device-side, 64 bytes
     uint32_t n_kept;                            // kept visibilities (home histogram total)
     uint32_t n_records;                         // records incl. halo copies
     uint32_t n_items;                           // heavy chunks queued
+    uint32_t n_light;                           // non-empty bins that are not heavy, listed for the gridder
     uint32_t overflow;                          // 1: record or item capacity exceeded, gridding skipped (cleared by every binning call)
     uint32_t sticky_overflow;                   // ... of ANY call since the last ws_async_status (which clears it)
-    uint32_t pad[11];
+    uint32_t pad[10];
 };
 
 struct ws_plan {
