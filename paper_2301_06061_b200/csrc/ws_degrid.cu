@@ -157,11 +157,11 @@ __device__ __forceinline__ void gather(const WsGeom& g, const float4* __restrict
     __syncwarp();
 }
 
-// Persistent kernel: warp w takes bins w, w + W, ... and the chunks of the heavy bins (items), interleaved.
+// Persistent kernel: warp w takes the listed (non-empty, not heavy) bins w, w + W, ... and the chunks of the heavy bins (items), interleaved.
 template <int S, bool KB>
 __global__ void __launch_bounds__(DgCfg<S>::THREADS, 2)
 k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
-         const uint4* __restrict__ items, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
+         const uint32_t* __restrict__ light, const uint4* __restrict__ items, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
          const float2* __restrict__ planes, float2* __restrict__ vis_out, float scale, int accumulate,
          const WsStatus* __restrict__ status, int xf_lr0, const uint32_t* __restrict__ orient) {
     using C = DgCfg<S>;
@@ -173,7 +173,8 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
     const uint32_t n_items = status->n_items;
     const uint32_t n_warps = gridDim.x * C::WARPS;
     const uint32_t gw = blockIdx.x * C::WARPS + wid;
-    const uint32_t my_tiles = gw < g.n_bins ? (g.n_bins - gw + n_warps - 1) / n_warps : 0u;
+    const uint32_t n_light = status->n_light;    // the non-empty bins that are not heavy, listed by k_prepare_heavy
+    const uint32_t my_tiles = gw < n_light ? (n_light - gw + n_warps - 1) / n_warps : 0u;
     const uint32_t my_items = gw < n_items ? (n_items - gw + n_warps - 1) / n_warps : 0u;
     const uint32_t gap = my_items ? max(1u, my_tiles / my_items) : 0xFFFFFFFFu;
     uint32_t it = gw, since = 0;
@@ -185,16 +186,15 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
         gather<S, KB>(g, records, perm, w.y, w.z, halo_start[w.x], region, vis_out, scale, accumulate, lane);
     };
 
-    for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
+    for (uint32_t i = gw; i < n_light; i += n_warps) {
         if (it < n_items && since >= gap) {
             do_item();
             since = 0;
         }
         ++since;
-        const uint32_t s = bin_start[bin], e = bin_start[bin + 1];
-        if (s == e || e - s > WS_CHUNK) continue;           // empty, or heavy: its chunks are items
+        const uint32_t bin = light[i];
         load_region<S>(g, planes, bin, region, lane, xf_lr0, tr);
-        gather<S, KB>(g, records, perm, s, e, halo_start[bin], region, vis_out, scale, accumulate, lane);
+        gather<S, KB>(g, records, perm, bin_start[bin], bin_start[bin + 1], halo_start[bin], region, vis_out, scale, accumulate, lane);
     }
     while (it < n_items) do_item();
 }
@@ -210,9 +210,10 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, const float2* planes, f
     const uint32_t* bin_start = (const uint32_t*)(ws + L.off_counts_home);
     const uint32_t* halo_start = (const uint32_t*)(ws + L.off_counts_halo);
     uint4* items = (uint4*)(ws + L.off_items);
-    int rc = ws_launch_items(plan, bin_start, items, L.item_capacity, st);
+    uint32_t* light = (uint32_t*)(ws + L.off_cursor_home);        // (the scatter's cursors are spent)
+    int rc = ws_launch_items(plan, bin_start, light, items, L.item_capacity, st);
     if (rc < 0) return rc;
-    k_degrid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(plan->geom, bin_start, halo_start, items,
+    k_degrid<S, KB><<<plan->sm_count * 2, C::THREADS, smem, st>>>(plan->geom, bin_start, halo_start, light, items,
                                                                   (const float4*)(ws + L.off_records),
                                                                   (const uint32_t*)(ws + L.off_perm), planes, vis_out, scale,
                                                                   accumulate, plan->d_status, xf_lr0, orient);

@@ -416,11 +416,12 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 
 }  // namespace
 
-// Work items for the lists of `starts` ([n_bins + 1] offsets) longer than WS_CHUNK: used by the degridder on the home lists.
-int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st) {
+// Work items for the lists of `starts` ([n_bins + 1] offsets) longer than WS_CHUNK, and the list of the other non-empty bins:
+// used by the degridder on the home lists.
+int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint32_t* light, uint4* items, uint32_t item_capacity, cudaStream_t st) {
     const WsGeom& g = plan->geom;
-    if (cudaMemsetAsync(&plan->d_status->n_items, 0, sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, nullptr, items, item_capacity, plan->d_status, nullptr,
+    if (cudaMemsetAsync(&plan->d_status->n_items, 0, 2 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light
+    k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, light, items, item_capacity, plan->d_status, nullptr,
                                                           WS_GRID_ACCUMULATE, nullptr, WsMaskView{nullptr, 0u, 1});
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;
     return 1;

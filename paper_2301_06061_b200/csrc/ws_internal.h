@@ -148,7 +148,7 @@ int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);
 WsMaskView ws_fft_mask_view(const ws_plan* plan);
-int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint4* items, uint32_t item_capacity, cudaStream_t st);
+int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint32_t* light, uint4* items, uint32_t item_capacity, cudaStream_t st);
 int ws_launch_wscreen_fwd(ws_plan* plan, const float2* image, float2* planes, int conj_out, cudaStream_t st);
 // xf_lr0 < 0: planes in natural (FFT-native) order; >= 0: log2(N / 256), the planes hold the CONJUGATE of the transform
 // with the rows where ws_fft_columns leaves them (frequency f at row ((f mod R0) << 8) | (f / R0))
