@@ -257,7 +257,9 @@ __device__ __forceinline__ void bfly(E* x) {
 // ([k][u][v]: the roles of tx and ty swap).  A WS_GRID_SPARSE mesh is private to this library, so the gridder stores
 // it in whichever orientation leaves fewer bands to transform (ctrl[2]): the uv tracks of an east-west-ish array are
 // squeezed in v by sin(dec), and a band costs 2 N x 256 B of traffic in pass 1b and pass 2.
-// Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; set = class masks, band masks.
+// Buffer: ctrl[8] = {bands of set 0, bands of set 1, transposed, ...} | set 0 | set 1; set = class masks, band masks,
+// band list.  band list: the k nt + tx of the non-empty bands, in the order they were first marked (ctrl[set] of
+// them): the column passes walk that list instead of testing every band of every plane.
 // Masks are OR-ed into (chunked gridding accumulates); ws_fft_masks_clear zeroes them.
 constexpr int MASK_CTRL = WS_MASK_CTRL;
 // Words per class mask (one bit per input of pass 1a's radix-R0 butterfly: R0 = 64 for N = 16384 needs two) and band
@@ -289,7 +291,10 @@ k_fft_masks(const uint32_t* __restrict__ rec_start, int nt, int r0, uint32_t n_c
         for (int i = 0; i < cw; ++i)
             if (mask[i]) atomicOr(class_mask + (size_t)id * cw + i, mask[i]);
         const uint32_t bit = 1u << (bs & 31);
-        if (!(atomicOr(band_mask + k * bw + (bs >> 5), bit) & bit)) atomicAdd(masks + set, 1u);
+        if (!(atomicOr(band_mask + k * bw + (bs >> 5), bit) & bit)) {
+            uint32_t* band_list = band_mask + (n_classes >> 3) / nt * bw;
+            band_list[atomicAdd(masks + set, 1u)] = kb;
+        }
     }
 }
 // Degridding (ws_degrid.cu): the planes are DENSE on the way in (rows of the model image times the w screen, transformed
@@ -324,7 +329,8 @@ k_fft_masks_degrid(const uint32_t* __restrict__ bin_start, int nt, int r0, uint3
             class_mask[((size_t)kb * 8u + c) * cw + i] = left >= 32 ? 0xFFFFFFFFu : (1u << left) - 1u;
         }
     atomicOr(band_mask + k * bw + (bs >> 5), 1u << (bs & 31));
-    atomicAdd(masks + set, 1u);
+    uint32_t* band_list = band_mask + n_kb / nt * bw;
+    band_list[atomicAdd(masks + set, 1u)] = kb;
 }
 
 // the orientation of a WS_GRID_SPARSE mesh: transposed iff that leaves fewer bands (allow = 0: as the header says)
@@ -399,9 +405,16 @@ template <int LOGN>
 __global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
-    const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
-    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x)
-        colA_item<LOGN>(grid, tw, class_mask, item >> 5, item & 31);      // 32 groups of 8 rows per (plane, band)
+    if (!masks) {
+        for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x)
+            colA_item<LOGN>(grid, tw, nullptr, item >> 5, item & 31);     // 32 groups of 8 rows per (plane, band)
+        return;
+    }
+    const uint32_t* class_mask = mask_set(masks, set_words);
+    const uint32_t* band_list = class_mask + (set_words - n_items / 32u);  // the non-empty (plane, band) pairs
+    const uint32_t n_list = masks[masks[2] ? 1 : 0] * 32u;
+    for (uint32_t item = blockIdx.x; item < n_list; item += gridDim.x)
+        colA_item<LOGN>(grid, tw, class_mask, band_list[item >> 5], item & 31);
 }
 
 // ---- pass 1b: the 256-point column transforms -------------------------------------------------------------------
@@ -468,11 +481,18 @@ __global__ void __launch_bounds__(CT, 2)
 k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
            uint32_t set_words, uint32_t n_items) {
     constexpr int R0 = 1 << (LOGN - 8);
-    const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
-    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const uint32_t m0 = item % R0, ktx = item / R0;
+    if (!masks) {
+        for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x)
+            colB_item<LOGN>(grid, tw, blk, 0xFFu, item / R0, item % R0);
+        return;
+    }
+    const uint32_t* class_mask = mask_set(masks, set_words);
+    const uint32_t* band_list = class_mask + (set_words - n_items / R0);    // the non-empty (plane, band) pairs
+    const uint32_t n_list = masks[masks[2] ? 1 : 0] * R0;
+    for (uint32_t item = blockIdx.x; item < n_list; item += gridDim.x) {
+        const uint32_t m0 = item % R0, ktx = band_list[item / R0];
         const uint32_t cmask = band_classes<LOGN>(class_mask, ktx);
         if (cmask == 0) continue;
         colB_item<LOGN>(grid, tw, blk, cmask, ktx, m0);
@@ -858,7 +878,8 @@ k_fft_rows(const __grid_constant__ WcParams prm, const float2* __restrict__ plan
     constexpr int N = C::N, ROWS = C::ROWS, NT = C::NT, R0 = C::R0, LAND = C::LAND, BW = C::BW, NBUF = C::NBUF;
     // occupancy: the band masks of the orientation the mesh is stored in; transposed: the mesh is [k][u][v], i.e. a
     // row position is a u-frequency and the image comes out transposed (the phase screen is symmetric in l and m)
-    const uint32_t* band_mask = masks ? mask_set(masks, set_words) + (set_words - (uint32_t)BW * (uint32_t)prm.n_wplanes) : nullptr;
+    const uint32_t* band_mask =
+        masks ? mask_set(masks, set_words) + (uint32_t)prm.n_wplanes * (uint32_t)(NT * 8 * class_words(R0)) : nullptr;
     const bool transposed = masks && masks[2];
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* landing0 = (float2*)smem_raw;                               // NBUF buffers of LAND points
@@ -1080,7 +1101,7 @@ int init_n(ws_plan* plan) {
     }
     const size_t n_class = (size_t)plan->prm.n_wplanes * (N / 32) * 8 * class_words(R0),
                  n_band = (size_t)plan->prm.n_wplanes * band_words(N / 32);
-    plan->mask_set_words = n_class + n_band;
+    plan->mask_set_words = n_class + n_band + (size_t)plan->prm.n_wplanes * (N / 32);      // + the band list
     plan->mask_class_words = class_words(R0);
     plan->mask_band_words = band_words(N / 32);
     plan->mask_words = MASK_CTRL + 2 * plan->mask_set_words;

@@ -102,7 +102,7 @@ struct ws_plan {
     size_t tw_off_a, tw_off_b, tw_off_c;        // entry offsets of the pass 1a / 1b tables and of the row kernel's register constants
     int mask_class_words, mask_band_words;      // words per class mask (2 for N = 16384) and band words per plane (16 for N = 16384)
     void* d_masks;                              // plan-owned tile-occupancy masks of the mesh (class masks, band masks)
-    size_t mask_words, mask_set_words;          // whole buffer; one set (class masks + band masks) of the two orientations
+    size_t mask_words, mask_set_words;          // whole buffer; one set (class masks, band masks, band list) of the two orientations
     double* d_sumwt;                            // plan-owned: sum of the weights of the kept visibilities (WS_FLAG_TRACK_SUMWT)
     float* d_taper;                             // plan-owned [N]: 1 / ghat((p - N/2)/N), fp64-computed on the host
     int64_t snapshot_rows;                      // ws_plan_set_snapshot_rows hint (0: none)
