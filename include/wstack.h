@@ -298,6 +298,26 @@ int ws_get_occupancy(ws_plan* plan, double* tiles, double* classes, double* band
  * exceeded -> WS_ERR_WORKSPACE, CUDA fault -> WS_ERR_CUDA). */
 int ws_async_status(ws_plan* plan, void* stream);
 
+/* a1 + a2 WITHOUT a caller-allocated workspace, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * serving loops, harnesses that forbid it): ws_grid_visibilities (Eq. 3 at :80) with its scratch -- the
+ * histograms, keys, permutation, sorted records and work items of the binning -- in a static device array of
+ * WS_STATIC_SCRATCH_BYTES that every GPU holding the library keeps until the process exits.  Same arguments, layouts,
+ * modes and results as ws_grid_visibilities (all device pointers, 16-byte aligned; freq_hz host or NULL); the call
+ * allocates and frees nothing on the device and calls no library routine that does.
+ *   Limit: the layout for n_rows * n_chan visibilities (n_rows under WS_FLAG_PRESUM_CHANNELS) and the plan's bins must
+ * fit the array: about 16 (n_bins + 1) + 28.1 n_vis bytes, e.g. the 1.13 million visibilities of a 2048^2 x 16-plane mesh.
+ * Beyond it the call returns WS_ERR_WORKSPACE before anything is launched and ws_last_error names the bytes needed and
+ * the limit; a WS_FLAG_MESH_F64 plan (which uses no scratch) is WS_ERR_UNSUPPORTED.
+ *   The array is SHARED by every plan and stream of the process on that device and keeps the last call's contents: the
+ * call clears what must start at zero (on `stream`), but two calls whose work overlaps on the GPU race -- keep them on
+ * one stream or order them with events -- and ws_get_bins after it reads the array, so it must come before the next
+ * static call.  The plan itself is created beforehand (ws_plan_create allocates). */
+#define WS_STATIC_SCRATCH_BYTES (32u << 20)
+int ws_grid_visibilities_static(ws_plan* plan, const float* uvw, const void* vis, const float* weights,
+                                const double* freq_hz, int64_t n_rows, int32_t n_chan, void* grid, int32_t mode,
+                                void* stream);
+size_t ws_static_scratch_bytes(void); /* = WS_STATIC_SCRATCH_BYTES of the library that is loaded */
+
 /* Diagnostic (not part of the path): the fp32 FMA rate, in TFLOP/s, that a register-only FFMA loop reaches on the plan's
  * device (best of four short launches; synchronises `stream`).  bench.py prints it beside the derived fp32 peak. */
 int ws_measure_fp32_tflops(ws_plan* plan, double* tflops, void* stream);

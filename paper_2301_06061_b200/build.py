@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwstack.so")
-SOURCES = ["ws_api.cu", "ws_bin.cu", "ws_grid.cu", "ws_wcorrect.cu", "ws_fft.cu", "ws_degrid.cu", "ws_probe.cu", "ws_f64.cu"]
+SOURCES = ["ws_api.cu", "ws_bin.cu", "ws_grid.cu", "ws_wcorrect.cu", "ws_fft.cu", "ws_degrid.cu", "ws_probe.cu", "ws_f64.cu", "ws_static.cu"]
 HEADERS = [os.path.join(CSRC, "ws_internal.h"), os.path.join(CSRC, "ws_phase.cuh"), os.path.join(CSRC, "ws_taps.cuh"), os.path.join(CSRC, "ws_place.cuh"), os.path.join(HERE, "..", "include", "wstack.h")]
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 

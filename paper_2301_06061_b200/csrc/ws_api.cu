@@ -158,6 +158,12 @@ int make_taps(const ws_params& p, WsGeom& g) {
 
 }  // namespace
 
+// Bytes of workspace a1 + a2 need for n_vis visibilities (the layout alone, with fit_layout's alignment margin; no FFT
+// work area): what ws_grid_visibilities_static (ws_static.cu) holds against the size of its static array.
+size_t ws_bin_layout_bytes(const ws_plan* plan, int64_t n_vis, int64_t presum_rows) {
+    return make_layout(plan, n_vis, (uint64_t)n_vis + 64, presum_rows).total + 4096;
+}
+
 extern "C" {
 
 int ws_version(void) { return WS_VERSION; }

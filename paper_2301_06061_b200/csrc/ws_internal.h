@@ -144,6 +144,7 @@ __device__ __forceinline__ bool ws_tile_occupied(const WsMaskView& mv, int nt, u
 #endif
 
 // ---- launchers (each returns the number of kernels it launched, or a negative WS_ERR_*) ----------------
+size_t ws_bin_layout_bytes(const ws_plan* plan, int64_t n_vis, int64_t presum_rows);      // ws_api.cu
 int ws_launch_bin(ws_plan* plan, const WsLayout& L, char* ws, const WsChanConsts& cc, const float* uvw,
                   const float2* vis, const float* wt, int64_t n_rows, int32_t n_chan, cudaStream_t st);
 int ws_launch_grid(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode, cudaStream_t st);

@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = [
     "ws_image_bytes", "ws_dirty_bytes", "ws_workspace_bytes", "ws_workspace_bytes_for", "ws_fft_workspace_bytes",
     "ws_plan_tile", "ws_plan_n_bins", "ws_grid_zero", "ws_grid_visibilities", "ws_bin_visibilities", "ws_grid_binned", "ws_fft_planes",
     "ws_wcorrect_accumulate", "ws_fft_wcorrect", "ws_fft_columns", "ws_fft_rows_wcorrect", "ws_plan_fft_is_own", "ws_get_occupancy", "ws_dirty_image", "ws_get_sum_weights", "ws_predict_planes", "ws_degrid_visibilities", "ws_predict_visibilities", "ws_dev_inputs_bytes", "ws_plan_set_e2e_chunk_bytes", "ws_image_from_host", "ws_get_bins", "ws_async_status",
-    "ws_launch_count", "ws_measure_fp32_tflops",
+    "ws_launch_count", "ws_measure_fp32_tflops", "ws_grid_visibilities_static", "ws_static_scratch_bytes",
 ]
 
 
@@ -77,6 +77,8 @@ def lib():
         "ws_grid_zero": (C.c_int, [vp, vp, vp]),
         "ws_grid_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, i32, vp, sz, vp]),
         "ws_bin_visibilities": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, sz, vp]),
+        "ws_grid_visibilities_static": (C.c_int, [vp, vp, vp, vp, C.POINTER(C.c_double), i64, i32, vp, i32, vp]),
+        "ws_static_scratch_bytes": (sz, []),
         "ws_grid_binned": (C.c_int, [vp, vp, i32, vp, sz, vp]),
         "ws_fft_planes": (C.c_int, [vp, vp, vp, sz, vp]),
         "ws_wcorrect_accumulate": (C.c_int, [vp, vp, vp, i32, vp, vp]),
@@ -107,6 +109,11 @@ def lib():
                            "(python -m paper_2301_06061_b200.build --force)")
     _lib = L
     return L
+
+
+def static_scratch_bytes() -> int:
+    """Size of the static device array behind Plan.grid_visibilities_static (WS_STATIC_SCRATCH_BYTES of the loaded library)."""
+    return int(lib().ws_static_scratch_bytes())
 
 
 def _stream(stream) -> int:
@@ -226,6 +233,17 @@ class Plan:
             _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan, _dev(grid, self._c, "grid"), mode,
             _dev(workspace, torch.uint8, "workspace"), workspace.numel(), _stream(stream)))
         self._ws = workspace
+
+    def grid_visibilities_static(self, uvw, vis, weights, freq_hz, grid, mode: int = WS_GRID_OVERWRITE, stream=None):
+        """grid_visibilities with the workspace in the library's static device array (no allocation; see wstack.h for
+        the size limit and the sharing rule)."""
+        n_rows = int(uvw.shape[0])
+        n_chan = int(vis.shape[1]) if vis.dim() == 2 else 1
+        keep, fp = _freq(freq_hz, n_chan)
+        self._check(lib().ws_grid_visibilities_static(
+            self._h, _dev(uvw, torch.float32, "uvw"), _dev(vis, torch.complex64, "vis"),
+            _dev(weights, torch.float32, "weights"), fp, n_rows, n_chan, _dev(grid, self._c, "grid"), mode, _stream(stream)))
+        self._ws = None
 
     def bin_visibilities(self, uvw, vis, weights, freq_hz, workspace, stream=None):
         n_rows = int(uvw.shape[0])
