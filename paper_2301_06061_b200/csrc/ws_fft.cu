@@ -434,7 +434,9 @@ __device__ __forceinline__ uint32_t band_classes(const uint32_t* __restrict__ cl
     }
     return cmask;
 }
-template <int LOGN>
+// L2: the rows were written by other CTAs of the SAME launch (k_fft_cols below): read them past L1, which may hold the
+// lines as they were when a pass-1a item on this SM read them
+template <int LOGN, bool L2 = false>
 __device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float2* __restrict__ tw, float2* __restrict__ blk,
                                           uint32_t cmask, uint32_t ktx, uint32_t m0) {
     constexpr int N = 1 << LOGN, NT = N / 32;
@@ -447,7 +449,8 @@ __device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float
         const int j = w + 8 * i;
 #pragma unroll
         for (int m = 0; m < 16; ++m)
-            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? __ldcs(p + (size_t)(j + 16 * m) * N) : make_float2(0.f, 0.f);
+            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? (L2 ? __ldcg(p + (size_t)(j + 16 * m) * N) : __ldcs(p + (size_t)(j + 16 * m) * N))
+                                                    : make_float2(0.f, 0.f);
     }
     __syncthreads();          // the previous item's second stage has read `blk`
 #pragma unroll
@@ -496,6 +499,77 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
         const uint32_t cmask = band_classes<LOGN>(class_mask, ktx);
         if (cmask == 0) continue;
         colB_item<LOGN>(grid, tw, blk, cmask, ktx, m0);
+    }
+}
+
+// ---- passes 1a + 1b of the listed bands in ONE launch ---------------------------------------------------------------
+// Two launches move a band's intermediate (the classes pass 1a writes: 10.8 GB on Large) out to DRAM and back in.  Here
+// the items of both passes are handed out from ONE queue (an atomic counter) in an order that puts pass 1b of a band
+// LAG bands (COL_LAG_ITEMS items) behind its pass 1a: round r = the IA items of pass 1a of band r, then the IB items of
+// pass 1b of band r - LAG.
+// A pass-1b item waits until the band's IA pass-1a items have signalled (sync[1 + band]); by then they were handed out at
+// least LAG (IA + IB) items ago, so the wait is a formality, and what they wrote (a few bands x 2 MB) is still in L2: DRAM
+// sees the occupied tiles once on the way in and the band once on the way out.  No deadlock: only pass-1b items wait, and
+// only for items that were handed out earlier, i.e. to CTAs that are running.  sync[] is zeroed before the launch.
+constexpr uint32_t COL_LAG_ITEMS = 768;      // measured on Large (bands of 2 MB, 64 items): 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows)
+__device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__host__ __device__ constexpr bool cols_fused(int logn) { return logn >= 9 && logn <= 13; }
+template <int LOGN>
+__global__ void __launch_bounds__(CT, 2)
+k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const float2* __restrict__ tw_b,
+           const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_kb, uint32_t* __restrict__ sync) {
+    constexpr uint32_t R0 = 1u << (LOGN - 8), IA = 32, IB = R0, PER = IA + IB, LAG = COL_LAG_ITEMS / PER;
+    const uint32_t* class_mask = mask_set(masks, set_words);
+    const uint32_t* band_list = class_mask + (set_words - n_kb);
+    const uint32_t n = masks[masks[2] ? 1 : 0];                       // listed bands
+    const uint32_t lag = n < LAG ? n : LAG;
+    const uint32_t head = lag * IA, body = (n - lag) * PER, total = n * PER;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
+    __shared__ uint32_t s_q;
+    uint32_t next = 0;
+    if (threadIdx.x == 0) s_q = atomicAdd(sync, 1u);
+    __syncthreads();
+    for (;;) {
+        const uint32_t q = s_q;
+        if (q >= total) break;
+        if (threadIdx.x == 0) next = atomicAdd(sync, 1u);             // the next item, asked for now, needed at the bottom
+        bool pass_a;
+        uint32_t band, item;
+        if (q < head) {
+            pass_a = true, band = q / IA, item = q % IA;
+        } else if (q < head + body) {
+            const uint32_t r = (q - head) / PER, rem = (q - head) % PER;
+            pass_a = rem < IA;
+            band = pass_a ? lag + r : r;
+            item = pass_a ? rem : rem - IA;
+        } else {
+            pass_a = false, band = n - lag + (q - head - body) / IB, item = (q - head - body) % IB;
+        }
+        const uint32_t ktx = band_list[band];
+        if (pass_a) {
+            colA_item<LOGN>(grid, tw_a, class_mask, ktx, item);
+            __syncthreads();                                          // every thread's stores, then the signal
+            if (threadIdx.x == 0) {
+                __threadfence();
+                atomicAdd(sync + 1 + band, 1u);
+            }
+        } else {
+            const uint32_t cmask = band_classes<LOGN>(class_mask, ktx);
+            if (cmask != 0) {
+                if (threadIdx.x == 0)
+                    while (ld_acquire(sync + 1 + band) < IA) __nanosleep(200);
+                __syncthreads();
+                colB_item<LOGN, true>(grid, tw_b, blk, cmask, ktx, item);
+            }
+        }
+        __syncthreads();                                              // everybody has read s_q
+        if (threadIdx.x == 0) s_q = next;
+        __syncthreads();
     }
 }
 
@@ -1104,7 +1178,7 @@ int init_n(ws_plan* plan) {
     plan->mask_set_words = n_class + n_band + (size_t)plan->prm.n_wplanes * (N / 32);      // + the band list
     plan->mask_class_words = class_words(R0);
     plan->mask_band_words = band_words(N / 32);
-    plan->mask_words = MASK_CTRL + 2 * plan->mask_set_words;
+    plan->mask_words = MASK_CTRL + 2 * plan->mask_set_words + 8 + (size_t)plan->prm.n_wplanes * (N / 32);   // + k_fft_cols' queue and signals
     if (cudaMalloc((void**)&plan->d_twiddles, tw.size() * sizeof(float2)) != cudaSuccess ||
         cudaMalloc((void**)&plan->d_masks, plan->mask_words * sizeof(uint32_t)) != cudaSuccess)
         return WS_ERR_CUDA;
@@ -1115,6 +1189,10 @@ int init_n(ws_plan* plan) {
             cudaSuccess ||
         cudaFuncSetAttribute(k_fft_colB<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 32 * 8) != cudaSuccess)
         return WS_ERR_CUDA;
+    if constexpr (cols_fused(LOGN)) {
+        if (cudaFuncSetAttribute(k_fft_cols<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 32 * 8) != cudaSuccess)
+            return WS_ERR_CUDA;
+    }
     return WS_OK;
 }
 
@@ -1126,6 +1204,15 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
     const uint32_t sw = (uint32_t)plan->mask_set_words;
     const uint32_t nw = (uint32_t)plan->prm.n_wplanes;
     int launches = 0;
+    if constexpr (cols_fused(LOGN)) {
+        if (sparse) {          // both passes from one queue, the intermediate stays in L2
+            uint32_t* sync = (uint32_t*)plan->d_masks + MASK_CTRL + 2 * plan->mask_set_words;
+            if (cudaMemsetAsync(sync, 0, (size_t)(1 + nw * NT) * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
+            k_fft_cols<LOGN><<<(uint32_t)plan->sm_count * 2u, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_a, tw + plan->tw_off_b, cm, sw,
+                                                                                 nw * NT, sync);
+            return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
+        }
+    }
     if (R0 > 1) {
         const uint32_t n_items = nw * NT * 32u;
         const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 8u ? n_items : (uint32_t)plan->sm_count * 8u;
