@@ -401,6 +401,41 @@ __device__ __forceinline__ void colA_item(float2* __restrict__ grid, const float
     }
 }
 
+// N = 16384 inside k_fft_cols (two CTAs per SM, 128 registers): the radix-64 step of 4 rows j per item, each by two
+// warps -- one forms a + b and leaves the even outputs, the other (a - b) W_64^m and the odd ones -- so that a thread
+// holds 32 points, not 64.  Both read all 64 inputs (the second read hits L1); the barrier keeps the in-place stores of
+// one behind the loads of the other.
+__device__ __forceinline__ void colA_half_item14(float2* __restrict__ grid, const float2* __restrict__ tw,
+                                                 const uint32_t* __restrict__ class_mask, uint32_t ktx, uint32_t jq) {
+    constexpr int N = 16384, NT = N / 32;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, h = w >> 2;
+    const uint32_t tx = ktx % NT, k = ktx / NT;
+    const int j = (int)jq * 4 + (w & 3);
+    float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
+    const uint32_t m_lo = class_mask[(ktx * 8 + (jq >> 3)) * 2], m_hi = class_mask[(ktx * 8 + (jq >> 3)) * 2 + 1];
+    if ((m_lo | m_hi) == 0) return;                       // (the whole CTA: one class)
+    float2 x[32];
+#pragma unroll
+    for (int m = 0; m < 32; ++m) x[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+#pragma unroll
+    for (int m = 0; m < 32; ++m) {
+        const float2 b = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
+        x[m] = h ? mul_w64(ssub(x[m], b), m) : sadd(x[m], b);
+    }
+    __syncthreads();
+    bfly<float2, 5, false>(x);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+        const int f = 2 * brev(r, 5) + h;
+        if (f) {                                          // (h is warp-uniform)
+            const float2 tv = __ldg(tw + (f - 1) * 256 + j);
+            x[r] = emul(x[r], tv.x, tv.y);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < 32; ++r) p[(size_t)(2 * brev(r, 5) + h) * 256 * N] = x[r];
+}
+
 template <int LOGN>
 __global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
@@ -452,7 +487,7 @@ __device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float
             x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? (L2 ? __ldcg(p + (size_t)(j + 16 * m) * N) : __ldcs(p + (size_t)(j + 16 * m) * N))
                                                     : make_float2(0.f, 0.f);
     }
-    __syncthreads();          // the previous item's second stage has read `blk`
+    if (!L2) __syncthreads();          // the previous item's second stage has read `blk` (k_fft_cols: its own barrier per item)
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
         const int j = w + 8 * i;
@@ -511,18 +546,19 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 // least LAG (IA + IB) items ago, so the wait is a formality, and what they wrote (a few bands x 2 MB) is still in L2: DRAM
 // sees the occupied tiles once on the way in and the band once on the way out.  No deadlock: only pass-1b items wait, and
 // only for items that were handed out earlier, i.e. to CTAs that are running.  sync[] is zeroed before the launch.
-constexpr uint32_t COL_LAG_ITEMS = 768;      // measured on Large (bands of 2 MB, 64 items): 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows)
+constexpr uint32_t COL_LAG_ITEMS = 768;      // measured on Large (bands of 2 MB, 64 items): 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows);
+                                             // Extreme (4 MB, 128 items): 2 bands 20.4 ms, 4-6: 16.1, 12: 16.5, 24: 18.8
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     uint32_t v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__host__ __device__ constexpr bool cols_fused(int logn) { return logn >= 9 && logn <= 13; }
+__host__ __device__ constexpr bool cols_fused(int logn) { return logn >= 9 && logn <= 14; }
 template <int LOGN>
 __global__ void __launch_bounds__(CT, 2)
 k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const float2* __restrict__ tw_b,
            const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_kb, uint32_t* __restrict__ sync) {
-    constexpr uint32_t R0 = 1u << (LOGN - 8), IA = 32, IB = R0, PER = IA + IB, LAG = COL_LAG_ITEMS / PER;
+    constexpr uint32_t R0 = 1u << (LOGN - 8), IA = LOGN == 14 ? 64 : 32, IB = R0, PER = IA + IB, LAG = COL_LAG_ITEMS / PER;
     const uint32_t* class_mask = mask_set(masks, set_words);
     const uint32_t* band_list = class_mask + (set_words - n_kb);
     const uint32_t n = masks[masks[2] ? 1 : 0];                       // listed bands
@@ -530,12 +566,12 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
     const uint32_t head = lag * IA, body = (n - lag) * PER, total = n * PER;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
-    __shared__ uint32_t s_q;
+    __shared__ uint32_t s_q[2];               // the item in hand and the next one, by the parity of the iteration
     uint32_t next = 0;
-    if (threadIdx.x == 0) s_q = atomicAdd(sync, 1u);
+    if (threadIdx.x == 0) s_q[0] = atomicAdd(sync, 1u);
     __syncthreads();
-    for (;;) {
-        const uint32_t q = s_q;
+    for (uint32_t it = 0;; ++it) {
+        const uint32_t q = s_q[it & 1];
         if (q >= total) break;
         if (threadIdx.x == 0) next = atomicAdd(sync, 1u);             // the next item, asked for now, needed at the bottom
         bool pass_a;
@@ -552,7 +588,8 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
         }
         const uint32_t ktx = band_list[band];
         if (pass_a) {
-            colA_item<LOGN>(grid, tw_a, class_mask, ktx, item);
+            if constexpr (LOGN == 14) colA_half_item14(grid, tw_a, class_mask, ktx, item);
+            else colA_item<LOGN>(grid, tw_a, class_mask, ktx, item);
             __syncthreads();                                          // every thread's stores, then the signal
             if (threadIdx.x == 0) {
                 __threadfence();
@@ -567,8 +604,7 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
                 colB_item<LOGN, true>(grid, tw_b, blk, cmask, ktx, item);
             }
         }
-        __syncthreads();                                              // everybody has read s_q
-        if (threadIdx.x == 0) s_q = next;
+        if (threadIdx.x == 0) s_q[(it + 1) & 1] = next;               // (that slot was read before the previous iteration's barrier)
         __syncthreads();
     }
 }
