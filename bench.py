@@ -484,10 +484,11 @@ def main():
     # a1: inputs read once (12 B/row + 12 B/visibility), keys + perm written (4 + 4 B per binned entry), records written
     alg_bin = 12.0 * d.n_rows + 12.0 * d.n_vis + 8.0 * n_keys + 16.0 * n_records
     if own:
-        # k_grid: records read + non-empty tiles written; pass 1a: non-empty tiles read, non-empty classes written; pass 1b:
-        # those classes read, the non-empty bands written; pass 2: non-empty bands read once, image + dirty written
+        # k_grid: records read + non-empty tiles written; column passes (k_fft_cols, one launch: the classes pass 1a writes
+        # stay in L2 until pass 1b has read them): non-empty tiles read, non-empty bands written (N = 256 has pass 1b only);
+        # pass 2: non-empty bands read once, image + dirty written
         alg = {"bin": alg_bin, "k_grid_tiles": 16.0 * n_records + mesh_b * occ["tiles"],
-               "k_fft_columns": mesh_b * (occ["tiles"] + 2 * occ["classes"] + occ["bands"]),
+               "k_fft_columns": mesh_b * (occ["tiles"] + occ["bands"]),
                "k_fft_rows_wcorrect": mesh_b * occ["bands"] + 12.0 * N * N}
         times = {"bin": med[0], "k_grid_tiles": med[1], "k_fft_columns": med[2], "k_fft_rows_wcorrect": med[3]}
         # nominal FFT flops (5 n log2 n per transform) of the transforms that are not skipped, + 8 per point-plane of Horner
