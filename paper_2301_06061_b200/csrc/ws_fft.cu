@@ -401,41 +401,6 @@ __device__ __forceinline__ void colA_item(float2* __restrict__ grid, const float
     }
 }
 
-// N = 16384 inside k_fft_cols (two CTAs per SM, 128 registers): the radix-64 step of 4 rows j per item, each by two
-// warps -- one forms a + b and leaves the even outputs, the other (a - b) W_64^m and the odd ones -- so that a thread
-// holds 32 points, not 64.  Both read all 64 inputs (the second read hits L1); the barrier keeps the in-place stores of
-// one behind the loads of the other.
-__device__ __forceinline__ void colA_half_item14(float2* __restrict__ grid, const float2* __restrict__ tw,
-                                                 const uint32_t* __restrict__ class_mask, uint32_t ktx, uint32_t jq) {
-    constexpr int N = 16384, NT = N / 32;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, h = w >> 2;
-    const uint32_t tx = ktx % NT, k = ktx / NT;
-    const int j = (int)jq * 4 + (w & 3);
-    float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
-    const uint32_t m_lo = class_mask[(ktx * 8 + (jq >> 3)) * 2], m_hi = class_mask[(ktx * 8 + (jq >> 3)) * 2 + 1];
-    if ((m_lo | m_hi) == 0) return;                       // (the whole CTA: one class)
-    float2 x[32];
-#pragma unroll
-    for (int m = 0; m < 32; ++m) x[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-#pragma unroll
-    for (int m = 0; m < 32; ++m) {
-        const float2 b = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
-        x[m] = h ? mul_w64(ssub(x[m], b), m) : sadd(x[m], b);
-    }
-    __syncthreads();
-    bfly<float2, 5, false>(x);
-#pragma unroll
-    for (int r = 0; r < 32; ++r) {
-        const int f = 2 * brev(r, 5) + h;
-        if (f) {                                          // (h is warp-uniform)
-            const float2 tv = __ldg(tw + (f - 1) * 256 + j);
-            x[r] = emul(x[r], tv.x, tv.y);
-        }
-    }
-#pragma unroll
-    for (int r = 0; r < 32; ++r) p[(size_t)(2 * brev(r, 5) + h) * 256 * N] = x[r];
-}
-
 template <int LOGN>
 __global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
 k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
@@ -469,9 +434,7 @@ __device__ __forceinline__ uint32_t band_classes(const uint32_t* __restrict__ cl
     }
     return cmask;
 }
-// L2: the rows were written by other CTAs of the SAME launch (k_fft_cols below): read them past L1, which may hold the
-// lines as they were when a pass-1a item on this SM read them
-template <int LOGN, bool L2 = false>
+template <int LOGN>
 __device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float2* __restrict__ tw, float2* __restrict__ blk,
                                           uint32_t cmask, uint32_t ktx, uint32_t m0) {
     constexpr int N = 1 << LOGN, NT = N / 32;
@@ -484,10 +447,9 @@ __device__ __forceinline__ void colB_item(float2* __restrict__ grid, const float
         const int j = w + 8 * i;
 #pragma unroll
         for (int m = 0; m < 16; ++m)
-            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? (L2 ? __ldcg(p + (size_t)(j + 16 * m) * N) : __ldcs(p + (size_t)(j + 16 * m) * N))
-                                                    : make_float2(0.f, 0.f);
+            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? __ldcs(p + (size_t)(j + 16 * m) * N) : make_float2(0.f, 0.f);
     }
-    if (!L2) __syncthreads();          // the previous item's second stage has read `blk` (k_fft_cols: its own barrier per item)
+    __syncthreads();          // the previous item's second stage has read `blk`
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
         const int j = w + 8 * i;
@@ -546,7 +508,8 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 // least LAG (IA + IB) items ago, so the wait is a formality, and what they wrote (a few bands x 2 MB) is still in L2: DRAM
 // sees the occupied tiles once on the way in and the band once on the way out.  No deadlock: only pass-1b items wait, and
 // only for items that were handed out earlier, i.e. to CTAs that are running.  sync[] is zeroed before the launch.
-constexpr uint32_t COL_LAG_ITEMS = 768;      // measured on Large (bands of 2 MB, 64 items): 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows);
+constexpr uint32_t COL_LAG_ITEMS = 768;      // in items of 64 KB (8-warp CTAs: x 8 / W for W warps).  Measured on Large (bands of 2 MB, 64 such
+                                             // items) with 8-warp CTAs: 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows);
                                              // Extreme (4 MB, 128 items): 2 bands 20.4 ms, 4-6: 16.1, 12: 16.5, 24: 18.8
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     uint32_t v;
@@ -554,18 +517,120 @@ __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     return v;
 }
 __host__ __device__ constexpr bool cols_fused(int logn) { return logn >= 9 && logn <= 14; }
-template <int LOGN>
-__global__ void __launch_bounds__(CT, 2)
+constexpr int COLS_W = 4;                 // warps per CTA of k_fft_cols
+// CTAs of W = 4 warps, four per SM (128 registers per thread either way), with items to match -- pass 1a: W rows j of the band
+// (N = 16384: W / 2 rows, two warps each: one forms a + b and leaves the even outputs of the radix-64 step, the other
+// (a - b) W_64^m and the odd ones, so that a thread holds 32 points, not 64; both read all 64 inputs, the second read hits L1,
+// and the barrier keeps the in-place stores of one behind the loads of the other); pass 1b: 256 rows x 4 W columns.  Every
+// item is a load phase, a compute phase and a store phase with barriers between them; four small CTAs whose phases fall at
+// different times keep an SM busier than two large ones (measured, Large / Extreme: W = 8: 5.74 / 16.0 ms, W = 4: 5.26 / 14.2,
+// W = 2: 5.87 / 15.6 -- 64-byte row segments).
+template <int LOGN, int W>
+__device__ __forceinline__ void colsA_item(float2* __restrict__ grid, const float2* __restrict__ tw,
+                                           const uint32_t* __restrict__ class_mask, uint32_t ktx, uint32_t jq) {
+    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t tx = ktx % NT, k = ktx / NT;
+    if constexpr (LOGN == 14) {
+        const int h = w / (W / 2), j = (int)jq * (W / 2) + (w % (W / 2));
+        float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
+        const uint32_t cls = jq / (64 / W);
+        const uint32_t m_lo = class_mask[(ktx * 8 + cls) * 2], m_hi = class_mask[(ktx * 8 + cls) * 2 + 1];
+        if ((m_lo | m_hi) == 0) return;                   // (the whole CTA: one class)
+        float2 x[32];
+#pragma unroll
+        for (int m = 0; m < 32; ++m) x[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+#pragma unroll
+        for (int m = 0; m < 32; ++m) {
+            const float2 b = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
+            x[m] = h ? mul_w64(ssub(x[m], b), m) : sadd(x[m], b);
+        }
+        __syncthreads();
+        bfly<float2, 5, false>(x);
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const int f = 2 * brev(r, 5) + h;
+            if (f) {
+                const float2 tv = __ldg(tw + (f - 1) * 256 + j);
+                x[r] = emul(x[r], tv.x, tv.y);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 32; ++r) p[(size_t)(2 * brev(r, 5) + h) * 256 * N] = x[r];
+    } else {
+        const int j = (int)jq * W + w;
+        float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
+        const uint32_t mask = class_mask[ktx * 8 + jq / (32 / W)];
+        if (mask == 0) return;
+        float2 x[R0];
+#pragma unroll
+        for (int m = 0; m < R0; ++m) x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
+        bfly<float2, LR0, false>(x);
+#pragma unroll
+        for (int r = 1; r < R0; ++r) {
+            const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
+            x[r] = emul(x[r], tv.x, tv.y);
+        }
+#pragma unroll
+        for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
+    }
+}
+// pass 1b of 4 W columns of a band block: lane = (column c, jj), warp w: rows j = (32 / COLS) w + jj + 8 i, i < 2, as in colB_item;
+// the rows were written by other CTAs of the SAME launch: read them past L1 (ld.global.cg), which may hold the lines as they
+// were when a pass-1a item on this SM read them
+template <int LOGN, int W>
+__device__ __forceinline__ void colsB_item(float2* __restrict__ grid, const float2* __restrict__ tw, float2* __restrict__ blk,
+                                           uint32_t cmask, uint32_t ktx, uint32_t item) {
+    constexpr int N = 1 << LOGN, NT = N / 32, COLS = 4 * W, JPW = 32 / COLS, PARTS = 32 / COLS;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, c = lane & (COLS - 1), jj = lane / COLS;
+    const uint32_t tx = ktx % NT, k = ktx / NT, m0 = item / PARTS, h = item % PARTS;
+    float2* p = grid + ((size_t)k * N + m0 * 256) * N + tx * 32 + h * COLS + c;
+    float2 x[32];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int j = JPW * w + jj + 8 * i;
+#pragma unroll
+        for (int m = 0; m < 16; ++m)
+            x[i * 16 + m] = (cmask >> (m >> 1)) & 1 ? __ldcg(p + (size_t)(j + 16 * m) * N) : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int j = JPW * w + jj + 8 * i;
+        bfly<float2, 4, false>(x + i * 16);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            float2 v = x[i * 16 + r];
+            if (r) {
+                const float2 tv = __ldg(tw + (brev(r, 4) - 1) * 16 + j);
+                v = emul(v, tv.x, tv.y);
+            }
+            blk[(j + 16 * brev(r, 4)) * COLS + c] = v;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int b = JPW * w + jj + 8 * i;
+#pragma unroll
+        for (int m = 0; m < 16; ++m) x[i * 16 + m] = blk[(16 * b + m) * COLS + c];
+        bfly<float2, 4, false>(x + i * 16);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) __stcs(p + (size_t)(b + 16 * brev(r, 4)) * N, x[i * 16 + r]);
+    }
+}
+
+template <int LOGN, int W>
+__global__ void __launch_bounds__(32 * W, 16 / W)
 k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const float2* __restrict__ tw_b,
-           const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_kb, uint32_t* __restrict__ sync) {
-    constexpr uint32_t R0 = 1u << (LOGN - 8), IA = LOGN == 14 ? 64 : 32, IB = R0, PER = IA + IB, LAG = COL_LAG_ITEMS / PER;
+            const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_kb, uint32_t* __restrict__ sync) {
+    constexpr uint32_t R0 = 1u << (LOGN - 8), IA = (LOGN == 14 ? 512 : 256) / W, IB = R0 * 8 / W, PER = IA + IB, LAG = (8 / W) * COL_LAG_ITEMS / PER;
     const uint32_t* class_mask = mask_set(masks, set_words);
     const uint32_t* band_list = class_mask + (set_words - n_kb);
     const uint32_t n = masks[masks[2] ? 1 : 0];                       // listed bands
     const uint32_t lag = n < LAG ? n : LAG;
     const uint32_t head = lag * IA, body = (n - lag) * PER, total = n * PER;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2* blk = (float2*)smem_raw;          // [256 rows][32 columns]
+    float2* blk = (float2*)smem_raw;          // [256 rows][4 W columns]
     __shared__ uint32_t s_q[2];               // the item in hand and the next one, by the parity of the iteration
     uint32_t next = 0;
     if (threadIdx.x == 0) s_q[0] = atomicAdd(sync, 1u);
@@ -573,7 +638,7 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
     for (uint32_t it = 0;; ++it) {
         const uint32_t q = s_q[it & 1];
         if (q >= total) break;
-        if (threadIdx.x == 0) next = atomicAdd(sync, 1u);             // the next item, asked for now, needed at the bottom
+        if (threadIdx.x == 0) next = atomicAdd(sync, 1u);
         bool pass_a;
         uint32_t band, item;
         if (q < head) {
@@ -588,9 +653,8 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
         }
         const uint32_t ktx = band_list[band];
         if (pass_a) {
-            if constexpr (LOGN == 14) colA_half_item14(grid, tw_a, class_mask, ktx, item);
-            else colA_item<LOGN>(grid, tw_a, class_mask, ktx, item);
-            __syncthreads();                                          // every thread's stores, then the signal
+            colsA_item<LOGN, W>(grid, tw_a, class_mask, ktx, item);
+            __syncthreads();
             if (threadIdx.x == 0) {
                 __threadfence();
                 atomicAdd(sync + 1 + band, 1u);
@@ -601,10 +665,10 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
                 if (threadIdx.x == 0)
                     while (ld_acquire(sync + 1 + band) < IA) __nanosleep(200);
                 __syncthreads();
-                colB_item<LOGN, true>(grid, tw_b, blk, cmask, ktx, item);
+                colsB_item<LOGN, W>(grid, tw_b, blk, cmask, ktx, item);
             }
         }
-        if (threadIdx.x == 0) s_q[(it + 1) & 1] = next;               // (that slot was read before the previous iteration's barrier)
+        if (threadIdx.x == 0) s_q[(it + 1) & 1] = next;
         __syncthreads();
     }
 }
@@ -1226,7 +1290,7 @@ int init_n(ws_plan* plan) {
         cudaFuncSetAttribute(k_fft_colB<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 32 * 8) != cudaSuccess)
         return WS_ERR_CUDA;
     if constexpr (cols_fused(LOGN)) {
-        if (cudaFuncSetAttribute(k_fft_cols<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 32 * 8) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_fft_cols<LOGN, COLS_W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 4 * COLS_W * 8) != cudaSuccess)
             return WS_ERR_CUDA;
     }
     return WS_OK;
@@ -1244,8 +1308,8 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
         if (sparse) {          // both passes from one queue, the intermediate stays in L2
             uint32_t* sync = (uint32_t*)plan->d_masks + MASK_CTRL + 2 * plan->mask_set_words;
             if (cudaMemsetAsync(sync, 0, (size_t)(1 + nw * NT) * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
-            k_fft_cols<LOGN><<<(uint32_t)plan->sm_count * 2u, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_a, tw + plan->tw_off_b, cm, sw,
-                                                                                 nw * NT, sync);
+            k_fft_cols<LOGN, COLS_W><<<(uint32_t)plan->sm_count * (16u / COLS_W), 32 * COLS_W, 256 * 4 * COLS_W * 8, st>>>(
+                grid, tw + plan->tw_off_a, tw + plan->tw_off_b, cm, sw, nw * NT, sync);
             return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
         }
     }
