@@ -143,6 +143,31 @@ def test_own_fft_fused_wcorrect_on_arbitrary_planes(oracle, n_pix, n_wplanes):
     assert np.array_equal(dirty.cpu().numpy(), image.cpu().numpy().real)
 
 
+@pytest.mark.parametrize("n_pix,n_wplanes,n_rows", [(512, 1, 3), (1024, 2, 5), (2048, 3, 40), (4096, 2, 2000)])
+def test_sparse_fft_with_few_and_many_listed_bands(oracle, n_pix, n_wplanes, n_rows):
+    # k_fft_cols hands pass 1b of a band out a fixed number of bands behind its pass 1a: fewer listed bands than that lag
+    # (a handful of visibilities), and more (thousands), against the oracle -- the image of the timed path (WS_GRID_SPARSE +
+    # occupancy), from a NaN-filled mesh, twice in a row on the same plan (the queue and the signals restart per launch)
+    import paper_2301_06061_b200 as ws
+    d = make_random_dataset(900 + n_rows, n_rows, 2, n_pix, n_wplanes, 7, wavelengths=False, fill=0.9, w_span=20.0, cell_rad=0.6 / n_pix)
+    plan = U.make_plan(d)
+    assert plan.fft_is_own
+    prm = U.oracle_params(oracle, d, plan.tile)
+    D = oracle.dirty_image(prm, d.uvw.numpy(), d.vis.numpy(), d.weights.numpy(), d.freqs_hz)
+    dev = d.to("cuda")
+    grid, image = plan.alloc_grid(), plan.alloc_image()
+    wsp = plan.alloc_workspace(d.n_vis)
+    for _ in range(2):
+        grid.fill_(float("nan"))
+        image.fill_(float("nan"))
+        plan.grid_visibilities(dev.uvw, dev.vis, dev.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_SPARSE)
+        plan.fft_wcorrect(grid, image, wsp, accumulate=False, dirty=None, fft_flags=ws.WS_FFT_USE_OCCUPANCY)
+        plan.async_status()
+        U.assert_close(image.cpu().numpy(), D, "image")
+    occ = plan.occupancy()
+    print("bands listed:", occ["bands"] * n_wplanes * (n_pix // 32))
+
+
 def test_library_fft_flag_and_occupancy_rules(oracle):
     import paper_2301_06061_b200 as ws
     d = make_random_dataset(31, 3000, 1, 256, 4, 7, fill=0.7, w_span=30.0, cell_rad=2e-3)
