@@ -77,7 +77,7 @@ extern "C" {
                                    if the library cannot know) */
 
 /* ws_params.flags */
-#define WS_FLAG_LIBRARY_FFT 1u /* a3 through cuFFT even where the library's own two-pass FFT exists (N = 2^8..2^13) */
+#define WS_FLAG_LIBRARY_FFT 1u /* a3 through cuFFT even where the library's own two-pass FFT exists (N = 2^8..2^14) */
 #define WS_FLAG_NO_TRANSPOSE 2u /* WS_GRID_SPARSE keeps the [k][v][u] orientation (default: it may store the mesh transposed) */
 
 #define WS_FLAG_TRACK_SUMWT 4u  /* every gridding call also sums the weights of the visibilities it kept (one extra
