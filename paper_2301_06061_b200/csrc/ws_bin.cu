@@ -230,21 +230,23 @@ k_scatter(const __grid_constant__ WsChanConsts cc, const __grid_constant__ WsGeo
     const int lane = threadIdx.x & 31;
     Placed pl;
     bool kept = false;
+    float2 v = make_float2(0.f, 0.f);
+    float w = 0.f;
     if (m < n_vis) {
         uint32_t row, c;
         row_chan(m, n_chan, chan_shift, row, c);
         const float* p = uvw + 3ull * row;
-        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), s_su[c], s_sw[c], pl);
-    }
-    uint32_t home = 0xFFFFFFFFu;
-    int lx = 0, ly = 0;
-    float2 v = make_float2(0.f, 0.f);
-    float w = 0.f;
-    if (kept) {
+        // the value and the weight are asked for together with the position, not after the drop test: the kernel is bound by
+        // its chain of round trips (position -> value -> slot), and dropped visibilities are rare
         if (vis) {                                  // NULL: bins for the degridder, the records carry positions only
             v = __ldcs(vis + m);
             w = wt ? __ldcs(wt + m) : 1.0f;         // NULL: pre-summed rows, the weights are already inside
         }
+        kept = place(cc, g, __ldg(p), __ldg(p + 1), __ldg(p + 2), s_su[c], s_sw[c], pl);
+    }
+    uint32_t home = 0xFFFFFFFFu;
+    int lx = 0, ly = 0;
+    if (kept) {
         lx = pl.i0 & (T - 1); ly = pl.j0 & (T - 1);
         home = bin_of(g, pl.k, pl.j0 >> T_LOG2, pl.i0 >> T_LOG2);
     }
