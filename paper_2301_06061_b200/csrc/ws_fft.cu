@@ -3,13 +3,16 @@
 //
 // The paper leaves the FFT to FFTW on the CPU (55-80 % of its GPU runs) and names a GPU FFT as
 // future work (:459).  A library 2-D FFT of an 8192^2 plane reads and writes the mesh three times (rows, and the
-// columns in two steps), and a4 reads it a fourth time.  Here, for N = R0 * 256 (N = 2^8 .. 2^13):
-//   pass 1a k_fft_colA   columns, first radix-R0 step across the N/R0-spaced rows, in registers: a warp = 32
+// columns in two steps), and a4 reads it a fourth time.  Here, for N = R0 * 256 (N = 2^8 .. 2^14):
+//   pass 1a              columns, first radix-R0 step across the N/R0-spaced rows, in registers: a warp = 32
 //                        adjacent columns, so every access is a whole 256-byte row segment; twiddles are
 //                        warp-uniform; no shared memory;
-//   pass 1b k_fft_colB   columns, the remaining 256-point transforms: a CTA holds a [256 rows x 32 columns] block
+//   pass 1b              columns, the remaining 256-point transforms of a [256 rows x 16 columns] block per item
 //                        (lane = column: conflict-free, coalesced), radix 16 x 16, in place.  Row position
 //                        256 m0 + f of the mesh then holds v-frequency m0 + R0 f;
+//                        both in ONE launch, k_fft_cols: items of the two passes from one queue, pass 1b of a band a
+//                        few bands behind its pass 1a, so that what pass 1a writes is read back from L2
+//                        (N = 256: pass 1b alone, k_fft_colB);
 //   pass 2  k_fft_rows   rows.  A CTA owns 8192 contiguous points (whole rows) of EVERY plane: bulk copies (TMA,
 //                        cp.async.bulk + mbarrier) land the next plane's rows in shared memory while the current one
 //                        is transformed (radix 32/16/8 in registers, in-place exchanges through padded shared memory).
@@ -336,87 +339,6 @@ k_fft_masks_degrid(const uint32_t* __restrict__ bin_start, int nt, int r0, uint3
 // the orientation of a WS_GRID_SPARSE mesh: transposed iff that leaves fewer bands (allow = 0: as the header says)
 __global__ void k_fft_orient(uint32_t* __restrict__ masks, int allow) { masks[2] = allow && masks[1] < masks[0] ? 1u : 0u; }
 
-// ---- pass 1a: first radix-R0 step of the column transforms ------------------------------------------------------
-// Thread = (column, row j of the first 256-row block): x[m] = row j + 256 m, m < R0; Y[m'] W_N^(j m') goes back to
-// row j + 256 m'.  A warp = 32 adjacent columns at one j, a CTA = 8 consecutive j.
-template <int LOGN>
-__device__ __forceinline__ void colA_item(float2* __restrict__ grid, const float2* __restrict__ tw,
-                                          const uint32_t* __restrict__ class_mask, uint32_t ktx, uint32_t jb) {
-    constexpr int N = 1 << LOGN, LR0 = LOGN - 8, R0 = 1 << LR0, NT = N / 32, CW = class_words(R0);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint32_t tx = ktx % NT, k = ktx / NT;
-    const int j = (int)jb * 8 + w;
-    float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
-    if constexpr (LOGN == 14) {
-        // radix 64 = one radix-2 step over the two halves of the column, then radix 32 on the sum and on the
-        // (twiddled) difference: a[r] = Y[2 brev5(r)], b[r] = Y[2 brev5(r) + 1]
-        const uint32_t m_lo = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW] : 0xFFFFFFFFu;
-        const uint32_t m_hi = class_mask ? class_mask[(ktx * 8 + (jb >> 2)) * CW + 1] : 0xFFFFFFFFu;
-        if ((m_lo | m_hi) == 0) return;
-        float2 a[32], b[32];
-#pragma unroll
-        for (int m = 0; m < 32; ++m) {
-            a[m] = (m_lo >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-            b[m] = (m_hi >> m) & 1 ? __ldcs(p + (size_t)(m + 32) * 256 * N) : make_float2(0.f, 0.f);
-        }
-#pragma unroll
-        for (int m = 0; m < 32; ++m) {
-            const float2 d = ssub(a[m], b[m]);
-            a[m] = sadd(a[m], b[m]);
-            b[m] = mul_w64(d, m);
-        }
-        bfly<float2, 5, false>(a);
-        bfly<float2, 5, false>(b);
-#pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            const int f0 = 2 * brev(r, 5);
-            if (f0) {
-                const float2 tv = __ldg(tw + (f0 - 1) * 256 + j);
-                a[r] = emul(a[r], tv.x, tv.y);
-            }
-            const float2 tu = __ldg(tw + f0 * 256 + j);
-            b[r] = emul(b[r], tu.x, tu.y);
-        }
-#pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            const int f0 = 2 * brev(r, 5);
-            p[(size_t)f0 * 256 * N] = a[r];
-            p[(size_t)(f0 + 1) * 256 * N] = b[r];
-        }
-    } else {
-        const uint32_t mask = class_mask ? class_mask[ktx * 8 + (jb >> 2)] : 0xFFFFFFFFu;
-        if (mask == 0) return;
-        float2 x[R0];
-#pragma unroll
-        for (int m = 0; m < R0; ++m)
-            x[m] = (mask >> m) & 1 ? __ldcs(p + (size_t)m * 256 * N) : make_float2(0.f, 0.f);
-        bfly<float2, LR0, false>(x);
-#pragma unroll
-        for (int r = 1; r < R0; ++r) {
-            const float2 tv = __ldg(tw + (brev(r, LR0) - 1) * 256 + j);
-            x[r] = emul(x[r], tv.x, tv.y);
-        }
-#pragma unroll
-        for (int r = 0; r < R0; ++r) p[(size_t)brev(r, LR0) * 256 * N] = x[r];
-    }
-}
-
-template <int LOGN>
-__global__ void __launch_bounds__(CT, LOGN == 14 ? 1 : 2)
-k_fft_colA(float2* __restrict__ grid, const float2* __restrict__ tw, const uint32_t* __restrict__ masks,
-           uint32_t set_words, uint32_t n_items) {
-    if (!masks) {
-        for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x)
-            colA_item<LOGN>(grid, tw, nullptr, item >> 5, item & 31);     // 32 groups of 8 rows per (plane, band)
-        return;
-    }
-    const uint32_t* class_mask = mask_set(masks, set_words);
-    const uint32_t* band_list = class_mask + (set_words - n_items / 32u);  // the non-empty (plane, band) pairs
-    const uint32_t n_list = masks[masks[2] ? 1 : 0] * 32u;
-    for (uint32_t item = blockIdx.x; item < n_list; item += gridDim.x)
-        colA_item<LOGN>(grid, tw, class_mask, band_list[item >> 5], item & 31);
-}
-
 // ---- pass 1b: the 256-point column transforms -------------------------------------------------------------------
 // Item = (plane, column band tx, block m0 of 256 rows).  Warp w, lane = column.  Stage 1: j in {w, w + 8}, rows
 // j + 16 m; stage 2: blocks b in {w, w + 8}, rows 16 b + m; frequency f = b + 16 m' is stored at row 256 m0 + f.
@@ -535,7 +457,8 @@ __device__ __forceinline__ void colsA_item(float2* __restrict__ grid, const floa
         const int h = w / (W / 2), j = (int)jq * (W / 2) + (w % (W / 2));
         float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
         const uint32_t cls = jq / (64 / W);
-        const uint32_t m_lo = class_mask[(ktx * 8 + cls) * 2], m_hi = class_mask[(ktx * 8 + cls) * 2 + 1];
+        const uint32_t m_lo = class_mask ? class_mask[(ktx * 8 + cls) * 2] : 0xFFFFFFFFu;      // (NULL: a dense mesh)
+        const uint32_t m_hi = class_mask ? class_mask[(ktx * 8 + cls) * 2 + 1] : 0xFFFFFFFFu;
         if ((m_lo | m_hi) == 0) return;                   // (the whole CTA: one class)
         float2 x[32];
 #pragma unroll
@@ -560,7 +483,7 @@ __device__ __forceinline__ void colsA_item(float2* __restrict__ grid, const floa
     } else {
         const int j = (int)jq * W + w;
         float2* p = grid + ((size_t)k * N + j) * N + tx * 32 + lane;
-        const uint32_t mask = class_mask[ktx * 8 + jq / (32 / W)];
+        const uint32_t mask = class_mask ? class_mask[ktx * 8 + jq / (32 / W)] : 0xFFFFFFFFu;
         if (mask == 0) return;
         float2 x[R0];
 #pragma unroll
@@ -624,9 +547,10 @@ __global__ void __launch_bounds__(32 * W, 16 / W)
 k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const float2* __restrict__ tw_b,
             const uint32_t* __restrict__ masks, uint32_t set_words, uint32_t n_kb, uint32_t* __restrict__ sync) {
     constexpr uint32_t R0 = 1u << (LOGN - 8), IA = (LOGN == 14 ? 512 : 256) / W, IB = R0 * 8 / W, PER = IA + IB, LAG = (8 / W) * COL_LAG_ITEMS / PER;
-    const uint32_t* class_mask = mask_set(masks, set_words);
-    const uint32_t* band_list = class_mask + (set_words - n_kb);
-    const uint32_t n = masks[masks[2] ? 1 : 0];                       // listed bands
+    // masks == NULL: a dense mesh, every band of every plane in storage order
+    const uint32_t* class_mask = masks ? mask_set(masks, set_words) : nullptr;
+    const uint32_t* band_list = masks ? class_mask + (set_words - n_kb) : nullptr;
+    const uint32_t n = masks ? masks[masks[2] ? 1 : 0] : n_kb;       // listed bands
     const uint32_t lag = n < LAG ? n : LAG;
     const uint32_t head = lag * IA, body = (n - lag) * PER, total = n * PER;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -651,7 +575,7 @@ k_fft_cols(float2* __restrict__ grid, const float2* __restrict__ tw_a, const flo
         } else {
             pass_a = false, band = n - lag + (q - head - body) / IB, item = (q - head - body) % IB;
         }
-        const uint32_t ktx = band_list[band];
+        const uint32_t ktx = band_list ? band_list[band] : band;
         if (pass_a) {
             colsA_item<LOGN, W>(grid, tw_a, class_mask, ktx, item);
             __syncthreads();
@@ -1305,7 +1229,7 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
     const uint32_t nw = (uint32_t)plan->prm.n_wplanes;
     int launches = 0;
     if constexpr (cols_fused(LOGN)) {
-        if (sparse) {          // both passes from one queue, the intermediate stays in L2
+        if (plan->d_masks) {   // both passes from one queue, the intermediate stays in L2 (cm == NULL: every band)
             uint32_t* sync = (uint32_t*)plan->d_masks + MASK_CTRL + 2 * plan->mask_set_words;
             if (cudaMemsetAsync(sync, 0, (size_t)(1 + nw * NT) * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;
             k_fft_cols<LOGN, COLS_W><<<(uint32_t)plan->sm_count * (16u / COLS_W), 32 * COLS_W, 256 * 4 * COLS_W * 8, st>>>(
@@ -1313,12 +1237,7 @@ int launch_cols_n(ws_plan* plan, float2* grid, bool sparse, cudaStream_t st) {
             return cudaGetLastError() == cudaSuccess ? 1 : WS_ERR_CUDA;
         }
     }
-    if (R0 > 1) {
-        const uint32_t n_items = nw * NT * 32u;
-        const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 8u ? n_items : (uint32_t)plan->sm_count * 8u;
-        k_fft_colA<LOGN><<<ctas, CT, 0, st>>>(grid, tw + plan->tw_off_a, cm, sw, n_items);
-        ++launches;
-    }
+    if (R0 > 1) return WS_ERR_UNSUPPORTED;          // (N >= 512 always goes through k_fft_cols: the plan owns the masks buffer)
     const uint32_t n_items = nw * NT * (uint32_t)R0;
     const uint32_t ctas = n_items < (uint32_t)plan->sm_count * 2u ? n_items : (uint32_t)plan->sm_count * 2u;
     k_fft_colB<LOGN><<<ctas, CT, 256 * 32 * 8, st>>>(grid, tw + plan->tw_off_b, cm, sw, n_items);
