@@ -327,7 +327,7 @@ template <int S, bool KB>
 __global__ void __launch_bounds__(TileCfg<S>::THREADS, 1)
 k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ occ_start,
        const uint32_t* __restrict__ light, const uint4* __restrict__ items, const float4* __restrict__ records,
-       float2* __restrict__ grid, int mode, const WsStatus* __restrict__ status, const uint32_t* __restrict__ orient) {
+       float2* __restrict__ grid, int mode, WsStatus* __restrict__ status, const uint32_t* __restrict__ orient) {
     using C = TileCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -353,21 +353,26 @@ k_grid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start,
     if (mode != WS_GRID_OVERWRITE) {
         // only the listed bins matter (k_prepare_heavy: non-empty, not heavy); 96 % of the tiles of Large hold nothing, and
         // walking them costs every warp a dependent load each -- again in every call of a chunked run
-        const uint32_t n_light = status->n_light;
-        const uint32_t my_light = gw < n_light ? (n_light - gw + n_warps - 1) / n_warps : 0u;
-        const uint32_t lgap = my_items ? max(1u, my_light / my_items) : 0xFFFFFFFFu;
-        for (uint32_t i = gw; i < n_light; i += n_warps) {
-            if (it < n_items && since >= lgap) {
-                do_item();
-                since = 0;
+        // The warps take their work from one counter: the chunks of the heavy bins first (1024 records each), then the
+        // listed bins (1 .. 1024 records), so that the short ones fill the end of the kernel evenly.
+        const uint32_t total = n_items + status->n_light;
+        for (;;) {
+            uint32_t q = 0;
+            if (lane == 0) q = atomicAdd(&status->queue, 1u);
+            q = __shfl_sync(0xffffffffu, q, 0);
+            if (q >= total) break;
+            uint32_t bin, lo, hi;
+            if (q < n_items) {
+                const uint4 w = items[q];
+                bin = w.x, lo = w.y, hi = w.z;
+            } else {
+                bin = light[q - n_items];
+                lo = bin_start[bin], hi = bin_start[bin + 1];
             }
-            ++since;
-            const uint32_t bin = light[i];
             zero_tile<S>(sm.tile, lane);
-            accumulate_records<S, KB>(g, records, bin_start[bin], bin_start[bin + 1], sm, lane);
+            accumulate_records<S, KB>(g, records, lo, hi, sm, lane);
             flush_ring<S>(g, sm, grid, bin, tr, lane);
         }
-        while (it < n_items) do_item();
         return;
     }
     for (uint32_t bin = gw; bin < g.n_bins; bin += n_warps) {
@@ -406,7 +411,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
     uint4* items = (uint4*)(ws + L.off_items);
     const WsGeom& g = plan->geom;
     uint32_t* light = (uint32_t*)(ws + L.off_cursor_home);        // (the scatter's cursors are spent)
-    if (cudaMemsetAsync(&status->n_items, 0, 2 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light
+    if (cudaMemsetAsync(&status->n_items, 0, 3 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light, queue
     k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, bin_start, occ_start, 1, light, items, L.item_capacity, status, grid,
                                                           mode, orient, mv);
     k_grid<S, KB><<<plan->sm_count, C::THREADS, smem, st>>>(g, bin_start, occ_start, light, items, records, grid, mode, status, orient);
@@ -420,7 +425,7 @@ int launch_s(ws_plan* plan, const WsLayout& L, char* ws, float2* grid, int mode,
 // used by the degridder on the home lists.
 int ws_launch_items(ws_plan* plan, const uint32_t* starts, uint32_t* light, uint4* items, uint32_t item_capacity, cudaStream_t st) {
     const WsGeom& g = plan->geom;
-    if (cudaMemsetAsync(&plan->d_status->n_items, 0, 2 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light
+    if (cudaMemsetAsync(&plan->d_status->n_items, 0, 3 * sizeof(uint32_t), st) != cudaSuccess) return WS_ERR_CUDA;    // n_items, n_light, queue
     k_prepare_heavy<<<(g.n_bins + 255) / 256, 256, 0, st>>>(g, starts, starts, 0, light, items, item_capacity, plan->d_status, nullptr,
                                                           WS_GRID_ACCUMULATE, nullptr, WsMaskView{nullptr, 0u, 1});
     if (cudaGetLastError() != cudaSuccess) return WS_ERR_CUDA;

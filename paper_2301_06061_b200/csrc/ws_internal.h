@@ -70,9 +70,10 @@ struct WsStatus {                               // device-side, 64 bytes
     uint32_t n_records;                         // records incl. halo copies
     uint32_t n_items;                           // heavy chunks queued
     uint32_t n_light;                           // non-empty bins that are not heavy, listed for the gridder
+    uint32_t queue;                             // k_grid's work counter: heavy chunks first, then the listed bins (zeroed with the two above)
     uint32_t overflow;                          // 1: record or item capacity exceeded, gridding skipped (cleared by every binning call)
     uint32_t sticky_overflow;                   // ... of ANY call since the last ws_async_status (which clears it)
-    uint32_t pad[10];
+    uint32_t pad[9];
 };
 
 struct ws_plan {
