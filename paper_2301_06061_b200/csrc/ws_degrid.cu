@@ -157,13 +157,13 @@ __device__ __forceinline__ void gather(const WsGeom& g, const float4* __restrict
     __syncwarp();
 }
 
-// Persistent kernel: warp w takes the listed (non-empty, not heavy) bins w, w + W, ... and the chunks of the heavy bins (items), interleaved.
+// Persistent kernel: the warps take the chunks of the heavy bins (items) and then the listed (non-empty, not heavy) bins from one counter.
 template <int S, bool KB>
 __global__ void __launch_bounds__(DgCfg<S>::THREADS, 2)
 k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ halo_start,
          const uint32_t* __restrict__ light, const uint4* __restrict__ items, const float4* __restrict__ records, const uint32_t* __restrict__ perm,
          const float2* __restrict__ planes, float2* __restrict__ vis_out, float scale, int accumulate,
-         const WsStatus* __restrict__ status, int xf_lr0, const uint32_t* __restrict__ orient) {
+         WsStatus* __restrict__ status, int xf_lr0, const uint32_t* __restrict__ orient) {
     using C = DgCfg<S>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -171,32 +171,23 @@ k_degrid(const __grid_constant__ WsGeom g, const uint32_t* __restrict__ bin_star
     if (status->overflow) return;
     const bool tr = orient && *orient;           // planes stored [k][u][v] (ws_predict_visibilities may choose so)
     const uint32_t n_items = status->n_items;
-    const uint32_t n_warps = gridDim.x * C::WARPS;
-    const uint32_t gw = blockIdx.x * C::WARPS + wid;
-    const uint32_t n_light = status->n_light;    // the non-empty bins that are not heavy, listed by k_prepare_heavy
-    const uint32_t my_tiles = gw < n_light ? (n_light - gw + n_warps - 1) / n_warps : 0u;
-    const uint32_t my_items = gw < n_items ? (n_items - gw + n_warps - 1) / n_warps : 0u;
-    const uint32_t gap = my_items ? max(1u, my_tiles / my_items) : 0xFFFFFFFFu;
-    uint32_t it = gw, since = 0;
-
-    auto do_item = [&]() {
-        const uint4 w = items[it];
-        it += n_warps;
-        load_region<S>(g, planes, w.x, region, lane, xf_lr0, tr);
-        gather<S, KB>(g, records, perm, w.y, w.z, halo_start[w.x], region, vis_out, scale, accumulate, lane);
-    };
-
-    for (uint32_t i = gw; i < n_light; i += n_warps) {
-        if (it < n_items && since >= gap) {
-            do_item();
-            since = 0;
+    const uint32_t total = n_items + status->n_light;    // the non-empty bins that are not heavy, listed by k_prepare_heavy
+    for (;;) {
+        uint32_t q = 0;
+        if (lane == 0) q = atomicAdd(&status->queue, 1u);
+        q = __shfl_sync(0xffffffffu, q, 0);
+        if (q >= total) break;
+        uint32_t bin, lo, hi;
+        if (q < n_items) {
+            const uint4 w = items[q];
+            bin = w.x, lo = w.y, hi = w.z;
+        } else {
+            bin = light[q - n_items];
+            lo = bin_start[bin], hi = bin_start[bin + 1];
         }
-        ++since;
-        const uint32_t bin = light[i];
         load_region<S>(g, planes, bin, region, lane, xf_lr0, tr);
-        gather<S, KB>(g, records, perm, bin_start[bin], bin_start[bin + 1], halo_start[bin], region, vis_out, scale, accumulate, lane);
+        gather<S, KB>(g, records, perm, lo, hi, halo_start[bin], region, vis_out, scale, accumulate, lane);
     }
-    while (it < n_items) do_item();
 }
 
 template <int S, bool KB>
