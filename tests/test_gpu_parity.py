@@ -168,6 +168,31 @@ def test_sparse_fft_with_few_and_many_listed_bands(oracle, n_pix, n_wplanes, n_r
     print("bands listed:", occ["bands"] * n_wplanes * (n_pix // 32))
 
 
+def test_column_passes_are_bitwise_repeatable():
+    # k_fft_cols couples its two passes through a work queue and per-band signal counters; its arithmetic does not depend on
+    # the order the items are taken in, so repeated launches on the same mesh must agree bit for bit -- a pass-1b item that
+    # read a row before pass 1a had written it would show up here.  Medium: 4096^2 x 32, sparse and dense.
+    import paper_2301_06061_b200 as ws
+    d = make_dataset(get_config("medium"), device="cuda")
+    plan = ws.Plan(d.n_pix, d.n_wplanes, d.support, d.cell_rad, d.w_min, d.w_max, sigma=d.sigma_cells)
+    grid = plan.alloc_grid()
+    wsp = plan.alloc_workspace(d.n_vis)
+    grid.zero_()
+    plan.grid_visibilities(d.uvw, d.vis, d.weights, d.freqs_hz, grid, wsp, mode=ws.WS_GRID_SPARSE)
+    plan.async_status()
+    backup = grid.clone()
+    for flags, n in ((ws.WS_FFT_USE_OCCUPANCY, 40), (0, 10)):
+        ref = None
+        for i in range(n):
+            grid.copy_(backup)
+            plan.fft_columns(grid, flags)
+            if ref is None:
+                ref = grid.clone()
+            else:
+                assert torch.equal(torch.view_as_real(grid).view(torch.int32), torch.view_as_real(ref).view(torch.int32)), \
+                    f"column passes (fft_flags = {flags}) differ at launch {i}"
+
+
 def test_library_fft_flag_and_occupancy_rules(oracle):
     import paper_2301_06061_b200 as ws
     d = make_random_dataset(31, 3000, 1, 256, 4, 7, fill=0.7, w_span=30.0, cell_rad=2e-3)
