@@ -433,6 +433,7 @@ k_fft_colB(float2* __restrict__ grid, const float2* __restrict__ tw, const uint3
 constexpr uint32_t COL_LAG_ITEMS = 768;      // in items of 64 KB (8-warp CTAs: x 8 / W for W warps).  Measured on Large (bands of 2 MB, 64 such
                                              // items) with 8-warp CTAs: 6 bands 6.55 ms, 10-16 bands 5.8, 24: 5.9, 48: 6.7 (L2 overflows);
                                              // Extreme (4 MB, 128 items): 2 bands 20.4 ms, 4-6: 16.1, 12: 16.5, 24: 18.8
+                                             // With 4-warp CTAs: Large 10-12 bands 5.26 ms, 16: 5.30, 20: 5.43; Extreme 3: 15.3, 4: 14.5, 6: 14.4, 8: 14.6, 10: 15.0
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     uint32_t v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
