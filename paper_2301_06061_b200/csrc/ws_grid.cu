@@ -22,8 +22,8 @@
 //     tile its footprint reaches and let one owner store each tile: 1.41 records per visibility on Large, 1.56
 //     with S = 9.)
 //   * a bin with more than WS_CHUNK records ("heavy": the dense core of the uv plane) is cut
-//     into chunks that become work items of their own (k_prepare_heavy), interleaved with the tiles in ONE
-//     persistent kernel.
+//     into chunks that become work items of their own (k_prepare_heavy); ONE persistent kernel takes the chunks and
+//     then the other non-empty bins (a list k_prepare_heavy writes) from one work counter.
 #include "ws_internal.h"
 #include "ws_taps.cuh"
 
@@ -319,7 +319,8 @@ __device__ __forceinline__ void flush_ring(const WsGeom& g, const WarpSmem<S>& s
     __syncwarp();
 }
 
-// Persistent kernel, one CTA per SM: warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved.
+// Persistent kernel, one CTA per SM of independent warps.  The warps take their work from one counter (WS_GRID_OVERWRITE: by
+// a fixed stride over ALL bins, warp w takes tiles w, w + W, ... and items w, w + W, ..., interleaved -- it stores zeros too).
 // bin_start: offsets of the record lists (one record per visibility, in its home bin); occ_start: home + halo counts,
 // scanned -- a tile whose entry does not grow receives nothing, and WS_GRID_OVERWRITE stores its zeros here (every other
 // tile was cleared by k_prepare_heavy, or holds what earlier calls put there, and is only ever added to).
